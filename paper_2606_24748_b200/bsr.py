@@ -1,0 +1,336 @@
+"""Python binding of libbsramg.so (include/bsr_amg.h): argument marshalling only.
+
+Every step of the hot path runs in the library's CUDA kernels; torch is used here for device memory and the
+stream only.  There is no CPU fallback: importing works anywhere, but every compute call needs the compiled
+library and a CUDA device and raises otherwise.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+from . import build as _build
+
+_lib = None
+
+ERRORS = {1: "NULL", 2: "SHAPE", 3: "BLOCK", 4: "STRUCTURE", 5: "ALLOC", 6: "CUDA", 7: "PLAN", 8: "ALIGN",
+          9: "NUMERIC", 10: "LIMIT"}
+
+# every symbol include/bsr_amg.h declares: name -> (restype, argtypes)
+_V, _I32, _I64, _D = C.c_void_p, C.c_int32, C.c_int64, C.c_double
+_PV, _PI32, _PI64 = C.POINTER(C.c_void_p), C.POINTER(C.c_int32), C.POINTER(C.c_int64)
+SYMBOLS = {
+    "bsr_last_error": (C.c_char_p, []),
+    "bsr_create": (C.c_int, [_PV, _I32, _I32, _I32, _I32, _I64, _V, _V, _V, _V]),
+    "bsr_values_changed": (C.c_int, [_V]),
+    "bsr_destroy": (C.c_int, [_V]),
+    "bsr_get_info": (C.c_int, [_V, _PI32, _PI32, _PI32, _PI32, _PI64, _PI64]),
+    "bsr_spmv": (C.c_int, [_V, _V, _V, _V]),
+    "bsr_spmv_t": (C.c_int, [_V, _V, _V, _V]),
+    "bsr_transpose_prepare": (C.c_int, [_V, _PI64, _V]),
+    "bsr_spmv_host": (C.c_int, [_V, _I32, _V, _V, _V]),
+    "bsr_spmv_bytes": (C.c_int64, [_V]),
+    "ptap_symbolic": (C.c_int, [_PV, _V, _V, _PI32, _PI64, _V]),
+    "ptap_structure": (C.c_int, [_V, _V, _V, _V]),
+    "ptap_numeric": (C.c_int, [_V, _V, _V, _V, _V]),
+    "ptap_get_info": (C.c_int, [_V, _PI64, _PI64, _PI64, _PI64, _PI64]),
+    "ptap_numeric_stage": (C.c_int, [_V, _I32, _V, _V, _V, _V]),
+    "ptap_get_ap": (C.c_int, [_V, _PV, _PV, _PV]),
+    "ptap_numeric_host": (C.c_int, [_V, _V, _V, _V, _V, _V, _V]),
+    "ptap_destroy": (C.c_int, [_V]),
+    "ptap_host_plan_build": (C.c_void_p, [_I32, _V, _V, _I32, _V, _V]),
+    "ptap_host_plan_get": (C.c_int, [_V, C.c_char_p, _PV, _PI64, _PI32]),
+    "ptap_host_plan_free": (None, [_V]),
+    "vcycle_create": (C.c_int, [_PV, _I32, _PV, _PV, C.POINTER(_D), _I32, _D, _D, _V]),
+    "vcycle_refresh": (C.c_int, [_V, _V]),
+    "vcycle_status": (C.c_int, [_V, _V]),
+    "vcycle_apply": (C.c_int, [_V, _V, _V, _V]),
+    "vcycle_smooth": (C.c_int, [_V, _I32, _V, _V, _V]),
+    "pcg_solve": (C.c_int, [_V, _V, _V, _I32, _V, _V]),
+    "vcycle_apply_host": (C.c_int, [_V, _V, _V, _V]),
+    "vcycle_destroy": (C.c_int, [_V]),
+    "bsr_counters": (C.c_int, [_PI64, _PI64]),
+}
+
+
+class BsrError(RuntimeError):
+    def __init__(self, code: int, msg: str):
+        super().__init__(f"libbsramg error {code} ({ERRORS.get(code, '?')}): {msg}")
+        self.code = code
+
+
+def lib():
+    """Loads (building if stale) the CUDA library.  Fails loudly when it cannot be built or loaded."""
+    global _lib
+    if _lib is None:
+        path = _build.build_cuda()
+        L = C.CDLL(path)
+        for name, (res, args) in SYMBOLS.items():
+            f = getattr(L, name)  # AttributeError if the library does not export a declared symbol
+            f.restype, f.argtypes = res, args
+        _lib = L
+    return _lib
+
+
+def _check(rc: int):
+    if rc != 0:
+        raise BsrError(rc, lib().bsr_last_error().decode())
+
+
+def _stream() -> int:
+    import torch
+    return int(torch.cuda.current_stream().cuda_stream)
+
+
+def _dev(t):
+    """Device pointer of a torch CUDA tensor (None -> null)."""
+    if t is None:
+        return None
+    assert t.is_cuda and t.is_contiguous()
+    return C.c_void_p(t.data_ptr())
+
+
+def counters():
+    a, b = C.c_int64(), C.c_int64()
+    lib().bsr_counters(C.byref(a), C.byref(b))
+    return a.value, b.value
+
+
+class Bsr:
+    """A block-CSR matrix on the device (bsr_create).  Keeps the torch tensors it borrows alive."""
+
+    def __init__(self, nbrows, nbcols, bs_r, bs_c, rowptr, colidx, vals):
+        import torch
+        self.nbrows, self.nbcols, self.bs_r, self.bs_c = int(nbrows), int(nbcols), int(bs_r), int(bs_c)
+        self.rowptr, self.colidx, self.vals = rowptr, colidx, vals
+        assert rowptr.dtype == torch.int32 and colidx.dtype == torch.int32 and vals.dtype == torch.float64
+        self.nnzb = int(colidx.numel())
+        h = C.c_void_p()
+        _check(lib().bsr_create(C.byref(h), self.nbrows, self.nbcols, self.bs_r, self.bs_c, self.nnzb, _dev(rowptr),
+                                _dev(colidx), _dev(vals), _stream()))
+        self.h = h
+
+    @classmethod
+    def from_host(cls, M, device="cuda"):
+        """Upload a host matrix (any object with nbrows, nbcols, bs_r, bs_c, rowptr, colidx, vals numpy arrays)."""
+        import torch
+        rp = torch.from_numpy(np.ascontiguousarray(M.rowptr, dtype=np.int32)).to(device)
+        ci = torch.from_numpy(np.ascontiguousarray(M.colidx, dtype=np.int32)).to(device)
+        va = torch.from_numpy(np.ascontiguousarray(M.vals, dtype=np.float64).reshape(-1)).to(device)
+        return cls(M.nbrows, M.nbcols, M.bs_r, M.bs_c, rp, ci, va)
+
+    def close(self):
+        if getattr(self, "h", None):
+            lib().bsr_destroy(self.h)
+            self.h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def values_changed(self):
+        _check(lib().bsr_values_changed(self.h))
+
+    def set_values(self, host_vals):
+        """Rewrite the values in place from a host array and bump the state counter."""
+        import torch
+        self.vals.copy_(torch.from_numpy(np.ascontiguousarray(host_vals, dtype=np.float64).reshape(-1)))
+        self.values_changed()
+
+    @property
+    def state(self) -> int:
+        s = C.c_int64()
+        _check(lib().bsr_get_info(self.h, None, None, None, None, None, C.byref(s)))
+        return s.value
+
+    def spmv_bytes(self) -> int:
+        return int(lib().bsr_spmv_bytes(self.h))
+
+    def spmv(self, x, y=None):
+        """y = A x (bsr_spmv)."""
+        import torch
+        if y is None:
+            y = torch.empty(self.nbrows * self.bs_r, dtype=torch.float64, device=x.device)
+        assert x.numel() == self.nbcols * self.bs_c and y.numel() == self.nbrows * self.bs_r
+        _check(lib().bsr_spmv(self.h, _dev(x), _dev(y), _stream()))
+        return y
+
+    def spmv_t(self, x, y=None):
+        """y = A^T x on the cached explicit transpose (bsr_spmv_t)."""
+        import torch
+        if y is None:
+            y = torch.empty(self.nbcols * self.bs_c, dtype=torch.float64, device=x.device)
+        assert x.numel() == self.nbrows * self.bs_r and y.numel() == self.nbcols * self.bs_c
+        _check(lib().bsr_spmv_t(self.h, _dev(x), _dev(y), _stream()))
+        return y
+
+    def transpose_prepare(self) -> int:
+        n = C.c_int64()
+        _check(lib().bsr_transpose_prepare(self.h, C.byref(n), _stream()))
+        return n.value
+
+    def spmv_host(self, h_x: np.ndarray, h_y: np.ndarray, trans: bool = False):
+        """End to end with host vectors (bsr_spmv_host)."""
+        assert h_x.dtype == np.float64 and h_y.dtype == np.float64
+        _check(lib().bsr_spmv_host(self.h, 1 if trans else 0, h_x.ctypes.data, h_y.ctypes.data, _stream()))
+        return h_y
+
+
+class PtapPlan:
+    """Cached symbolic structure and block coordinate plan of A_c = P^T A P (ptap_symbolic)."""
+
+    def __init__(self, A: Bsr, P: Bsr):
+        import torch
+        self.A, self.P = A, P
+        h, nbr, nnz = C.c_void_p(), C.c_int32(), C.c_int64()
+        _check(lib().ptap_symbolic(C.byref(h), A.h, P.h, C.byref(nbr), C.byref(nnz), _stream()))
+        self.h = h
+        self.nbrows_c, self.nnzb_c, self.bs_c = nbr.value, nnz.value, P.bs_c
+        dev = A.vals.device
+        self.rowptr_c = torch.empty(self.nbrows_c + 1, dtype=torch.int32, device=dev)
+        self.colidx_c = torch.empty(self.nnzb_c, dtype=torch.int32, device=dev)
+        _check(lib().ptap_structure(self.h, _dev(self.rowptr_c), _dev(self.colidx_c), _stream()))
+
+    def close(self):
+        if getattr(self, "h", None):
+            lib().ptap_destroy(self.h)
+            self.h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def info(self) -> dict:
+        v = [C.c_int64() for _ in range(5)]
+        _check(lib().ptap_get_info(self.h, *[C.byref(t) for t in v]))
+        return dict(nnzb_ap=v[0].value, n_products_1=v[1].value, n_products_2=v[2].value,
+                    algorithmic_bytes=v[3].value, n_r_value_builds=v[4].value)
+
+    def new_values(self):
+        import torch
+        return torch.empty(self.nnzb_c * self.bs_c * self.bs_c, dtype=torch.float64, device=self.A.vals.device)
+
+    def numeric(self, vals_c=None):
+        """vals_c = values of P^T A P for the current values of A and P (ptap_numeric)."""
+        if vals_c is None:
+            vals_c = self.new_values()
+        _check(lib().ptap_numeric(self.h, self.A.h, self.P.h, _dev(vals_c), _stream()))
+        return vals_c
+
+    def numeric_stage(self, stage: int, vals_c=None):
+        _check(lib().ptap_numeric_stage(self.h, stage, self.A.h, self.P.h, _dev(vals_c), _stream()))
+
+    def numeric_host(self, h_vals_a: np.ndarray, h_vals_c: np.ndarray, vals_c):
+        _check(lib().ptap_numeric_host(self.h, self.A.h, self.P.h, h_vals_a.ctypes.data, h_vals_c.ctypes.data,
+                                       _dev(vals_c), _stream()))
+        return h_vals_c
+
+    def coarse_matrix(self, vals_c) -> Bsr:
+        """Wrap A_c (structure of the plan, given values) as a Bsr."""
+        return Bsr(self.nbrows_c, self.nbrows_c, self.bs_c, self.bs_c, self.rowptr_c, self.colidx_c, vals_c)
+
+    def ap_host(self):
+        """(rowptr, colidx, vals) of the cached AP copied to the host (tests)."""
+        import torch
+        info = self.info()
+        n, bf, bc = info["nnzb_ap"], self.A.bs_r, self.P.bs_c
+        p = [C.c_void_p() for _ in range(3)]
+        _check(lib().ptap_get_ap(self.h, *[C.byref(t) for t in p]))
+        torch.cuda.synchronize()
+        out = [np.empty(self.A.nbrows + 1, np.int32), np.empty(n, np.int32), np.empty(n * bf * bc, np.float64)]
+        cudart = torch.cuda.cudart()
+        for dst, src in zip(out, p):
+            if dst.nbytes:
+                rc = cudart.cudaMemcpy(dst.ctypes.data, src.value, dst.nbytes, 2)  # cudaMemcpyDeviceToHost
+                assert int(rc) == 0 if not isinstance(rc, tuple) else int(rc[0]) == 0
+        return out[0], out[1], out[2].reshape(n, bf, bc)
+
+
+class HostPlan:
+    """The host (integer) part of ptap_symbolic on host arrays -- usable without a GPU (tests of the plan)."""
+    NAMES = ["rowptr_ap", "colidx_ap", "rowidx_ap", "rowptr_c", "colidx_c", "rowidx_c", "rowptr_r", "colidx_r",
+             "perm_r", "pairptr1", "k1", "q1", "pstart", "pairptr2", "t2", "s2", "apstart"]
+
+    def __init__(self, A, P):
+        ra, ca = np.ascontiguousarray(A.rowptr, np.int32), np.ascontiguousarray(A.colidx, np.int32)
+        rp, cp = np.ascontiguousarray(P.rowptr, np.int32), np.ascontiguousarray(P.colidx, np.int32)
+        h = lib().ptap_host_plan_build(A.nbrows, ra.ctypes.data, ca.ctypes.data, P.nbcols, rp.ctypes.data,
+                                       cp.ctypes.data)
+        if not h:
+            raise BsrError(-1, lib().bsr_last_error().decode())
+        try:
+            for name in self.NAMES:
+                ptr, cnt, eb = C.c_void_p(), C.c_int64(), C.c_int32()
+                _check(lib().ptap_host_plan_get(h, name.encode(), C.byref(ptr), C.byref(cnt), C.byref(eb)))
+                dt = np.int32 if eb.value == 4 else np.uint16
+                if cnt.value:
+                    buf = (C.c_char * (cnt.value * eb.value)).from_address(ptr.value)
+                    arr = np.frombuffer(buf, dtype=dt).copy()
+                else:
+                    arr = np.empty(0, dt)
+                setattr(self, name, arr)
+        finally:
+            lib().ptap_host_plan_free(h)
+
+
+class VCycle:
+    """V-cycle preconditioner over a hierarchy of Bsr operators and prolongators (vcycle_create)."""
+
+    def __init__(self, As, Ps, lambdas, cheb_degree: int = 2, lo: float = 0.1, hi: float = 1.1):
+        assert len(Ps) == len(As) - 1 and len(lambdas) >= len(Ps)
+        self.As, self.Ps = list(As), list(Ps)
+        n = len(As)
+        a = (C.c_void_p * n)(*[A.h for A in As])
+        p = (C.c_void_p * max(n - 1, 1))(*[P.h for P in Ps])
+        lam = (C.c_double * max(n - 1, 1))(*[float(v) for v in lambdas[:n - 1]])
+        h = C.c_void_p()
+        _check(lib().vcycle_create(C.byref(h), n, a, p, lam, cheb_degree, lo, hi, _stream()))
+        self.h = h
+        self.n = As[0].nbrows * As[0].bs_r
+
+    def close(self):
+        if getattr(self, "h", None):
+            lib().vcycle_destroy(self.h)
+            self.h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def refresh(self, check: bool = True):
+        _check(lib().vcycle_refresh(self.h, _stream()))
+        if check:
+            _check(lib().vcycle_status(self.h, _stream()))
+
+    def apply(self, b, x=None):
+        """x = M^-1 b, one V-cycle from a zero guess (vcycle_apply)."""
+        import torch
+        if x is None:
+            x = torch.empty_like(b)
+        assert b.numel() == self.n and x.numel() == self.n
+        _check(lib().vcycle_apply(self.h, _dev(b), _dev(x), _stream()))
+        return x
+
+    def smooth(self, level: int, b, x):
+        _check(lib().vcycle_smooth(self.h, level, _dev(b), _dev(x), _stream()))
+        return x
+
+    def pcg(self, b, iters: int = 20):
+        """(x, residual history) of `iters` PCG iterations with the V-cycle as preconditioner (pcg_solve)."""
+        import torch
+        x = torch.empty_like(b)
+        hist = torch.empty(iters + 1, dtype=torch.float64, device=b.device)
+        _check(lib().pcg_solve(self.h, _dev(b), _dev(x), iters, _dev(hist), _stream()))
+        return x, hist
+
+    def apply_host(self, h_b: np.ndarray, h_x: np.ndarray):
+        _check(lib().vcycle_apply_host(self.h, h_b.ctypes.data, h_x.ctypes.data, _stream()))
+        return h_x

@@ -1,0 +1,443 @@
+// bsr.cu -- the block-CSR container, the blocked SpMV family and the cached explicit transpose.
+//
+// Container: PAPER.md:20-28, 62-66 (block-CSR with independent bs_r x bs_c).  SpMV: PAPER.md:22, 121, 140-147
+// (bandwidth-bound; 8*bs_r*bs_c + 4 bytes per block).  Transpose cache: PAPER.md:103 ("the transpose R", rebuilt
+// only when the prolongator's state changes).
+//
+// SpMV kernel design (sm_100a, HBM-bound, no tensor cores -- DESIGN.md "Kernels"):
+//   A lane GROUP of LB = bs_r * (bs_c / VW) lanes owns one stored block per step; lane (r, cv) of the group loads
+//   VW consecutive doubles of block row r (VW = 2 -> one 16-byte load when bs_c is even, else one 8-byte load), the
+//   matching VW entries of x, and keeps ONE accumulator for output row r.  Consecutive lanes read consecutive
+//   addresses, so a group's load is one contiguous bs_r*bs_c*8-byte run and the GPW = 32/LB groups of a warp read
+//   GPW consecutive blocks (TEAM mode, long rows: the whole warp on one block row) or GPW different block rows
+//   (ROW mode, short rows such as the prolongator's).  The row sum is finished with warp shuffles in a fixed order
+//   (deterministic); the epilogue (y = Ax, y = b - Ax, y -= Ax, y += Ax) is fused into the store.
+#include <algorithm>
+#include <cstring>
+
+#include "internal.h"
+
+namespace bsramg {
+
+thread_local std::string t_err = "";
+std::atomic<int64_t> g_launches{0};
+std::atomic<int64_t> g_allocs{0};
+
+int fail(int code, const char* fmt, ...) {
+  char buf[512];
+  va_list ap;
+  va_start(ap, fmt);
+  vsnprintf(buf, sizeof buf, fmt, ap);
+  va_end(ap);
+  t_err = buf;
+  return code;
+}
+
+int dev_alloc(void** p, size_t bytes) {
+  *p = nullptr;
+  cudaError_t e = cudaMalloc(p, bytes ? bytes : 16);
+  if (e != cudaSuccess) {
+    cudaGetLastError();
+    return fail(e == cudaErrorMemoryAllocation ? BSR_ERR_ALLOC : BSR_ERR_CUDA, "cudaMalloc(%zu): %s", bytes,
+                cudaGetErrorString(e));
+  }
+  g_allocs.fetch_add(1, std::memory_order_relaxed);
+  return BSR_OK;
+}
+void dev_free(void* p) {
+  if (p) cudaFree(p);
+}
+
+// ------------------------------------------------------------------ lane mapping of one block shape
+template <int BR, int BC>
+struct Shape {
+  static constexpr int VW = (BC % 2 == 0) ? 2 : 1;  // doubles per load
+  static constexpr int LPR = BC / VW;               // lanes per block row
+  static constexpr int LB = BR * LPR;               // lanes per block
+  static constexpr int GPW = 32 / LB;               // lane groups per warp
+  static constexpr int BB = BR * BC;
+};
+
+template <int VW>
+struct Vec;
+template <>
+struct Vec<1> {
+  double a;
+  __device__ __forceinline__ static Vec stream(const double* p) { return {__ldcs(p)}; }
+  __device__ __forceinline__ static Vec cached(const double* p) { return {__ldg(p)}; }
+  __device__ __forceinline__ static Vec zero() { return {0.0}; }
+  __device__ __forceinline__ double dot(const Vec& o, double acc) const { return fma(a, o.a, acc); }
+};
+template <>
+struct Vec<2> {
+  double a, b;
+  __device__ __forceinline__ static Vec stream(const double* p) {
+    double2 v = __ldcs(reinterpret_cast<const double2*>(p));
+    return {v.x, v.y};
+  }
+  __device__ __forceinline__ static Vec cached(const double* p) {
+    double2 v = __ldg(reinterpret_cast<const double2*>(p));
+    return {v.x, v.y};
+  }
+  __device__ __forceinline__ static Vec zero() { return {0.0, 0.0}; }
+  __device__ __forceinline__ double dot(const Vec& o, double acc) const { return fma(b, o.b, fma(a, o.a, acc)); }
+};
+
+// y (op)= A x.  TEAM = number of lane groups that share one block row (1 or GPW).  U = blocks in flight per group.
+template <int BR, int BC, int TEAM, int U, int EPI>
+__global__ void __launch_bounds__(256)
+spmv_kernel(int32_t nbrows, const int32_t* __restrict__ rowptr, const int32_t* __restrict__ colidx,
+            const double* __restrict__ vals, const double* __restrict__ x, double* __restrict__ y,
+            const double* __restrict__ b) {
+  using S = Shape<BR, BC>;
+  constexpr int ROWS_PER_WARP = S::GPW / TEAM;
+  const int lane = threadIdx.x & 31;
+  const int64_t warp = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+  const int g = lane / S::LB;  // lane group
+  const int q = lane % S::LB;  // lane inside the group
+  const int r = q / S::LPR;    // block row of this lane
+  const int cv = q % S::LPR;   // which VW-wide piece of the block row
+  const int team = g / TEAM, member = g % TEAM;
+  const int64_t row = warp * ROWS_PER_WARP + team;
+  const bool live = (g < ROWS_PER_WARP * TEAM) && (row < nbrows);
+
+  double acc = 0.0;
+  if (live) {
+    const int32_t k1 = rowptr[row + 1];
+    const int lane_off = r * BC + cv * S::VW;
+    for (int32_t k = rowptr[row] + member; k < k1; k += TEAM * U) {
+      int32_t col[U];
+      Vec<S::VW> v[U], xv[U];
+#pragma unroll
+      for (int u = 0; u < U; ++u) {
+        const int32_t ku = k + u * TEAM;
+        col[u] = (ku < k1) ? __ldg(colidx + ku) : 0;
+      }
+#pragma unroll
+      for (int u = 0; u < U; ++u) {
+        const int32_t ku = k + u * TEAM;
+        v[u] = (ku < k1) ? Vec<S::VW>::stream(vals + (int64_t)ku * S::BB + lane_off) : Vec<S::VW>::zero();
+      }
+#pragma unroll
+      for (int u = 0; u < U; ++u) xv[u] = Vec<S::VW>::cached(x + (int64_t)col[u] * BC + cv * S::VW);
+#pragma unroll
+      for (int u = 0; u < U; ++u) acc = v[u].dot(xv[u], acc);
+    }
+  }
+  // sum the LPR pieces of a block row (adjacent lanes), then the TEAM groups (lanes LB apart); fixed order
+  if (S::LPR == 3) {
+    const double t1 = __shfl_down_sync(0xffffffffu, acc, 1);
+    const double t2 = __shfl_down_sync(0xffffffffu, acc, 2);
+    acc = (acc + t1) + t2;
+  } else if (S::LPR == 2) {
+    acc += __shfl_down_sync(0xffffffffu, acc, 1);
+  }
+#pragma unroll
+  for (int s = 1; s < TEAM; s <<= 1) {
+    const double t = __shfl_down_sync(0xffffffffu, acc, (s * S::LB) & 31);
+    if (member + s < TEAM) acc += t;
+  }
+  if (live && cv == 0 && member == 0) {
+    const int64_t o = row * BR + r;
+    if (EPI == EPI_ASSIGN) y[o] = acc;
+    else if (EPI == EPI_RESID) y[o] = b[o] - acc;
+    else if (EPI == EPI_SUB) y[o] = y[o] - acc;
+    else y[o] = y[o] + acc;
+  }
+}
+
+template <int BR, int BC, int TEAM, int U>
+static int spmv_dispatch_epi(bsr_t A, const double* x, double* y, const double* b, Epilogue epi, cudaStream_t st) {
+  using S = Shape<BR, BC>;
+  constexpr int ROWS_PER_WARP = S::GPW / TEAM;
+  const int64_t warps = ((int64_t)A->nbrows + ROWS_PER_WARP - 1) / ROWS_PER_WARP;
+  const int64_t blocks = (warps + 7) / 8;
+  if (blocks == 0) return BSR_OK;
+  if (blocks > 0x7fffffffLL) return fail(BSR_ERR_LIMIT, "grid too large");
+  const dim3 grid((unsigned)blocks), block(256);
+  switch (epi) {
+    case EPI_ASSIGN:
+      LAUNCH((spmv_kernel<BR, BC, TEAM, U, EPI_ASSIGN>), grid, block, 0, st, A->nbrows, A->d_rowptr, A->d_colidx,
+             A->d_vals, x, y, b);
+      break;
+    case EPI_RESID:
+      LAUNCH((spmv_kernel<BR, BC, TEAM, U, EPI_RESID>), grid, block, 0, st, A->nbrows, A->d_rowptr, A->d_colidx,
+             A->d_vals, x, y, b);
+      break;
+    case EPI_SUB:
+      LAUNCH((spmv_kernel<BR, BC, TEAM, U, EPI_SUB>), grid, block, 0, st, A->nbrows, A->d_rowptr, A->d_colidx,
+             A->d_vals, x, y, b);
+      break;
+    default:
+      LAUNCH((spmv_kernel<BR, BC, TEAM, U, EPI_ADD>), grid, block, 0, st, A->nbrows, A->d_rowptr, A->d_colidx,
+             A->d_vals, x, y, b);
+      break;
+  }
+  return BSR_OK;
+}
+
+template <int BR, int BC>
+static int spmv_dispatch_team(bsr_t A, const double* x, double* y, const double* b, Epilogue epi, cudaStream_t st) {
+  using S = Shape<BR, BC>;
+  constexpr int U = (S::GPW == 1) ? 8 : 4;
+  if (S::GPW > 1 && A->team_mode == 1) return spmv_dispatch_epi<BR, BC, S::GPW, U>(A, x, y, b, epi, st);
+  return spmv_dispatch_epi<BR, BC, 1, U>(A, x, y, b, epi, st);
+}
+
+int spmv_launch(bsr_t A, const double* x, double* y, const double* b, Epilogue epi, cudaStream_t st) {
+  if (((uintptr_t)x | (uintptr_t)y | (uintptr_t)b) & 15) return fail(BSR_ERR_ALIGN, "vector pointer not 16-byte aligned");
+  const int key = A->bs_r * 10 + A->bs_c;
+  switch (key) {
+    case 22: return spmv_dispatch_team<2, 2>(A, x, y, b, epi, st);
+    case 23: return spmv_dispatch_team<2, 3>(A, x, y, b, epi, st);
+    case 32: return spmv_dispatch_team<3, 2>(A, x, y, b, epi, st);
+    case 33: return spmv_dispatch_team<3, 3>(A, x, y, b, epi, st);
+    case 36: return spmv_dispatch_team<3, 6>(A, x, y, b, epi, st);
+    case 63: return spmv_dispatch_team<6, 3>(A, x, y, b, epi, st);
+    case 66: return spmv_dispatch_team<6, 6>(A, x, y, b, epi, st);
+  }
+  return fail(BSR_ERR_BLOCK, "unsupported block shape %dx%d", A->bs_r, A->bs_c);
+}
+
+// ------------------------------------------------------------------ cached explicit transpose
+void host_transpose_structure(int32_t nbrows, int32_t nbcols, const int32_t* rowptr, const int32_t* colidx,
+                              std::vector<int32_t>& rowptr_t, std::vector<int32_t>& colidx_t,
+                              std::vector<int32_t>& perm) {
+  const int64_t nnzb = rowptr[nbrows];
+  rowptr_t.assign((size_t)nbcols + 1, 0);
+  colidx_t.resize((size_t)nnzb);
+  perm.resize((size_t)nnzb);
+  for (int64_t k = 0; k < nnzb; ++k) rowptr_t[(size_t)colidx[k] + 1]++;
+  for (int32_t j = 0; j < nbcols; ++j) rowptr_t[(size_t)j + 1] += rowptr_t[j];
+  std::vector<int32_t> fill(rowptr_t.begin(), rowptr_t.end() - 1);
+  // rows visited in ascending order -> every transposed row comes out sorted by column
+  for (int32_t i = 0; i < nbrows; ++i)
+    for (int32_t k = rowptr[i]; k < rowptr[i + 1]; ++k) {
+      const int32_t t = fill[colidx[k]]++;
+      colidx_t[t] = i;
+      perm[t] = k;
+    }
+}
+
+// T.vals[t] = (vals[perm[t]])^T ; one thread per value of T (coalesced writes)
+__global__ void __launch_bounds__(256)
+transpose_values_kernel(int64_t nvals, int br, int bc, const int32_t* __restrict__ perm,
+                        const double* __restrict__ vals, double* __restrict__ tvals) {
+  const int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (e >= nvals) return;
+  const int bb = br * bc;
+  const int64_t t = e / bb;
+  const int pos = (int)(e - t * bb);  // position in the bc x br transposed block
+  const int c = pos / br, r = pos - c * br;
+  tvals[e] = __ldg(vals + (int64_t)__ldg(perm + t) * bb + r * bc + c);
+}
+
+static void choose_team_mode(bsr_t A) {
+  // the whole warp shares a row only when the row keeps every lane group busy for a few steps
+  int gpw = 1;
+  switch (A->bs_r * 10 + A->bs_c) {
+    case 22: gpw = 16; break;
+    case 23: gpw = 5; break;
+    case 32: gpw = 10; break;
+    case 33: gpw = 3; break;
+    case 36: gpw = 3; break;
+    default: gpw = 1;
+  }
+  A->team_mode = (gpw > 1 && A->avg_row_len >= 2.0 * gpw) ? 1 : 0;
+}
+
+int transpose_ensure(bsr_t A, cudaStream_t st) {
+  if (!A->T) {  // cold: build the structure on the host from the mirror taken at bsr_create
+    std::vector<int32_t> rp, ci, perm;
+    host_transpose_structure(A->nbrows, A->nbcols, A->h_rowptr.data(), A->h_colidx.data(), rp, ci, perm);
+    bsr_matrix_s* T = new (std::nothrow) bsr_matrix_s();
+    if (!T) return fail(BSR_ERR_ALLOC, "host allocation failed");
+    T->nbrows = A->nbcols; T->nbcols = A->nbrows; T->bs_r = A->bs_c; T->bs_c = A->bs_r; T->nnzb = A->nnzb;
+    T->magic = BSR_MAGIC; T->owns_arrays = true;
+    int32_t *d_rp = nullptr, *d_ci = nullptr;
+    int rc = upload(&d_rp, rp, st);
+    if (rc == BSR_OK) rc = upload(&d_ci, ci, st);
+    if (rc == BSR_OK) rc = upload(&A->T_perm, perm, st);
+    if (rc == BSR_OK) rc = dev_alloc_t(&T->d_vals, (size_t)A->nnzb * A->bs_r * A->bs_c);
+    T->d_rowptr = d_rp; T->d_colidx = d_ci;
+    if (rc == BSR_OK && cudaStreamSynchronize(st) != cudaSuccess) rc = fail(BSR_ERR_CUDA, "transpose upload failed");
+    if (rc != BSR_OK) {
+      dev_free(d_rp); dev_free(d_ci); dev_free(A->T_perm); dev_free(T->d_vals);
+      A->T_perm = nullptr;
+      delete T;
+      return rc;
+    }
+    int32_t mx = 0;
+    for (int32_t j = 0; j < T->nbrows; ++j) mx = std::max(mx, rp[(size_t)j + 1] - rp[j]);
+    T->max_row_len = mx;
+    T->avg_row_len = T->nbrows ? (double)T->nnzb / T->nbrows : 0.0;
+    T->h_rowptr.swap(rp);
+    T->h_colidx.swap(ci);
+    choose_team_mode(T);
+    A->T = T;
+    A->T_state = -1;
+  }
+  if (A->T_state != A->state) {  // state gate: values re-transposed on the device only when A's values moved
+    const int64_t nvals = A->nnzb * A->bs_r * A->bs_c;
+    if (nvals > 0)
+      LAUNCH(transpose_values_kernel, (unsigned)((nvals + 255) / 256), 256, 0, st, nvals, (int)A->bs_r, (int)A->bs_c,
+             A->T_perm, A->d_vals, A->T->d_vals);
+    A->T_state = A->state;
+    A->T_builds++;
+    A->T->state++;
+  }
+  return BSR_OK;
+}
+
+static bool valid(bsr_t A) { return A && A->magic == BSR_MAGIC; }
+
+}  // namespace bsramg
+
+using namespace bsramg;
+
+// =================================================================== C ABI
+extern "C" {
+
+const char* bsr_last_error(void) { return t_err.c_str(); }
+
+int bsr_counters(int64_t* n_kernel_launches, int64_t* n_allocs) {
+  if (n_kernel_launches) *n_kernel_launches = g_launches.load();
+  if (n_allocs) *n_allocs = g_allocs.load();
+  return BSR_OK;
+}
+
+int bsr_create(bsr_t* out, int32_t nbrows, int32_t nbcols, int32_t bs_r, int32_t bs_c, int64_t nnzb,
+               const int32_t* d_rowptr, const int32_t* d_colidx, double* d_vals, void* stream) {
+  if (!out) return fail(BSR_ERR_NULL, "bsr_create: out is null");
+  *out = nullptr;
+  if (!d_rowptr || (nnzb > 0 && (!d_colidx || !d_vals))) return fail(BSR_ERR_NULL, "bsr_create: null array");
+  if (nbrows < 0 || nbcols < 0 || nnzb < 0) return fail(BSR_ERR_SHAPE, "bsr_create: negative size");
+  if (!shape_supported(bs_r, bs_c)) return fail(BSR_ERR_BLOCK, "unsupported block shape %dx%d", bs_r, bs_c);
+  if (nnzb * bs_r * bs_c >= (1LL << 31)) return fail(BSR_ERR_LIMIT, "nnzb*bs_r*bs_c >= 2^31");
+  if ((uintptr_t)d_vals & 15) return fail(BSR_ERR_ALIGN, "d_vals not 16-byte aligned");
+  cudaStream_t st = (cudaStream_t)stream;
+  bsr_matrix_s* A = new (std::nothrow) bsr_matrix_s();
+  if (!A) return fail(BSR_ERR_ALLOC, "host allocation failed");
+  A->h_rowptr.resize((size_t)nbrows + 1);
+  A->h_colidx.resize((size_t)nnzb);
+  cudaError_t e = cudaMemcpyAsync(A->h_rowptr.data(), d_rowptr, ((size_t)nbrows + 1) * 4, cudaMemcpyDeviceToHost, st);
+  if (e == cudaSuccess && nnzb)
+    e = cudaMemcpyAsync(A->h_colidx.data(), d_colidx, (size_t)nnzb * 4, cudaMemcpyDeviceToHost, st);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+  if (e != cudaSuccess) {
+    delete A;
+    cudaGetLastError();
+    return fail(BSR_ERR_CUDA, "bsr_create: structure copy failed: %s", cudaGetErrorString(e));
+  }
+  // validation of the canonical form
+  const int32_t* rp = A->h_rowptr.data();
+  const int32_t* ci = A->h_colidx.data();
+  int bad = 0;
+  if (rp[0] != 0 || (int64_t)rp[nbrows] != nnzb) bad = 1;
+  int32_t mx = 0;
+  if (!bad) {
+#pragma omp parallel for schedule(static) reduction(max : mx) reduction(| : bad)
+    for (int32_t i = 0; i < nbrows; ++i) {
+      const int32_t a = rp[i], b = rp[i + 1];
+      if (b < a || a < 0 || (int64_t)b > nnzb) { bad |= 2; continue; }
+      mx = std::max(mx, b - a);
+      for (int32_t k = a; k < b; ++k) {
+        if (ci[k] < 0 || ci[k] >= nbcols) bad |= 4;
+        if (k > a && ci[k] <= ci[k - 1]) bad |= 8;
+      }
+    }
+  }
+  if (bad) {
+    delete A;
+    return fail(BSR_ERR_STRUCTURE, "malformed structure (%s%s%s%s)", (bad & 1) ? "rowptr ends " : "",
+                (bad & 2) ? "rowptr not monotone " : "", (bad & 4) ? "column out of range " : "",
+                (bad & 8) ? "columns not strictly ascending" : "");
+  }
+  A->nbrows = nbrows; A->nbcols = nbcols; A->bs_r = bs_r; A->bs_c = bs_c; A->nnzb = nnzb;
+  A->d_rowptr = d_rowptr; A->d_colidx = d_colidx; A->d_vals = d_vals;
+  A->magic = BSR_MAGIC;
+  A->max_row_len = mx;
+  A->avg_row_len = nbrows ? (double)nnzb / nbrows : 0.0;
+  choose_team_mode(A);
+  *out = A;
+  return BSR_OK;
+}
+
+int bsr_values_changed(bsr_t A) {
+  if (!valid(A)) return fail(BSR_ERR_NULL, "invalid matrix handle");
+  A->state++;
+  return BSR_OK;
+}
+
+int bsr_destroy(bsr_t A) {
+  if (!A) return BSR_OK;
+  if (A->magic != BSR_MAGIC) return fail(BSR_ERR_NULL, "invalid matrix handle");
+  if (A->T) {
+    dev_free((void*)A->T->d_rowptr); dev_free((void*)A->T->d_colidx); dev_free(A->T->d_vals);
+    A->T->magic = 0;
+    delete A->T;
+  }
+  dev_free(A->T_perm);
+  A->magic = 0;
+  delete A;
+  return BSR_OK;
+}
+
+int bsr_get_info(bsr_t A, int32_t* nbrows, int32_t* nbcols, int32_t* bs_r, int32_t* bs_c, int64_t* nnzb,
+                 int64_t* state) {
+  if (!valid(A)) return fail(BSR_ERR_NULL, "invalid matrix handle");
+  if (nbrows) *nbrows = A->nbrows;
+  if (nbcols) *nbcols = A->nbcols;
+  if (bs_r) *bs_r = A->bs_r;
+  if (bs_c) *bs_c = A->bs_c;
+  if (nnzb) *nnzb = A->nnzb;
+  if (state) *state = A->state;
+  return BSR_OK;
+}
+
+int64_t bsr_spmv_bytes(bsr_t A) {
+  if (!valid(A)) return -1;
+  return A->nnzb * (8LL * A->bs_r * A->bs_c + 4) + 4LL * (A->nbrows + 1) + 8LL * A->bs_c * A->nbcols +
+         8LL * A->bs_r * A->nbrows;
+}
+
+int bsr_spmv(bsr_t A, const double* d_x, double* d_y, void* stream) {
+  if (!valid(A)) return fail(BSR_ERR_NULL, "invalid matrix handle");
+  if (!d_x || !d_y) return fail(BSR_ERR_NULL, "null vector");
+  return spmv_launch(A, d_x, d_y, nullptr, EPI_ASSIGN, (cudaStream_t)stream);
+}
+
+int bsr_transpose_prepare(bsr_t A, int64_t* n_value_builds, void* stream) {
+  if (!valid(A)) return fail(BSR_ERR_NULL, "invalid matrix handle");
+  BSR_TRY(transpose_ensure(A, (cudaStream_t)stream));
+  if (n_value_builds) *n_value_builds = A->T_builds;
+  return BSR_OK;
+}
+
+int bsr_spmv_t(bsr_t A, const double* d_x, double* d_y, void* stream) {
+  if (!valid(A)) return fail(BSR_ERR_NULL, "invalid matrix handle");
+  if (!d_x || !d_y) return fail(BSR_ERR_NULL, "null vector");
+  BSR_TRY(transpose_ensure(A, (cudaStream_t)stream));
+  return spmv_launch(A->T, d_x, d_y, nullptr, EPI_ASSIGN, (cudaStream_t)stream);
+}
+
+int bsr_spmv_host(bsr_t A, int32_t trans, const double* h_x, double* h_y, void* stream) {
+  if (!valid(A)) return fail(BSR_ERR_NULL, "invalid matrix handle");
+  if (!h_x || !h_y) return fail(BSR_ERR_NULL, "null vector");
+  cudaStream_t st = (cudaStream_t)stream;
+  const size_t nx = (size_t)(trans ? A->nbrows * (int64_t)A->bs_r : A->nbcols * (int64_t)A->bs_c);
+  const size_t ny = (size_t)(trans ? A->nbcols * (int64_t)A->bs_c : A->nbrows * (int64_t)A->bs_r);
+  double *dx = nullptr, *dy = nullptr;
+  int rc = dev_alloc_t(&dx, nx);
+  if (rc == BSR_OK) rc = dev_alloc_t(&dy, ny);
+  if (rc == BSR_OK && cudaMemcpyAsync(dx, h_x, nx * 8, cudaMemcpyHostToDevice, st) != cudaSuccess)
+    rc = fail(BSR_ERR_CUDA, "H2D copy failed");
+  if (rc == BSR_OK) rc = trans ? bsr_spmv_t(A, dx, dy, stream) : bsr_spmv(A, dx, dy, stream);
+  if (rc == BSR_OK && cudaMemcpyAsync(h_y, dy, ny * 8, cudaMemcpyDeviceToHost, st) != cudaSuccess)
+    rc = fail(BSR_ERR_CUDA, "D2H copy failed");
+  if (rc == BSR_OK && cudaStreamSynchronize(st) != cudaSuccess) rc = fail(BSR_ERR_CUDA, "stream synchronise failed");
+  dev_free(dx); dev_free(dy);
+  return rc;
+}
+
+}  // extern "C"

@@ -1,0 +1,119 @@
+// internal.h -- private declarations of libbsramg.so (not part of the C ABI; see include/bsr_amg.h).
+#pragma once
+#include <atomic>
+#include <cstdarg>
+#include <cstdint>
+#include <cstdio>
+#include <string>
+#include <vector>
+
+#include <cuda_runtime.h>
+
+#include "bsr_amg.h"
+
+namespace bsramg {
+
+// ------------------------------------------------------------------ errors and counters
+int fail(int code, const char* fmt, ...);
+extern std::atomic<int64_t> g_launches;
+extern std::atomic<int64_t> g_allocs;
+
+#define CUDA_TRY(expr)                                                                         \
+  do {                                                                                         \
+    cudaError_t e__ = (expr);                                                                  \
+    if (e__ != cudaSuccess) return ::bsramg::fail(BSR_ERR_CUDA, "%s: %s", #expr, cudaGetErrorString(e__)); \
+  } while (0)
+
+#define BSR_TRY(expr)            \
+  do {                           \
+    int rc__ = (expr);           \
+    if (rc__ != BSR_OK) return rc__; \
+  } while (0)
+
+// every kernel launch of the library goes through this: counts it and checks the launch status
+#define LAUNCH(kernel, grid, block, smem, stream, ...)                                   \
+  do {                                                                                   \
+    kernel<<<(grid), (block), (smem), (stream)>>>(__VA_ARGS__);                          \
+    ::bsramg::g_launches.fetch_add(1, std::memory_order_relaxed);                        \
+    cudaError_t e__ = cudaGetLastError();                                                \
+    if (e__ != cudaSuccess) return ::bsramg::fail(BSR_ERR_CUDA, "launch %s: %s", #kernel, cudaGetErrorString(e__)); \
+  } while (0)
+
+int dev_alloc(void** p, size_t bytes);  // cudaMalloc + counter (cold paths only)
+void dev_free(void* p);
+
+template <typename T>
+int dev_alloc_t(T** p, size_t n) { return dev_alloc(reinterpret_cast<void**>(p), (n ? n : 1) * sizeof(T)); }
+
+template <typename T>
+int upload(T** d, const std::vector<T>& h, cudaStream_t st) {
+  BSR_TRY(dev_alloc_t(d, h.size()));
+  if (!h.empty()) CUDA_TRY(cudaMemcpyAsync(*d, h.data(), h.size() * sizeof(T), cudaMemcpyHostToDevice, st));
+  return BSR_OK;
+}
+
+inline bool shape_supported(int br, int bc) {
+  return (br == 2 && bc == 2) || (br == 2 && bc == 3) || (br == 3 && bc == 2) || (br == 3 && bc == 3) ||
+         (br == 3 && bc == 6) || (br == 6 && bc == 3) || (br == 6 && bc == 6);
+}
+
+// epilogues of the SpMV kernels (the V-cycle glue fused into the product)
+enum Epilogue { EPI_ASSIGN = 0, /* y = A x */ EPI_RESID = 1, /* y = b - A x */ EPI_SUB = 2, /* y -= A x */
+                EPI_ADD = 3 /* y += A x */ };
+
+// internal SpMV with epilogue; b only for EPI_RESID
+int spmv_launch(bsr_t A, const double* d_x, double* d_y, const double* d_b, Epilogue epi, cudaStream_t st);
+// makes sure the cached transpose exists and its values are current; hot when nothing changed
+int transpose_ensure(bsr_t A, cudaStream_t st);
+
+// ------------------------------------------------------------------ host side of the symbolic phase
+struct HostPlan {
+  // inputs (borrowed while build() runs)
+  int32_t nbrows_a = 0, nbcols_p = 0;
+  // structures
+  std::vector<int32_t> rowptr_ap, colidx_ap, rowidx_ap;  // rowidx_ap[s] = fine row of AP slot s
+  std::vector<int32_t> rowptr_c, colidx_c, rowidx_c;     // rowidx_c[u]  = coarse row of A_c slot u
+  // stage 1: AP(s) = sum over p in [pairptr1[s], pairptr1[s+1]) of A(rowptr_a[i] + k1[p]) * P(pstart[...] + q1[p])
+  std::vector<int32_t> pairptr1;
+  std::vector<uint16_t> k1, q1;  // offsets inside A's row i / inside P's row j
+  std::vector<int32_t> pstart;   // per A slot k: rowptr_p[colidx_a[k]]
+  // stage 2: A_c(u) = sum over p of R(rowptr_r[I] + t2[p]) * AP(apstart[...] + s2[p])
+  std::vector<int32_t> pairptr2;
+  std::vector<uint16_t> t2, s2;  // offsets inside R's row I / inside AP's row i
+  std::vector<int32_t> apstart;  // per R slot t: rowptr_ap[colidx_r[t]]
+  int32_t max_k1 = 0, max_q1 = 0, max_t2 = 0, max_s2 = 0;
+  std::string err;
+  // builds everything from the host structures of A, P and R = P^T.  Returns BSR_OK or an error code.
+  int build(int32_t nbrows_a, const int32_t* rowptr_a, const int32_t* colidx_a, int32_t nbcols_p,
+            const int32_t* rowptr_p, const int32_t* colidx_p, const int32_t* rowptr_r, const int32_t* colidx_r);
+};
+
+// explicit transpose structure on the host: R = P^T rows sorted; perm[t] = slot of P that R's slot t comes from
+void host_transpose_structure(int32_t nbrows, int32_t nbcols, const int32_t* rowptr, const int32_t* colidx,
+                              std::vector<int32_t>& rowptr_t, std::vector<int32_t>& colidx_t,
+                              std::vector<int32_t>& perm);
+
+}  // namespace bsramg
+
+// ------------------------------------------------------------------ the opaque handle types
+struct bsr_matrix_s {
+  int32_t nbrows = 0, nbcols = 0, bs_r = 0, bs_c = 0;
+  int64_t nnzb = 0;
+  const int32_t* d_rowptr = nullptr;
+  const int32_t* d_colidx = nullptr;
+  double* d_vals = nullptr;
+  int64_t state = 0;  // bumped by bsr_values_changed
+  uint64_t magic = 0;
+  // host mirror of the structure (taken at bsr_create, used by the cold symbolic paths)
+  std::vector<int32_t> h_rowptr, h_colidx;
+  int32_t max_row_len = 0;
+  double avg_row_len = 0;
+  int team_mode = 0;  // 0: one lane group per row, 1: the whole warp per row
+  // cached explicit transpose (library-owned)
+  bsr_matrix_s* T = nullptr;
+  int32_t* T_perm = nullptr;  // device: source slot per transposed slot
+  int64_t T_state = -1;       // state of this matrix when T's values were last built
+  int64_t T_builds = 0;
+  bool owns_arrays = false;  // true for library-created matrices (the transposes)
+};
+static const uint64_t BSR_MAGIC = 0x425352414d473031ull;

@@ -1,0 +1,612 @@
+// vcycle.cu -- V-cycle over the reused hierarchy, polynomial point-block-Jacobi smoother, dense coarsest solve, PCG.
+//
+// PAPER.md:42 (two-level cycle: pre-smooth, form and restrict the residual, coarse correction, prolong and add,
+// post-smooth; recursion gives the V-cycle); 83, 121 (the V-cycle is the recurring, SpMV-bound solve phase);
+// 113 (point-block Jacobi smoother, CG accelerator, unpreconditioned residual norm).
+// The smoother is the Chebyshev polynomial in D^-1 A named by BASELINE.json config 4 (reading R15):
+//   theta=(lmax+lmin)/2, delta=(lmax-lmin)/2, sigma=theta/delta, rho_0=1/sigma
+//   r=b-Ax; d_0=D^-1 r/theta; x+=d_0;
+//   k=1..deg-1: r-=A d_{k-1}; rho_k=1/(2 sigma-rho_{k-1}); d_k=rho_k rho_{k-1} d_{k-1}+(2 rho_k/delta) D^-1 r; x+=d_k
+// Every SpMV runs in the blocked kernels of bsr.cu with the vector update fused into its epilogue
+// (r = b - A x, r -= A d, x += P e); D^-1 r and the d/x update are one small kernel.
+// Coarsest level (reading R17): dense Cholesky A = L L^T on the device (blocked, 32x32 tiles), then the
+// explicit triangular inverse L^-1 so that every later solve is two fully parallel triangular mat-vecs.
+#include <algorithm>
+#include <cmath>
+
+#include "internal.h"
+
+namespace bsramg {
+
+constexpr int TS = 32;  // tile size of the dense coarsest-level kernels
+
+struct Level {
+  bsr_t A = nullptr, P = nullptr;
+  double lambda = 0;
+  int64_t n = 0;
+  int bs = 0;
+  double *Dinv = nullptr, *r = nullptr, *d = nullptr, *b = nullptr, *x = nullptr;
+};
+
+}  // namespace bsramg
+
+struct vcycle_s {
+  uint64_t magic = 0;
+  int nlevels = 0, degree = 2;
+  double lo = 0.1, hi = 1.1;
+  std::vector<bsramg::Level> L;
+  // coarsest level, dense
+  int64_t nc = 0, npad = 0;
+  double *dense = nullptr, *diaginv = nullptr, *linv = nullptr, *linvT = nullptr, *ytmp = nullptr;
+  int* d_status = nullptr;
+  // PCG work space
+  double *pr = nullptr, *pz = nullptr, *pp = nullptr, *pq = nullptr, *partial = nullptr, *scal = nullptr;
+};
+static const uint64_t VC_MAGIC = 0x5643594330303031ull;
+
+namespace bsramg {
+
+// ------------------------------------------------------------------ point-block Jacobi data: D^-1 per block row
+template <int BS>
+__global__ void __launch_bounds__(128)
+dinv_kernel(int32_t nbrows, const int32_t* __restrict__ rowptr, const int32_t* __restrict__ colidx,
+            const double* __restrict__ vals, double* __restrict__ dinv, int* __restrict__ status) {
+  const int32_t i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= nbrows) return;
+  int32_t kd = -1;
+  for (int32_t k = rowptr[i]; k < rowptr[i + 1]; ++k)
+    if (colidx[k] == i) { kd = k; break; }
+  double M[BS][2 * BS];
+#pragma unroll
+  for (int r = 0; r < BS; ++r)
+#pragma unroll
+    for (int c = 0; c < BS; ++c) {
+      M[r][c] = (kd >= 0) ? vals[(int64_t)kd * BS * BS + r * BS + c] : 0.0;
+      M[r][BS + c] = (r == c) ? 1.0 : 0.0;
+    }
+  bool ok = kd >= 0;
+  // Gauss-Jordan with partial pivoting, fully unrolled (row swaps by value exchange)
+#pragma unroll
+  for (int c = 0; c < BS; ++c) {
+#pragma unroll
+    for (int r = c + 1; r < BS; ++r) {
+      if (fabs(M[r][c]) > fabs(M[c][c])) {
+#pragma unroll
+        for (int j = 0; j < 2 * BS; ++j) { const double t = M[r][j]; M[r][j] = M[c][j]; M[c][j] = t; }
+      }
+    }
+    const double piv = M[c][c];
+    if (piv == 0.0) ok = false;
+    const double ip = 1.0 / piv;
+#pragma unroll
+    for (int j = 0; j < 2 * BS; ++j) M[c][j] *= ip;
+#pragma unroll
+    for (int r = 0; r < BS; ++r) {
+      if (r != c) {
+        const double f = M[r][c];
+#pragma unroll
+        for (int j = 0; j < 2 * BS; ++j) M[r][j] = fma(-f, M[c][j], M[r][j]);
+      }
+    }
+  }
+  if (!ok) atomicOr(status, 1);
+#pragma unroll
+  for (int r = 0; r < BS; ++r)
+#pragma unroll
+    for (int c = 0; c < BS; ++c) dinv[(int64_t)i * BS * BS + r * BS + c] = M[r][BS + c];
+}
+
+// z = D^-1 r (block row wise);  d = cd*d + cz*z  (first step: d = z/theta);  x = d or x += d
+template <int BS>
+__global__ void __launch_bounds__(256)
+cheb_update_kernel(int64_t n, const double* __restrict__ dinv, const double* __restrict__ r, double* __restrict__ d,
+                   double* __restrict__ x, int first, double theta, double cd, double cz, int x_zero) {
+  const int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (e >= n) return;
+  const int64_t i = e / BS;
+  const int a = (int)(e - i * BS);
+  double z = 0.0;
+#pragma unroll
+  for (int b = 0; b < BS; ++b) z = fma(dinv[(i * BS + a) * BS + b], r[i * BS + b], z);
+  const double dn = first ? z / theta : cd * d[e] + cz * z;
+  d[e] = dn;
+  x[e] = x_zero ? dn : x[e] + dn;
+}
+
+static int launch_dinv(Level& lv, int* status, cudaStream_t st) {
+  bsr_t A = lv.A;
+  const unsigned grid = (unsigned)((A->nbrows + 127) / 128);
+  if (!grid) return BSR_OK;
+  switch (lv.bs) {
+    case 2: LAUNCH(dinv_kernel<2>, grid, 128, 0, st, A->nbrows, A->d_rowptr, A->d_colidx, A->d_vals, lv.Dinv, status); break;
+    case 3: LAUNCH(dinv_kernel<3>, grid, 128, 0, st, A->nbrows, A->d_rowptr, A->d_colidx, A->d_vals, lv.Dinv, status); break;
+    case 6: LAUNCH(dinv_kernel<6>, grid, 128, 0, st, A->nbrows, A->d_rowptr, A->d_colidx, A->d_vals, lv.Dinv, status); break;
+    default: return fail(BSR_ERR_BLOCK, "unsupported block size %d", lv.bs);
+  }
+  return BSR_OK;
+}
+
+static int launch_cheb(Level& lv, double* x, int first, double theta, double cd, double cz, int x_zero,
+                       cudaStream_t st) {
+  const unsigned grid = (unsigned)((lv.n + 255) / 256);
+  if (!grid) return BSR_OK;
+  switch (lv.bs) {
+    case 2: LAUNCH(cheb_update_kernel<2>, grid, 256, 0, st, lv.n, lv.Dinv, lv.r, lv.d, x, first, theta, cd, cz, x_zero); break;
+    case 3: LAUNCH(cheb_update_kernel<3>, grid, 256, 0, st, lv.n, lv.Dinv, lv.r, lv.d, x, first, theta, cd, cz, x_zero); break;
+    case 6: LAUNCH(cheb_update_kernel<6>, grid, 256, 0, st, lv.n, lv.Dinv, lv.r, lv.d, x, first, theta, cd, cz, x_zero); break;
+    default: return fail(BSR_ERR_BLOCK, "unsupported block size %d", lv.bs);
+  }
+  return BSR_OK;
+}
+
+// one polynomial smoother application on level l: x <- x + p(D^-1 A)(b - A x); x_zero: x is known to be 0
+static int smooth(vcycle_t vc, int l, const double* b, double* x, bool x_zero, cudaStream_t st) {
+  Level& lv = vc->L[l];
+  const double lmin = vc->lo * lv.lambda, lmax = vc->hi * lv.lambda;
+  const double theta = (lmax + lmin) / 2, delta = (lmax - lmin) / 2, sigma = theta / delta;
+  if (x_zero) {
+    // r_0 = b exactly; the first D^-1 r reads b in place of r
+    double* saved = lv.r;
+    lv.r = const_cast<double*>(b);
+    int rc = launch_cheb(lv, x, 1, theta, 0.0, 0.0, 1, st);
+    lv.r = saved;
+    BSR_TRY(rc);
+  } else {
+    BSR_TRY(spmv_launch(lv.A, x, lv.r, b, EPI_RESID, st));
+    BSR_TRY(launch_cheb(lv, x, 1, theta, 0.0, 0.0, 0, st));
+  }
+  double rho = 1 / sigma;
+  for (int k = 1; k < vc->degree; ++k) {
+    if (x_zero && k == 1) BSR_TRY(spmv_launch(lv.A, lv.d, lv.r, b, EPI_RESID, st));  // r = b - A d_0
+    else BSR_TRY(spmv_launch(lv.A, lv.d, lv.r, nullptr, EPI_SUB, st));               // r -= A d_{k-1}
+    const double rho_new = 1 / (2 * sigma - rho);
+    BSR_TRY(launch_cheb(lv, x, 0, theta, rho_new * rho, 2 * rho_new / delta, 0, st));
+    rho = rho_new;
+  }
+  return BSR_OK;
+}
+
+// ------------------------------------------------------------------ coarsest level: dense Cholesky + L^-1
+// dense is npad x npad row-major, npad a multiple of TS; rows/cols >= nc carry the identity.
+__global__ void dense_pad_kernel(int64_t nc, int64_t npad, double* __restrict__ dense) {
+  const int64_t i = nc + (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < npad) dense[i * npad + i] = 1.0;
+}
+
+__global__ void __launch_bounds__(256)
+dense_fill_kernel(int64_t nvals, int bs, const int32_t* __restrict__ rowidx_of_slot, const int32_t* __restrict__ colidx,
+                  const double* __restrict__ vals, int64_t npad, double* __restrict__ dense) {
+  const int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (e >= nvals) return;
+  const int bb = bs * bs;
+  const int64_t k = e / bb;
+  const int pos = (int)(e - k * bb);
+  const int r = pos / bs, c = pos - r * bs;
+  dense[((int64_t)rowidx_of_slot[k] * bs + r) * npad + (int64_t)colidx[k] * bs + c] = vals[e];
+}
+
+// factor the diagonal tile j in place (lower Cholesky) and store its inverse in diaginv[j]
+__global__ void __launch_bounds__(TS * TS)
+potrf_tile_kernel(int64_t npad, int j, double* __restrict__ dense, double* __restrict__ diaginv,
+                  int* __restrict__ status) {
+  __shared__ double a[TS][TS + 1];
+  __shared__ double inv[TS][TS + 1];
+  const int tx = threadIdx.x, ty = threadIdx.y;
+  double* tile = dense + ((int64_t)j * TS) * npad + (int64_t)j * TS;
+  a[ty][tx] = tile[(int64_t)ty * npad + tx];
+  inv[ty][tx] = 0.0;
+  __syncthreads();
+  for (int k = 0; k < TS; ++k) {
+    if (tx == k && ty == k) {
+      double p = a[k][k];
+      if (!(p > 0.0)) { atomicOr(status, 2); p = 1.0; }
+      a[k][k] = sqrt(p);
+    }
+    __syncthreads();
+    if (tx == k && ty > k) a[ty][k] /= a[k][k];
+    __syncthreads();
+    if (tx > k && ty >= tx) a[ty][tx] = fma(-a[ty][k], a[tx][k], a[ty][tx]);
+    __syncthreads();
+  }
+  if (tx > ty) a[ty][tx] = 0.0;
+  __syncthreads();
+  if (ty == 0) {  // column tx of the inverse by forward substitution
+    const int c = tx;
+    inv[c][c] = 1.0 / a[c][c];
+    for (int r = c + 1; r < TS; ++r) {
+      double s = 0.0;
+      for (int k = c; k < r; ++k) s = fma(a[r][k], inv[k][c], s);
+      inv[r][c] = -s / a[r][r];
+    }
+  }
+  __syncthreads();
+  tile[(int64_t)ty * npad + tx] = a[ty][tx];
+  diaginv[((int64_t)j * TS + ty) * TS + tx] = inv[ty][tx];
+}
+
+// panel below the diagonal tile: L_ij = A_ij * inv(L_jj)^T for i = j+1+blockIdx.x
+__global__ void __launch_bounds__(TS * TS)
+trsm_tile_kernel(int64_t npad, int j, double* __restrict__ dense, const double* __restrict__ diaginv) {
+  __shared__ double a[TS][TS + 1];
+  __shared__ double w[TS][TS + 1];
+  const int tx = threadIdx.x, ty = threadIdx.y;
+  const int i = j + 1 + blockIdx.x;
+  double* tile = dense + ((int64_t)i * TS) * npad + (int64_t)j * TS;
+  a[ty][tx] = tile[(int64_t)ty * npad + tx];
+  w[ty][tx] = diaginv[((int64_t)j * TS + ty) * TS + tx];
+  __syncthreads();
+  double s = 0.0;
+#pragma unroll 8
+  for (int k = 0; k < TS; ++k) s = fma(a[ty][k], w[tx][k], s);
+  tile[(int64_t)ty * npad + tx] = s;
+}
+
+// trailing update: A_ik -= L_ij * L_kj^T for the lower tiles i >= k > j
+__global__ void __launch_bounds__(TS * TS)
+syrk_tile_kernel(int64_t npad, int j, double* __restrict__ dense) {
+  const int bi = j + 1 + blockIdx.y, bk = j + 1 + blockIdx.x;
+  if (bk > bi) return;
+  __shared__ double li[TS][TS + 1];
+  __shared__ double lk[TS][TS + 1];
+  const int tx = threadIdx.x, ty = threadIdx.y;
+  li[ty][tx] = dense[((int64_t)bi * TS + ty) * npad + (int64_t)j * TS + tx];
+  lk[ty][tx] = dense[((int64_t)bk * TS + ty) * npad + (int64_t)j * TS + tx];
+  __syncthreads();
+  double s = 0.0;
+#pragma unroll 8
+  for (int m = 0; m < TS; ++m) s = fma(li[ty][m], lk[tx][m], s);
+  double* c = dense + ((int64_t)bi * TS + ty) * npad + (int64_t)bk * TS + tx;
+  *c -= s;
+}
+
+// X = L^-1, one CTA per tile column j, tile rows in order (each needs the ones above it in the same column):
+//   X_jj = inv(L_jj);  X_ij = -inv(L_ii) * sum_{k=j}^{i-1} L_ik X_kj
+__global__ void __launch_bounds__(TS * TS)
+trinv_kernel(int64_t npad, int nb, const double* __restrict__ dense, const double* __restrict__ diaginv,
+             double* linv) {
+  __shared__ double a[TS][TS + 1];
+  __shared__ double b[TS][TS + 1];
+  const int tx = threadIdx.x, ty = threadIdx.y;
+  const int j = blockIdx.x;
+  linv[((int64_t)j * TS + ty) * npad + (int64_t)j * TS + tx] = diaginv[((int64_t)j * TS + ty) * TS + tx];
+  __threadfence();
+  __syncthreads();
+  for (int i = j + 1; i < nb; ++i) {
+    double s = 0.0;
+    for (int k = j; k < i; ++k) {
+      a[ty][tx] = dense[((int64_t)i * TS + ty) * npad + (int64_t)k * TS + tx];
+      b[ty][tx] = linv[((int64_t)k * TS + ty) * npad + (int64_t)j * TS + tx];  // written by this CTA
+      __syncthreads();
+#pragma unroll 8
+      for (int m = 0; m < TS; ++m) s = fma(a[ty][m], b[m][tx], s);
+      __syncthreads();
+    }
+    a[ty][tx] = diaginv[((int64_t)i * TS + ty) * TS + tx];
+    b[ty][tx] = s;
+    __syncthreads();
+    double o = 0.0;
+#pragma unroll 8
+    for (int m = 0; m < TS; ++m) o = fma(a[ty][m], b[m][tx], o);
+    linv[((int64_t)i * TS + ty) * npad + (int64_t)j * TS + tx] = -o;
+    __threadfence();
+    __syncthreads();
+  }
+}
+
+__global__ void __launch_bounds__(TS * TS)
+transpose_tile_kernel(int64_t npad, const double* __restrict__ src, double* __restrict__ dst) {
+  __shared__ double t[TS][TS + 1];
+  const int tx = threadIdx.x, ty = threadIdx.y;
+  t[ty][tx] = src[((int64_t)blockIdx.y * TS + ty) * npad + (int64_t)blockIdx.x * TS + tx];
+  __syncthreads();
+  dst[((int64_t)blockIdx.x * TS + ty) * npad + (int64_t)blockIdx.y * TS + tx] = t[tx][ty];
+}
+
+// y[i] = sum_{j in [j0(i), j1(i))} M[i][j] x[j]; lower: j in [0, i]; upper: j in [i, n).  One warp per row.
+__global__ void __launch_bounds__(256)
+trigemv_kernel(int64_t n, int64_t npad, const double* __restrict__ M, const double* __restrict__ x,
+               double* __restrict__ y, int upper) {
+  const int lane = threadIdx.x & 31;
+  const int64_t i = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+  if (i >= n) return;
+  const int64_t j0 = upper ? (i & ~31LL) : 0, j1 = upper ? n : i + 1;
+  double s = 0.0;
+  for (int64_t j = j0 + lane; j < j1; j += 32) s = fma(M[i * npad + j], x[j], s);  // M is 0 outside the triangle
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
+  if (lane == 0) y[i] = s;
+}
+
+static int coarse_factor(vcycle_t vc, const int32_t* rowidx_slot, cudaStream_t st) {
+  bsr_t A = vc->L[vc->nlevels - 1].A;
+  const int64_t np = vc->npad;
+  const int nb = (int)(np / TS);
+  CUDA_TRY(cudaMemsetAsync(vc->dense, 0, (size_t)np * np * 8, st));
+  CUDA_TRY(cudaMemsetAsync(vc->linv, 0, (size_t)np * np * 8, st));
+  if (np > vc->nc) LAUNCH(dense_pad_kernel, (unsigned)((np - vc->nc + 63) / 64), 64, 0, st, vc->nc, np, vc->dense);
+  const int64_t nvals = A->nnzb * A->bs_r * A->bs_c;
+  if (nvals)
+    LAUNCH(dense_fill_kernel, (unsigned)((nvals + 255) / 256), 256, 0, st, nvals, (int)A->bs_r, rowidx_slot,
+           A->d_colidx, A->d_vals, np, vc->dense);
+  const dim3 tb(TS, TS);
+  for (int j = 0; j < nb; ++j) {
+    LAUNCH(potrf_tile_kernel, 1, tb, 0, st, np, j, vc->dense, vc->diaginv, vc->d_status);
+    const int rest = nb - j - 1;
+    if (rest > 0) {
+      LAUNCH(trsm_tile_kernel, (unsigned)rest, tb, 0, st, np, j, vc->dense, vc->diaginv);
+      LAUNCH(syrk_tile_kernel, dim3(rest, rest), tb, 0, st, np, j, vc->dense);
+    }
+  }
+  LAUNCH(trinv_kernel, (unsigned)nb, tb, 0, st, np, nb, vc->dense, vc->diaginv, vc->linv);
+  LAUNCH(transpose_tile_kernel, dim3(nb, nb), tb, 0, st, np, vc->linv, vc->linvT);
+  return BSR_OK;
+}
+
+static int coarse_solve(vcycle_t vc, const double* b, double* x, cudaStream_t st) {
+  const unsigned grid = (unsigned)((vc->nc * 32 + 255) / 256);
+  if (!grid) return BSR_OK;
+  LAUNCH(trigemv_kernel, grid, 256, 0, st, vc->nc, vc->npad, vc->linv, b, vc->ytmp, 0);   // y = L^-1 b
+  LAUNCH(trigemv_kernel, grid, 256, 0, st, vc->nc, vc->npad, vc->linvT, vc->ytmp, x, 1);  // x = L^-T y
+  return BSR_OK;
+}
+
+// ------------------------------------------------------------------ the cycle
+static int cycle(vcycle_t vc, int l, const double* b, double* x, cudaStream_t st) {
+  if (l == vc->nlevels - 1) return coarse_solve(vc, b, x, st);
+  Level& lv = vc->L[l];
+  Level& nx = vc->L[l + 1];
+  BSR_TRY(smooth(vc, l, b, x, true, st));                           // pre-smooth from the zero guess
+  BSR_TRY(spmv_launch(lv.A, x, lv.r, b, EPI_RESID, st));             // r = b - A x
+  BSR_TRY(transpose_ensure(lv.P, st));
+  BSR_TRY(spmv_launch(lv.P->T, lv.r, nx.b, nullptr, EPI_ASSIGN, st)); // b_c = P^T r
+  BSR_TRY(cycle(vc, l + 1, nx.b, nx.x, st));                         // coarse correction
+  BSR_TRY(spmv_launch(lv.P, nx.x, x, nullptr, EPI_ADD, st));         // x += P x_c
+  return smooth(vc, l, b, x, false, st);                             // post-smooth
+}
+
+// ------------------------------------------------------------------ PCG vector kernels (fixed-order reductions)
+constexpr int DOT_BLOCKS = 592;  // 4 per SM on 148 SMs; fixed so that the summation order never changes
+
+__global__ void __launch_bounds__(256)
+dot_partial_kernel(int64_t n, const double* __restrict__ a, const double* __restrict__ b, double* __restrict__ partial) {
+  __shared__ double sh[8];
+  double s = 0.0;
+  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x)
+    s = fma(a[i], b[i], s);
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
+  if ((threadIdx.x & 31) == 0) sh[threadIdx.x >> 5] = s;
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    double t = 0.0;
+    for (int w = 0; w < 8; ++w) t += sh[w];
+    partial[blockIdx.x] = t;
+  }
+}
+
+// out[0] = sum(partial) ; if hist != null also hist[0] = sqrt(sum)
+__global__ void __launch_bounds__(32)
+dot_final_kernel(int nparts, const double* __restrict__ partial, double* __restrict__ out, double* __restrict__ hist) {
+  double s = 0.0;
+  for (int i = threadIdx.x; i < nparts; i += 32) s += partial[i];
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
+  if (threadIdx.x == 0) {
+    out[0] = s;
+    if (hist) hist[0] = sqrt(s);
+  }
+}
+
+// alpha = rz / pq ;  x += alpha p ;  r -= alpha q
+__global__ void __launch_bounds__(256)
+pcg_xr_kernel(int64_t n, const double* __restrict__ rz, const double* __restrict__ pq, const double* __restrict__ p,
+              const double* __restrict__ q, double* __restrict__ x, double* __restrict__ r) {
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  const double alpha = rz[0] / pq[0];
+  x[i] += alpha * p[i];
+  r[i] -= alpha * q[i];
+}
+
+// beta = rz_new / rz ;  p = z + beta p
+__global__ void __launch_bounds__(256)
+pcg_p_kernel(int64_t n, const double* __restrict__ rz_new, const double* __restrict__ rz,
+             const double* __restrict__ z, double* __restrict__ p) {
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  const double beta = rz_new[0] / rz[0];
+  p[i] = z[i] + beta * p[i];
+}
+
+static int dot(vcycle_t vc, int64_t n, const double* a, const double* b, double* out, double* hist, cudaStream_t st) {
+  LAUNCH(dot_partial_kernel, DOT_BLOCKS, 256, 0, st, n, a, b, vc->partial);
+  LAUNCH(dot_final_kernel, 1, 32, 0, st, DOT_BLOCKS, vc->partial, out, hist);
+  return BSR_OK;
+}
+
+static void vc_release(vcycle_t vc) {
+  if (!vc) return;
+  for (auto& lv : vc->L) { dev_free(lv.Dinv); dev_free(lv.r); dev_free(lv.d); dev_free(lv.b); dev_free(lv.x); }
+  dev_free(vc->dense); dev_free(vc->diaginv); dev_free(vc->linv); dev_free(vc->linvT); dev_free(vc->ytmp);
+  dev_free(vc->d_status); dev_free(vc->pr); dev_free(vc->pz); dev_free(vc->pp); dev_free(vc->pq);
+  dev_free(vc->partial); dev_free(vc->scal);
+  vc->magic = 0;
+  delete vc;
+}
+
+static bool vc_ok(vcycle_t vc) { return vc && vc->magic == VC_MAGIC; }
+
+}  // namespace bsramg
+
+using namespace bsramg;
+
+
+extern "C" {
+
+int vcycle_refresh(vcycle_t vc, void* stream) {
+  if (!vc_ok(vc)) return fail(BSR_ERR_NULL, "invalid vcycle handle");
+  cudaStream_t st = (cudaStream_t)stream;
+  CUDA_TRY(cudaMemsetAsync(vc->d_status, 0, sizeof(int), st));
+  for (int l = 0; l + 1 < vc->nlevels; ++l) {
+    BSR_TRY(launch_dinv(vc->L[l], vc->d_status, st));
+    BSR_TRY(transpose_ensure(vc->L[l].P, st));
+  }
+  return coarse_factor(vc, reinterpret_cast<const int32_t*>(vc->L[vc->nlevels - 1].Dinv), st);
+}
+
+int vcycle_status(vcycle_t vc, void* stream) {
+  if (!vc_ok(vc)) return fail(BSR_ERR_NULL, "invalid vcycle handle");
+  int h = 0;
+  CUDA_TRY(cudaMemcpyAsync(&h, vc->d_status, sizeof(int), cudaMemcpyDeviceToHost, (cudaStream_t)stream));
+  CUDA_TRY(cudaStreamSynchronize((cudaStream_t)stream));
+  if (h & 1) return fail(BSR_ERR_NUMERIC, "singular or missing diagonal block");
+  if (h & 2) return fail(BSR_ERR_NUMERIC, "coarsest operator is not positive definite");
+  return BSR_OK;
+}
+
+int vcycle_create(vcycle_t* out, int32_t nlevels, const bsr_t* A, const bsr_t* P, const double* lambda_est,
+                  int32_t cheb_degree, double lo, double hi, void* stream) {
+  if (!out) return fail(BSR_ERR_NULL, "vcycle_create: out is null");
+  *out = nullptr;
+  if (nlevels < 1 || !A || (nlevels > 1 && (!P || !lambda_est))) return fail(BSR_ERR_NULL, "vcycle_create: null argument");
+  if (cheb_degree < 1 || cheb_degree > 4 || !(hi > lo) || !(lo > 0)) return fail(BSR_ERR_SHAPE, "bad smoother parameters");
+  for (int l = 0; l < nlevels; ++l) {
+    if (!A[l] || A[l]->magic != BSR_MAGIC) return fail(BSR_ERR_NULL, "invalid matrix handle (A[%d])", l);
+    if (A[l]->nbrows != A[l]->nbcols || A[l]->bs_r != A[l]->bs_c) return fail(BSR_ERR_SHAPE, "A[%d] is not square", l);
+    if (l + 1 < nlevels) {
+      if (!P[l] || P[l]->magic != BSR_MAGIC) return fail(BSR_ERR_NULL, "invalid matrix handle (P[%d])", l);
+      if (P[l]->nbrows != A[l]->nbrows || P[l]->bs_r != A[l]->bs_r || P[l]->nbcols != A[l + 1]->nbrows ||
+          P[l]->bs_c != A[l + 1]->bs_r)
+        return fail(BSR_ERR_SHAPE, "P[%d] does not connect A[%d] and A[%d]", l, l, l + 1);
+      if (!(lambda_est[l] > 0)) return fail(BSR_ERR_SHAPE, "lambda_est[%d] must be positive", l);
+    }
+  }
+  bsr_t Ac = A[nlevels - 1];
+  const int64_t nc = (int64_t)Ac->nbrows * Ac->bs_r;
+  if (nc > 16384) return fail(BSR_ERR_LIMIT, "coarsest level has %lld unknowns (limit 16384)", (long long)nc);
+  cudaStream_t st = (cudaStream_t)stream;
+  vcycle_s* vc = new (std::nothrow) vcycle_s();
+  if (!vc) return fail(BSR_ERR_ALLOC, "host allocation failed");
+  vc->nlevels = nlevels; vc->degree = cheb_degree; vc->lo = lo; vc->hi = hi;
+  vc->L.resize(nlevels);
+  int rc = BSR_OK;
+  for (int l = 0; l < nlevels && rc == BSR_OK; ++l) {
+    Level& lv = vc->L[l];
+    lv.A = A[l]; lv.P = (l + 1 < nlevels) ? P[l] : nullptr;
+    lv.lambda = (l + 1 < nlevels) ? lambda_est[l] : 0.0;
+    lv.bs = A[l]->bs_r;
+    lv.n = (int64_t)A[l]->nbrows * lv.bs;
+    if (l + 1 < nlevels) {
+      rc = dev_alloc_t(&lv.Dinv, (size_t)lv.n * lv.bs);
+      if (rc == BSR_OK) rc = dev_alloc_t(&lv.r, (size_t)lv.n);
+      if (rc == BSR_OK) rc = dev_alloc_t(&lv.d, (size_t)lv.n);
+    }
+    if (l > 0 && rc == BSR_OK) {
+      rc = dev_alloc_t(&lv.b, (size_t)lv.n);
+      if (rc == BSR_OK) rc = dev_alloc_t(&lv.x, (size_t)lv.n);
+    }
+  }
+  vc->nc = nc;
+  vc->npad = ((nc + TS - 1) / TS) * TS;
+  if (vc->npad == 0) vc->npad = TS;
+  const size_t np2 = (size_t)vc->npad * vc->npad;
+  if (rc == BSR_OK) rc = dev_alloc_t(&vc->dense, np2);
+  if (rc == BSR_OK) rc = dev_alloc_t(&vc->linv, np2);
+  if (rc == BSR_OK) rc = dev_alloc_t(&vc->linvT, np2);
+  if (rc == BSR_OK) rc = dev_alloc_t(&vc->diaginv, (size_t)vc->npad * TS);
+  if (rc == BSR_OK) rc = dev_alloc_t(&vc->ytmp, (size_t)vc->npad);
+  if (rc == BSR_OK) rc = dev_alloc_t(&vc->d_status, 1);
+  const int64_t n0 = vc->L[0].n;
+  if (rc == BSR_OK) rc = dev_alloc_t(&vc->pr, (size_t)n0);
+  if (rc == BSR_OK) rc = dev_alloc_t(&vc->pz, (size_t)n0);
+  if (rc == BSR_OK) rc = dev_alloc_t(&vc->pp, (size_t)n0);
+  if (rc == BSR_OK) rc = dev_alloc_t(&vc->pq, (size_t)n0);
+  if (rc == BSR_OK) rc = dev_alloc_t(&vc->partial, (size_t)DOT_BLOCKS);
+  if (rc == BSR_OK) rc = dev_alloc_t(&vc->scal, 8);
+  if (rc == BSR_OK) {
+    // block row of every stored block of the coarsest operator (for the dense fill); kept in the coarsest
+    // level's otherwise unused Dinv slot
+    std::vector<int32_t> rowidx((size_t)Ac->nnzb);
+    for (int32_t i = 0; i < Ac->nbrows; ++i)
+      for (int32_t k = Ac->h_rowptr[i]; k < Ac->h_rowptr[(size_t)i + 1]; ++k) rowidx[(size_t)k] = i;
+    int32_t* d = nullptr;
+    rc = upload(&d, rowidx, st);
+    vc->L[nlevels - 1].Dinv = reinterpret_cast<double*>(d);
+    if (rc == BSR_OK && cudaStreamSynchronize(st) != cudaSuccess) rc = fail(BSR_ERR_CUDA, "upload failed");
+  }
+  if (rc == BSR_OK) {
+    vc->magic = VC_MAGIC;
+    rc = vcycle_refresh(vc, stream);
+  }
+  if (rc == BSR_OK) rc = vcycle_status(vc, stream);
+  if (rc != BSR_OK) {
+    vc_release(vc);
+    return rc;
+  }
+  *out = vc;
+  return BSR_OK;
+}
+
+int vcycle_apply(vcycle_t vc, const double* d_b, double* d_x, void* stream) {
+  if (!vc_ok(vc)) return fail(BSR_ERR_NULL, "invalid vcycle handle");
+  if (!d_b || !d_x) return fail(BSR_ERR_NULL, "null vector");
+  return cycle(vc, 0, d_b, d_x, (cudaStream_t)stream);
+}
+
+int vcycle_smooth(vcycle_t vc, int32_t level, const double* d_b, double* d_x, void* stream) {
+  if (!vc_ok(vc)) return fail(BSR_ERR_NULL, "invalid vcycle handle");
+  if (!d_b || !d_x) return fail(BSR_ERR_NULL, "null vector");
+  if (level < 0 || level >= vc->nlevels - 1) return fail(BSR_ERR_SHAPE, "level %d has no smoother", level);
+  return smooth(vc, level, d_b, d_x, false, (cudaStream_t)stream);
+}
+
+int pcg_solve(vcycle_t vc, const double* d_b, double* d_x, int32_t iters, double* d_resid_hist, void* stream) {
+  if (!vc_ok(vc)) return fail(BSR_ERR_NULL, "invalid vcycle handle");
+  if (!d_b || !d_x || !d_resid_hist) return fail(BSR_ERR_NULL, "null vector");
+  if (iters < 0) return fail(BSR_ERR_SHAPE, "negative iteration count");
+  cudaStream_t st = (cudaStream_t)stream;
+  bsr_t A = vc->L[0].A;
+  const int64_t n = vc->L[0].n;
+  const unsigned grid = (unsigned)((n + 255) / 256);
+  double *r = vc->pr, *z = vc->pz, *p = vc->pp, *q = vc->pq;
+  double *rz = vc->scal + 0, *rz_new = vc->scal + 1, *pq = vc->scal + 2, *rr = vc->scal + 3;
+  CUDA_TRY(cudaMemcpyAsync(r, d_b, (size_t)n * 8, cudaMemcpyDeviceToDevice, st));
+  CUDA_TRY(cudaMemsetAsync(d_x, 0, (size_t)n * 8, st));
+  BSR_TRY(dot(vc, n, r, r, rr, d_resid_hist, st));
+  BSR_TRY(cycle(vc, 0, r, z, st));
+  CUDA_TRY(cudaMemcpyAsync(p, z, (size_t)n * 8, cudaMemcpyDeviceToDevice, st));
+  BSR_TRY(dot(vc, n, r, z, rz, nullptr, st));
+  for (int k = 0; k < iters; ++k) {
+    BSR_TRY(spmv_launch(A, p, q, nullptr, EPI_ASSIGN, st));
+    BSR_TRY(dot(vc, n, p, q, pq, nullptr, st));
+    if (grid) LAUNCH(pcg_xr_kernel, grid, 256, 0, st, n, rz, pq, p, q, d_x, r);
+    BSR_TRY(dot(vc, n, r, r, rr, d_resid_hist + k + 1, st));
+    BSR_TRY(cycle(vc, 0, r, z, st));
+    BSR_TRY(dot(vc, n, r, z, rz_new, nullptr, st));
+    if (grid) LAUNCH(pcg_p_kernel, grid, 256, 0, st, n, rz_new, rz, z, p);
+    std::swap(rz, rz_new);
+  }
+  return BSR_OK;
+}
+
+int vcycle_apply_host(vcycle_t vc, const double* h_b, double* h_x, void* stream) {
+  if (!vc_ok(vc)) return fail(BSR_ERR_NULL, "invalid vcycle handle");
+  if (!h_b || !h_x) return fail(BSR_ERR_NULL, "null vector");
+  cudaStream_t st = (cudaStream_t)stream;
+  const size_t n = (size_t)vc->L[0].n;
+  // the PCG work vectors double as staging buffers
+  CUDA_TRY(cudaMemcpyAsync(vc->pr, h_b, n * 8, cudaMemcpyHostToDevice, st));
+  BSR_TRY(cycle(vc, 0, vc->pr, vc->pz, st));
+  CUDA_TRY(cudaMemcpyAsync(h_x, vc->pz, n * 8, cudaMemcpyDeviceToHost, st));
+  CUDA_TRY(cudaStreamSynchronize(st));
+  return BSR_OK;
+}
+
+int vcycle_destroy(vcycle_t vc) {
+  if (!vc) return BSR_OK;
+  if (vc->magic != VC_MAGIC) return fail(BSR_ERR_NULL, "invalid vcycle handle");
+  vc_release(vc);
+  return BSR_OK;
+}
+
+}  // extern "C"
