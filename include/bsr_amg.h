@@ -121,10 +121,10 @@ int ptap_get_info(ptap_plan_t plan, int64_t* nnzb_ap, int64_t* n_products_1, int
 /* Runs only one stage of ptap_numeric (1: AP = A*P, 2: A_c = R*AP from the AP left by the last stage 1); for
  * profiling and tests.  stage 2 needs d_vals_c, stage 1 ignores it. */
 int ptap_numeric_stage(ptap_plan_t plan, int32_t stage, bsr_t A, bsr_t P, double* d_vals_c, void* stream);
-/* Device pointers of the plan's cached AP (structure and current values), for tests: borrowed, valid until
- * ptap_destroy. */
-int ptap_get_ap(ptap_plan_t plan, const int32_t** d_rowptr_ap, const int32_t** d_colidx_ap,
-                const double** d_vals_ap);
+/* Copies the plan's cached AP (structure and the values left by the last stage 1) into caller-allocated DEVICE
+ * arrays d_rowptr_ap[nbrows(A)+1], d_colidx_ap[nnzb_ap], d_vals_ap[nnzb_ap*bs*bs_coarse]; any of them may be null
+ * (skipped).  Enqueued on `stream`.  For tests. */
+int ptap_get_ap(ptap_plan_t plan, int32_t* d_rowptr_ap, int32_t* d_colidx_ap, double* d_vals_ap, void* stream);
 /* End-to-end convenience: new operator values arrive on the HOST (h_vals_a[nnzb(A)*bs*bs], copied into A's
  * borrowed device array), the recompute runs, A_c's values are copied to h_vals_c and `stream` is synchronised. */
 int ptap_numeric_host(ptap_plan_t plan, bsr_t A, bsr_t P, const double* h_vals_a, double* h_vals_c,

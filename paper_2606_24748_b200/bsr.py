@@ -37,7 +37,7 @@ SYMBOLS = {
     "ptap_numeric": (C.c_int, [_V, _V, _V, _V, _V]),
     "ptap_get_info": (C.c_int, [_V, _PI64, _PI64, _PI64, _PI64, _PI64]),
     "ptap_numeric_stage": (C.c_int, [_V, _I32, _V, _V, _V, _V]),
-    "ptap_get_ap": (C.c_int, [_V, _PV, _PV, _PV]),
+    "ptap_get_ap": (C.c_int, [_V, _V, _V, _V, _V]),
     "ptap_numeric_host": (C.c_int, [_V, _V, _V, _V, _V, _V, _V]),
     "ptap_destroy": (C.c_int, [_V]),
     "ptap_host_plan_build": (C.c_void_p, [_I32, _V, _V, _I32, _V, _V]),
@@ -238,18 +238,13 @@ class PtapPlan:
     def ap_host(self):
         """(rowptr, colidx, vals) of the cached AP copied to the host (tests)."""
         import torch
-        info = self.info()
-        n, bf, bc = info["nnzb_ap"], self.A.bs_r, self.P.bs_c
-        p = [C.c_void_p() for _ in range(3)]
-        _check(lib().ptap_get_ap(self.h, *[C.byref(t) for t in p]))
-        torch.cuda.synchronize()
-        out = [np.empty(self.A.nbrows + 1, np.int32), np.empty(n, np.int32), np.empty(n * bf * bc, np.float64)]
-        cudart = torch.cuda.cudart()
-        for dst, src in zip(out, p):
-            if dst.nbytes:
-                rc = cudart.cudaMemcpy(dst.ctypes.data, src.value, dst.nbytes, 2)  # cudaMemcpyDeviceToHost
-                assert int(rc) == 0 if not isinstance(rc, tuple) else int(rc[0]) == 0
-        return out[0], out[1], out[2].reshape(n, bf, bc)
+        n, bf, bc = self.info()["nnzb_ap"], self.A.bs_r, self.P.bs_c
+        dev = self.A.vals.device
+        rp = torch.empty(self.A.nbrows + 1, dtype=torch.int32, device=dev)
+        ci = torch.empty(n, dtype=torch.int32, device=dev)
+        va = torch.empty(n * bf * bc, dtype=torch.float64, device=dev)
+        _check(lib().ptap_get_ap(self.h, _dev(rp), _dev(ci), _dev(va), _stream()))
+        return rp.cpu().numpy(), ci.cpu().numpy(), va.cpu().numpy().reshape(n, bf, bc)
 
 
 class HostPlan:

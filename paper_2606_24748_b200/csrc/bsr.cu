@@ -5,13 +5,13 @@
 // only when the prolongator's state changes).
 //
 // SpMV kernel design (sm_100a, HBM-bound, no tensor cores -- DESIGN.md "Kernels"):
-//   A lane GROUP of LB = bs_r * (bs_c / VW) lanes owns one stored block per step; lane (r, cv) of the group loads
-//   VW consecutive doubles of block row r (VW = 2 -> one 16-byte load when bs_c is even, else one 8-byte load), the
-//   matching VW entries of x, and keeps ONE accumulator for output row r.  Consecutive lanes read consecutive
-//   addresses, so a group's load is one contiguous bs_r*bs_c*8-byte run and the GPW = 32/LB groups of a warp read
-//   GPW consecutive blocks (TEAM mode, long rows: the whole warp on one block row) or GPW different block rows
-//   (ROW mode, short rows such as the prolongator's).  The row sum is finished with warp shuffles in a fixed order
-//   (deterministic); the epilogue (y = Ax, y = b - Ax, y -= Ax, y += Ax) is fused into the store.
+//   A lane GROUP of LB lanes owns one stored block per step.  A block is a flat run of bs_r*bs_c doubles; when that
+//   count is even a lane loads one 16-byte pair of the run (3x6, 6x3, 6x6, 2x2, 2x3, 3x2), otherwise one double (3x3,
+//   whose 72-byte blocks are only 8-byte aligned).  Consecutive lanes read consecutive addresses, so a group's load
+//   is one contiguous block and the GPW = 32/LB groups of a warp read GPW consecutive blocks (TEAM mode, long rows:
+//   the whole warp on one block row) or GPW different block rows (ROW mode, short rows such as the prolongator's).
+//   All index / value / x loads of U steps are issued before the first FMA.  The row sum is finished with warp
+//   shuffles in a fixed order (deterministic); the epilogue (y = Ax, b - Ax, y -= Ax, y += Ax) is fused in.
 #include <algorithm>
 #include <cstring>
 
@@ -49,43 +49,24 @@ void dev_free(void* p) {
 }
 
 // ------------------------------------------------------------------ lane mapping of one block shape
+// A stored block is a flat run of BB = BR*BC doubles.  When BB is even a lane owns the 16-byte pair (2q, 2q+1) of
+// that run (PAIR); when BC is even too both elements sit in one block row and the matching x entries are one
+// aligned 16-byte pair (ROWPAIR).  3x3 (72-byte blocks, only 8-byte aligned for odd k) uses one lane per element.
 template <int BR, int BC>
 struct Shape {
-  static constexpr int VW = (BC % 2 == 0) ? 2 : 1;  // doubles per load
-  static constexpr int LPR = BC / VW;               // lanes per block row
-  static constexpr int LB = BR * LPR;               // lanes per block
-  static constexpr int GPW = 32 / LB;               // lane groups per warp
   static constexpr int BB = BR * BC;
-};
-
-template <int VW>
-struct Vec;
-template <>
-struct Vec<1> {
-  double a;
-  __device__ __forceinline__ static Vec stream(const double* p) { return {__ldcs(p)}; }
-  __device__ __forceinline__ static Vec cached(const double* p) { return {__ldg(p)}; }
-  __device__ __forceinline__ static Vec zero() { return {0.0}; }
-  __device__ __forceinline__ double dot(const Vec& o, double acc) const { return fma(a, o.a, acc); }
-};
-template <>
-struct Vec<2> {
-  double a, b;
-  __device__ __forceinline__ static Vec stream(const double* p) {
-    double2 v = __ldcs(reinterpret_cast<const double2*>(p));
-    return {v.x, v.y};
-  }
-  __device__ __forceinline__ static Vec cached(const double* p) {
-    double2 v = __ldg(reinterpret_cast<const double2*>(p));
-    return {v.x, v.y};
-  }
-  __device__ __forceinline__ static Vec zero() { return {0.0, 0.0}; }
-  __device__ __forceinline__ double dot(const Vec& o, double acc) const { return fma(b, o.b, fma(a, o.a, acc)); }
+  static constexpr bool PAIR = (BB % 2 == 0);
+  static constexpr bool ROWPAIR = PAIR && (BC % 2 == 0);
+  static constexpr int LB = PAIR ? BB / 2 : BB;            // lanes per block
+  static constexpr int LPR = ROWPAIR ? BC / 2 : BC;        // lanes per block row (ROWPAIR and scalar layouts)
+  static constexpr int GPW = 32 / LB;                      // lane groups per warp
 };
 
 // y (op)= A x.  TEAM = number of lane groups that share one block row (1 or GPW).  U = blocks in flight per group.
+// Loads are unconditional (the block index is clamped to the row's last block, the product of a clamped step is
+// discarded) so that all U index, value and x loads of a step are issued before the first FMA.
 template <int BR, int BC, int TEAM, int U, int EPI>
-__global__ void __launch_bounds__(256)
+__global__ void __launch_bounds__(256, 4)  // a minimum CTA count makes ptxas keep the batched loads (56 regs)
 spmv_kernel(int32_t nbrows, const int32_t* __restrict__ rowptr, const int32_t* __restrict__ colidx,
             const double* __restrict__ vals, const double* __restrict__ x, double* __restrict__ y,
             const double* __restrict__ b) {
@@ -95,54 +76,106 @@ spmv_kernel(int32_t nbrows, const int32_t* __restrict__ rowptr, const int32_t* _
   const int64_t warp = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
   const int g = lane / S::LB;  // lane group
   const int q = lane % S::LB;  // lane inside the group
-  const int r = q / S::LPR;    // block row of this lane
-  const int cv = q % S::LPR;   // which VW-wide piece of the block row
   const int team = g / TEAM, member = g % TEAM;
   const int64_t row = warp * ROWS_PER_WARP + team;
   const bool live = (g < ROWS_PER_WARP * TEAM) && (row < nbrows);
+  // element(s) of the block this lane owns
+  const int eA = S::PAIR ? 2 * q : q;
+  const int cA = eA % BC;
+  const int cB = (eA + 1) % BC;  // PAIR && !ROWPAIR only
 
-  double acc = 0.0;
+  double accA = 0.0, accB = 0.0;
   if (live) {
-    const int32_t k1 = rowptr[row + 1];
-    const int lane_off = r * BC + cv * S::VW;
-    for (int32_t k = rowptr[row] + member; k < k1; k += TEAM * U) {
-      int32_t col[U];
-      Vec<S::VW> v[U], xv[U];
+    const int32_t k0 = __ldg(rowptr + row), k1 = __ldg(rowptr + row + 1);
+    for (int32_t k = k0 + member; k < k1; k += TEAM * U) {
+      bool ok[U];
+      int32_t kc[U], col[U];
 #pragma unroll
       for (int u = 0; u < U; ++u) {
         const int32_t ku = k + u * TEAM;
-        col[u] = (ku < k1) ? __ldg(colidx + ku) : 0;
+        ok[u] = ku < k1;
+        kc[u] = ok[u] ? ku : k1 - 1;
+        col[u] = __ldg(colidx + kc[u]);
       }
+      if (S::ROWPAIR) {
+        double2 v[U], xv[U];
 #pragma unroll
-      for (int u = 0; u < U; ++u) {
-        const int32_t ku = k + u * TEAM;
-        v[u] = (ku < k1) ? Vec<S::VW>::stream(vals + (int64_t)ku * S::BB + lane_off) : Vec<S::VW>::zero();
+        for (int u = 0; u < U; ++u) v[u] = __ldcs(reinterpret_cast<const double2*>(vals + (int64_t)kc[u] * S::BB + eA));
+#pragma unroll
+        for (int u = 0; u < U; ++u) xv[u] = __ldg(reinterpret_cast<const double2*>(x + (int64_t)col[u] * BC + cA));
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+          const double t = fma(v[u].y, xv[u].y, v[u].x * xv[u].x);
+          accA += ok[u] ? t : 0.0;
+        }
+      } else if (S::PAIR) {
+        double2 v[U];
+        double xa[U], xb[U];
+#pragma unroll
+        for (int u = 0; u < U; ++u) v[u] = __ldcs(reinterpret_cast<const double2*>(vals + (int64_t)kc[u] * S::BB + eA));
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+          xa[u] = __ldg(x + (int64_t)col[u] * BC + cA);
+          xb[u] = __ldg(x + (int64_t)col[u] * BC + cB);
+        }
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+          accA = fma(ok[u] ? v[u].x : 0.0, xa[u], accA);
+          accB = fma(ok[u] ? v[u].y : 0.0, xb[u], accB);
+        }
+      } else {
+        double v[U], xv[U];
+#pragma unroll
+        for (int u = 0; u < U; ++u) v[u] = __ldcs(vals + (int64_t)kc[u] * S::BB + eA);
+#pragma unroll
+        for (int u = 0; u < U; ++u) xv[u] = __ldg(x + (int64_t)col[u] * BC + cA);
+#pragma unroll
+        for (int u = 0; u < U; ++u) accA = fma(ok[u] ? v[u] : 0.0, xv[u], accA);
       }
-#pragma unroll
-      for (int u = 0; u < U; ++u) xv[u] = Vec<S::VW>::cached(x + (int64_t)col[u] * BC + cv * S::VW);
-#pragma unroll
-      for (int u = 0; u < U; ++u) acc = v[u].dot(xv[u], acc);
     }
   }
-  // sum the LPR pieces of a block row (adjacent lanes), then the TEAM groups (lanes LB apart); fixed order
-  if (S::LPR == 3) {
-    const double t1 = __shfl_down_sync(0xffffffffu, acc, 1);
-    const double t2 = __shfl_down_sync(0xffffffffu, acc, 2);
-    acc = (acc + t1) + t2;
-  } else if (S::LPR == 2) {
-    acc += __shfl_down_sync(0xffffffffu, acc, 1);
-  }
+  // 1) the TEAM groups of a row (lanes LB apart), fixed order
 #pragma unroll
   for (int s = 1; s < TEAM; s <<= 1) {
-    const double t = __shfl_down_sync(0xffffffffu, acc, (s * S::LB) & 31);
-    if (member + s < TEAM) acc += t;
+    const double tA = __shfl_down_sync(0xffffffffu, accA, (s * S::LB) & 31);
+    const double tB = __shfl_down_sync(0xffffffffu, accB, (s * S::LB) & 31);
+    if (member + s < TEAM) { accA += tA; accB += tB; }
   }
-  if (live && cv == 0 && member == 0) {
+  // 2) the lanes of one block row
+  double out;
+  bool writer;
+  int r;
+  if (S::PAIR && !S::ROWPAIR) {
+    // lane t < BR of the group gathers elements t*BC .. t*BC+BC-1: element e sits in lane e/2, slot e%2
+    out = 0.0;
+    const int base = lane - q;
+#pragma unroll
+    for (int c = 0; c < BC; ++c) {
+      const int e = (q < BR ? q : 0) * BC + c;
+      const double a = __shfl_sync(0xffffffffu, accA, (base + e / 2) & 31);
+      const double bb = __shfl_sync(0xffffffffu, accB, (base + e / 2) & 31);
+      out += (e & 1) ? bb : a;
+    }
+    r = q;
+    writer = q < BR;
+  } else {
+    out = accA;
+    if (S::LPR == 3) {
+      const double t1 = __shfl_down_sync(0xffffffffu, out, 1);
+      const double t2 = __shfl_down_sync(0xffffffffu, out, 2);
+      out = (out + t1) + t2;
+    } else if (S::LPR == 2) {
+      out += __shfl_down_sync(0xffffffffu, out, 1);
+    }
+    r = q / S::LPR;
+    writer = (q % S::LPR) == 0;
+  }
+  if (live && writer && member == 0) {
     const int64_t o = row * BR + r;
-    if (EPI == EPI_ASSIGN) y[o] = acc;
-    else if (EPI == EPI_RESID) y[o] = b[o] - acc;
-    else if (EPI == EPI_SUB) y[o] = y[o] - acc;
-    else y[o] = y[o] + acc;
+    if (EPI == EPI_ASSIGN) y[o] = out;
+    else if (EPI == EPI_RESID) y[o] = b[o] - out;
+    else if (EPI == EPI_SUB) y[o] = y[o] - out;
+    else y[o] = y[o] + out;
   }
 }
 
@@ -179,9 +212,12 @@ static int spmv_dispatch_epi(bsr_t A, const double* x, double* y, const double* 
 template <int BR, int BC>
 static int spmv_dispatch_team(bsr_t A, const double* x, double* y, const double* b, Epilogue epi, cudaStream_t st) {
   using S = Shape<BR, BC>;
-  constexpr int U = (S::GPW == 1) ? 8 : 4;
-  if (S::GPW > 1 && A->team_mode == 1) return spmv_dispatch_epi<BR, BC, S::GPW, U>(A, x, y, b, epi, st);
-  return spmv_dispatch_epi<BR, BC, 1, U>(A, x, y, b, epi, st);
+  if (A->team_mode == 1) {
+    // the whole warp on one block row: U steps of GPW blocks cover a 27-block row of A in one pass
+    constexpr int U = (S::GPW >= 8) ? 2 : (S::GPW == 1 ? 8 : 9);
+    return spmv_dispatch_epi<BR, BC, S::GPW, U>(A, x, y, b, epi, st);
+  }
+  return spmv_dispatch_epi<BR, BC, 1, 4>(A, x, y, b, epi, st);
 }
 
 int spmv_launch(bsr_t A, const double* x, double* y, const double* b, Epilogue epi, cudaStream_t st) {
@@ -237,13 +273,14 @@ static void choose_team_mode(bsr_t A) {
   int gpw = 1;
   switch (A->bs_r * 10 + A->bs_c) {
     case 22: gpw = 16; break;
-    case 23: gpw = 5; break;
+    case 23: gpw = 10; break;
     case 32: gpw = 10; break;
     case 33: gpw = 3; break;
     case 36: gpw = 3; break;
+    case 63: gpw = 3; break;
     default: gpw = 1;
   }
-  A->team_mode = (gpw > 1 && A->avg_row_len >= 2.0 * gpw) ? 1 : 0;
+  A->team_mode = (A->avg_row_len >= 2.0 * gpw) ? 1 : 0;
 }
 
 int transpose_ensure(bsr_t A, cudaStream_t st) {
@@ -403,7 +440,8 @@ int64_t bsr_spmv_bytes(bsr_t A) {
 
 int bsr_spmv(bsr_t A, const double* d_x, double* d_y, void* stream) {
   if (!valid(A)) return fail(BSR_ERR_NULL, "invalid matrix handle");
-  if (!d_x || !d_y) return fail(BSR_ERR_NULL, "null vector");
+  if (A->nbrows == 0) return BSR_OK;  // nothing to write; null vectors are fine for an empty matrix
+  if ((!d_x && A->nbcols > 0) || !d_y) return fail(BSR_ERR_NULL, "null vector");
   return spmv_launch(A, d_x, d_y, nullptr, EPI_ASSIGN, (cudaStream_t)stream);
 }
 
@@ -416,7 +454,8 @@ int bsr_transpose_prepare(bsr_t A, int64_t* n_value_builds, void* stream) {
 
 int bsr_spmv_t(bsr_t A, const double* d_x, double* d_y, void* stream) {
   if (!valid(A)) return fail(BSR_ERR_NULL, "invalid matrix handle");
-  if (!d_x || !d_y) return fail(BSR_ERR_NULL, "null vector");
+  if (A->nbcols == 0) return BSR_OK;
+  if ((!d_x && A->nbrows > 0) || !d_y) return fail(BSR_ERR_NULL, "null vector");
   BSR_TRY(transpose_ensure(A, (cudaStream_t)stream));
   return spmv_launch(A->T, d_x, d_y, nullptr, EPI_ASSIGN, (cudaStream_t)stream);
 }

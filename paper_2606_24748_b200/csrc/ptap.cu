@@ -326,11 +326,15 @@ int ptap_get_info(ptap_plan_t pl, int64_t* nnzb_ap, int64_t* n_products_1, int64
   return BSR_OK;
 }
 
-int ptap_get_ap(ptap_plan_t pl, const int32_t** d_rowptr_ap, const int32_t** d_colidx_ap, const double** d_vals_ap) {
+int ptap_get_ap(ptap_plan_t pl, int32_t* d_rowptr_ap, int32_t* d_colidx_ap, double* d_vals_ap, void* stream) {
   if (!plan_ok(pl)) return fail(BSR_ERR_NULL, "invalid plan handle");
-  if (d_rowptr_ap) *d_rowptr_ap = pl->rowptr_ap;
-  if (d_colidx_ap) *d_colidx_ap = pl->colidx_ap;
-  if (d_vals_ap) *d_vals_ap = pl->vals_ap;
+  cudaStream_t st = (cudaStream_t)stream;
+  if (d_rowptr_ap)
+    CUDA_TRY(cudaMemcpyAsync(d_rowptr_ap, pl->rowptr_ap, ((size_t)pl->nbrows_a + 1) * 4, cudaMemcpyDeviceToDevice, st));
+  if (d_colidx_ap && pl->nnzb_ap)
+    CUDA_TRY(cudaMemcpyAsync(d_colidx_ap, pl->colidx_ap, (size_t)pl->nnzb_ap * 4, cudaMemcpyDeviceToDevice, st));
+  if (d_vals_ap && pl->nnzb_ap)
+    CUDA_TRY(cudaMemcpyAsync(d_vals_ap, pl->vals_ap, (size_t)pl->nnzb_ap * pl->bf * pl->bc * 8, cudaMemcpyDeviceToDevice, st));
   return BSR_OK;
 }
 
