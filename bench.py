@@ -1,0 +1,370 @@
+#!/usr/bin/env python
+"""bench.py -- the hot path of arxiv/paper_2606_24748 on B200, measured.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 3] [--impl ours|reference]
+
+One STEP = one pass of the whole hot path over one synthetic elasticity problem (BASELINE.json config 3 by default:
+128^3 Q1 hex elements, 6.44 M unknowns, bs 3 -> 6, lognormal modulus, seed 3):
+    y = A x (3x3)   y = P x_c (3x6)   y = P^T x (6x3)   A_c = P^T A P numeric recompute (AP = A*P, then A_c = R*AP)
+Prints ONE JSON line.  `value` is the algorithmic bytes of the step (from the block format: 8*bs_r*bs_c+4 bytes per
+block) divided by the step time, inputs resident in HBM; the per-operation GB/s, ms and roofline
+fractions BASELINE.json's metric names are in `ops`.  `e2e` is the same metric through the C ABI's *_host calls with
+host buffers (H2D of x vectors and of A's new values, D2H of y vectors and of A_c's values inside the timed region).
+`cpu_baseline` is the CPU oracle (oracle/, as it stands) timed on this box's host cores on one pass of the workload.
+`--impl reference` times the oracle alone (the reference arm of this tier).  N > 1 (torchrun): every rank runs its own
+independent problem of the same shape (weak scaling, no data-path collective); time = max over ranks.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "blocked SpMV GB/s & PtAP-recompute ms at 128^3 elasticity, % of HBM peak"
+NOMINAL_HBM_GBS = 8000.0   # the figure north_star names
+FALLBACK_HBM_GBS = 6650.0  # /opt/skills/guides/B200_PROFILING.md fallback
+
+
+def measured_peak():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        with open(p) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    except Exception:
+        return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md)"
+
+
+def bsr_bytes(M) -> int:
+    return M.nnzb * (8 * M.bs_r * M.bs_c + 4) + 4 * (M.nbrows + 1)
+
+
+def spmv_bytes(M) -> int:
+    """nnzb*(8*bs_r*bs_c+4) + 4*(nbrows+1) + 8*bs_c*nbcols + 8*bs_r*nbrows."""
+    return bsr_bytes(M) + 8 * M.bs_c * M.nbcols + 8 * M.bs_r * M.nbrows
+
+
+class ClockSampler:
+    """nvidia-smi clocks and throttle reasons sampled DURING the timed region (B200_PROFILING.md recipe)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index, self.proc, self.lines = index, None, []
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._read, daemon=True)
+            self.thread.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.lines.append(line.strip())
+
+    def stop(self) -> dict:
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=2)
+        except Exception:
+            self.proc.kill()
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for ln in self.lines:
+            f = [t.strip() for t in ln.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0])); mx.append(float(f[1]))
+            except ValueError:
+                continue
+            for n, v in zip(names, f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+# ------------------------------------------------------------------ workload
+def make_problem(cfg: int, ne: int | None = None):
+    """Host matrices A (fine operator) and P (smoothed prolongator) of a BASELINE.json config (DESIGN.md recipe)."""
+    from paper_2606_24748_b200 import problems as pr
+    g = pr.make_generator(cfg, **({"ne": ne} if ne else {}))
+    A = g.A(0)
+    g.build_prolongator(0)
+    return g, A, g.P(0)
+
+
+def workload_name(cfg: int, A, P, ne=None) -> str:
+    from paper_2606_24748_b200 import problems as pr
+    base = pr.CONFIGS[cfg]["name"]
+    if ne:
+        base += f" [sample grid: {ne}^{pr.CONFIGS[cfg]['d']} elements, same recipe]"
+    return f"{base}; {A.nbrows * A.bs_r} unknowns, nnzb(A)={A.nnzb}, nnzb(P)={P.nnzb}"
+
+
+# ------------------------------------------------------------------ the oracle pass (cpu_baseline / --impl reference)
+class OraclePass:
+    """One pass of the hot path in the CPU oracle as it stands: spmv_fast on A, P and the explicit R = P^T, and PtAP
+    form 2 (materialised AP, then R*AP); double accumulators, OpenMP over rows.  Symbolic work is done once here."""
+
+    def __init__(self, A, P, seed: int):
+        from oracle import oracle as orc
+        from paper_2606_24748_b200 import problems as pr
+        self.orc = orc
+        self.A, self.P = A, P
+        self.f2 = orc.PtapForm2(A, P)
+        self.R = self.f2.R
+        self.hA, self.hP, self.hR = orc._Held(A), orc._Held(P), orc._Held(self.R)
+        self.x = pr.uniform(seed, pr.PURPOSE_FINE, A.nbrows * A.bs_r)
+        self.xc = pr.uniform(seed, pr.PURPOSE_COARSE, P.nbcols * P.bs_c)
+        self.y = np.empty(A.nbrows * A.bs_r)
+        self.yc = np.empty(P.nbcols * P.bs_c)
+        nb = lambda n, br, bc, rows: n * (8 * br * bc + 4) + 4 * (rows + 1)
+        bAP = nb(self.f2.cap.shape[0], A.bs_r, P.bs_c, A.nbrows)
+        bAc = nb(self.f2.cc.shape[0], P.bs_c, P.bs_c, P.nbcols)
+        self.bytes = {"spmv_A": spmv_bytes(A), "spmv_P": spmv_bytes(P), "spmv_Pt": spmv_bytes(self.R),
+                      "ptap": bsr_bytes(A) + bsr_bytes(P) + bAP + bsr_bytes(self.R) + bAP + bAc}
+        self.total_bytes = sum(self.bytes.values())
+
+    def run(self) -> dict:
+        t = {}
+        t0 = time.perf_counter(); self.orc.spmv_fast(self.A, self.x, self.y, held=self.hA)
+        t1 = time.perf_counter(); self.orc.spmv_fast(self.P, self.xc, self.y, held=self.hP)
+        t2 = time.perf_counter(); self.orc.spmv_fast(self.R, self.x, self.yc, held=self.hR)
+        t3 = time.perf_counter(); self.f2.run()
+        t4 = time.perf_counter()
+        t["spmv_A"], t["spmv_P"], t["spmv_Pt"], t["ptap"], t["total"] = t1 - t0, t2 - t1, t3 - t2, t4 - t3, t4 - t0
+        return t
+
+
+def omp_threads() -> int:
+    v = os.environ.get("OMP_NUM_THREADS")
+    return int(v) if v and v.isdigit() else (os.cpu_count() or 1)
+
+
+def run_reference(args) -> dict:
+    """The reference arm of this tier: the oracle alone, on a bounded sample per step."""
+    ne = args.ref_ne
+    gen, A, P = make_problem(args.config, ne)  # gen owns the arrays A and P view
+    from paper_2606_24748_b200 import problems as pr
+    op = OraclePass(A, P, pr.CONFIGS[args.config]["seed"])
+    for _ in range(args.warmup):
+        op.run()
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        op.run()
+    dt = time.perf_counter() - t0
+    val = op.total_bytes * args.steps / dt / 1e9
+    sample = f"{ne}^3-element grid of the same recipe per step (all four operations, {op.total_bytes / 1e9:.3f} GB)"
+    return {"impl": "reference", "metric": METRIC, "value": val, "unit": "GB/s", "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": dt / args.steps * 1e3, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": workload_name(args.config, A, P, ne)},
+            "cpu_baseline": {"value": val, "unit": "GB/s", "cores": omp_threads(), "kind": "oracle", "sample": sample},
+            "e2e": {"value": val, "unit": "GB/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
+
+
+# ------------------------------------------------------------------ the CUDA arm
+def run_ours(args) -> dict | None:
+    import torch
+    import torch.distributed as dist
+    from paper_2606_24748_b200 import bsr, problems as pr
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device -- the product path has no CPU fallback")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    bsr.lib()  # fails loudly if the CUDA library cannot be built / loaded
+    cfg = args.config
+    seed = pr.CONFIGS[cfg]["seed"]
+    gen, A, P = make_problem(cfg)
+    dev = torch.device("cuda", local)
+    GA, GP = bsr.Bsr.from_host(A, dev), bsr.Bsr.from_host(P, dev)
+    plan = bsr.PtapPlan(GA, GP)                     # cold: symbolic + block coordinate plan
+    GP.transpose_prepare()                          # cold: R = P^T cached
+    info = plan.info()
+    x = torch.from_numpy(pr.uniform(seed, pr.PURPOSE_FINE, A.nbrows * A.bs_r)).to(dev)
+    xc = torch.from_numpy(pr.uniform(seed, pr.PURPOSE_COARSE, P.nbcols * P.bs_c)).to(dev)
+    y, yc = torch.empty_like(x), torch.empty_like(xc)
+    vals_c = plan.new_values()
+    Rshape = pr.HostBSR(P.nbcols, P.nbrows, P.bs_c, P.bs_r, None, P.colidx, None)
+    nbytes = {"spmv_A": spmv_bytes(A), "spmv_P": spmv_bytes(P), "spmv_Pt": spmv_bytes(Rshape),
+              "ptap": info["algorithmic_bytes"]}
+    bAP = info["nnzb_ap"] * (8 * A.bs_r * P.bs_c + 4) + 4 * (A.nbrows + 1)
+    bAc = plan.nnzb_c * (8 * P.bs_c * P.bs_c + 4) + 4 * (P.nbcols + 1)
+    nbytes_k = {"ptap_stage1_AP": bsr_bytes(A) + bsr_bytes(P) + bAP, "ptap_stage2_RAP": bsr_bytes(Rshape) + bAP + bAc}
+    total_bytes = sum(nbytes.values())
+    names = ["spmv_A", "spmv_P", "spmv_Pt", "ptap_stage1_AP", "ptap_stage2_RAP"]
+
+    def step(ev=None):
+        if ev: ev[0].record()
+        GA.spmv(x, y)
+        if ev: ev[1].record()
+        GP.spmv(xc, y)
+        if ev: ev[2].record()
+        GP.spmv_t(x, yc)
+        if ev: ev[3].record()
+        plan.numeric_stage(1)               # AP = A*P      } together: ptap_numeric (same two launches, same gate)
+        if ev: ev[4].record()
+        plan.numeric_stage(2, vals_c)       # A_c = R*(AP)  }
+        if ev: ev[5].record()
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+            torch.cuda.synchronize()
+
+    for _ in range(max(args.warmup, 3)):
+        step()
+    evs = [[torch.cuda.Event(enable_timing=True) for _ in range(6)] for _ in range(args.steps)]
+    sampler = ClockSampler(local)
+    sampler.start()
+    barrier()
+    l0, a0 = bsr.counters()
+    t_start, t_end = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    t_start.record()
+    for k in range(args.steps):
+        step(evs[k])
+    t_end.record()
+    barrier()
+    l1, a1 = bsr.counters()
+    clocks = sampler.stop()
+    ms_total = t_start.elapsed_time(t_end)
+    per = {n: float(np.mean([evs[k][i].elapsed_time(evs[k][i + 1]) for k in range(args.steps)]))
+           for i, n in enumerate(names)}
+    if world > 1:
+        t = torch.tensor([ms_total], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms_total = float(t.item())
+    ms_step = ms_total / args.steps
+    value = total_bytes * world / (ms_step * 1e-3) / 1e9
+    peak, peak_src = measured_peak()
+
+    # ---- e2e: the same step through the C ABI's host-buffer calls (pinned host memory, copies inside the timed region)
+    hx = torch.from_numpy(pr.uniform(seed, pr.PURPOSE_FINE, A.nbrows * A.bs_r)).pin_memory()
+    hxc = torch.from_numpy(pr.uniform(seed, pr.PURPOSE_COARSE, P.nbcols * P.bs_c)).pin_memory()
+    hy, hyc = torch.empty_like(hx).pin_memory(), torch.empty_like(hxc).pin_memory()
+    hvals_a = torch.from_numpy(np.ascontiguousarray(A.vals).reshape(-1)).pin_memory()
+    hvals_c = torch.empty(vals_c.numel(), dtype=torch.float64).pin_memory()
+
+    def step_host():
+        GA.spmv_host(hx.numpy(), hy.numpy())
+        GP.spmv_host(hxc.numpy(), hy.numpy())
+        GP.spmv_host(hx.numpy(), hyc.numpy(), trans=True)
+        plan.numeric_host(hvals_a.numpy(), hvals_c.numpy(), vals_c)
+
+    h2d = 8 * (2 * hx.numel() + hxc.numel() + hvals_a.numel())
+    d2h = 8 * (2 * hy.numel() + hyc.numel() + hvals_c.numel())
+    e2e_steps = max(1, min(args.steps, args.e2e_steps))
+    step_host()
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(e2e_steps):
+        step_host()
+    barrier()
+    e2e_s = time.perf_counter() - t0
+    if world > 1:
+        t = torch.tensor([e2e_s], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        e2e_s = float(t.item())
+    e2e_val = total_bytes * world * e2e_steps / e2e_s / 1e9
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return None
+
+    ops = {}
+    for n in ["spmv_A", "spmv_P", "spmv_Pt"]:
+        gbs = nbytes[n] / (per[n] * 1e-3) / 1e9
+        ops[n] = {"ms": per[n], "GB/s": gbs, "algorithmic_GB": nbytes[n] / 1e9, "frac_of_measured_hbm": gbs / peak,
+                  "frac_of_nominal_8TBs": gbs / NOMINAL_HBM_GBS}
+    ptap_ms = per["ptap_stage1_AP"] + per["ptap_stage2_RAP"]
+    gbs = nbytes["ptap"] / (ptap_ms * 1e-3) / 1e9
+    ops["ptap_numeric"] = {"ms": ptap_ms, "GB/s": gbs, "algorithmic_GB": nbytes["ptap"] / 1e9,
+                           "frac_of_measured_hbm": gbs / peak, "frac_of_nominal_8TBs": gbs / NOMINAL_HBM_GBS,
+                           "stage1_ms": per["ptap_stage1_AP"], "stage2_ms": per["ptap_stage2_RAP"],
+                           "GFLOP": 2.0 * (info["n_products_1"] * A.bs_r * A.bs_r * P.bs_c +
+                                           info["n_products_2"] * P.bs_c * A.bs_r * P.bs_c) / 1e9}
+    ops["ptap_numeric"]["fp64_TFLOPs"] = ops["ptap_numeric"]["GFLOP"] / ptap_ms
+    kb = dict(nbytes); kb.update(nbytes_k)
+    dom = max(names, key=lambda n: per[n])
+    ach = kb[dom] / (per[dom] * 1e-3) / 1e9
+    traffic = None
+    tp = os.path.join(ROOT, "profiles", "ncu_traffic.json")  # written by hand from the ncu --set full capture
+    if os.path.exists(tp):
+        try:
+            traffic = json.load(open(tp)).get(dom)
+        except Exception:
+            traffic = None
+    roofline = {"bound": "hbm", "kernel": dom, "achieved": ach, "peak": peak, "peak_source": peak_src, "unit": "GB/s",
+                "frac": ach / peak, "traffic": traffic, "algorithmic_bytes_per_launch": kb[dom],
+                "ms_per_launch": per[dom], "share_of_step": per[dom] / sum(per.values()),
+                "all_kernels": {n: {"ms": per[n], "GB/s": kb[n] / (per[n] * 1e-3) / 1e9,
+                                    "frac": kb[n] / (per[n] * 1e-3) / 1e9 / peak} for n in names}}
+    out = {"metric": METRIC, "value": value, "unit": "GB/s", "n_gpus": world, "steps": args.steps,
+           "warmup": max(args.warmup, 3), "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak",
+           "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+           "config": {"workload": workload_name(cfg, A, P), "l2": "inputs exceed L2 (A alone is %.2f GB); no flush" %
+                      (bsr_bytes(A) / 1e9), "per_rank": "one independent problem per GPU", "step":
+                      "y=Ax, y=Px_c, y=P^T x, ptap_numeric (AP=A*P; A_c=R*AP)"},
+           "ops": ops, "roofline": roofline, "clocks": clocks,
+           "e2e": {"value": e2e_val, "unit": "GB/s", "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+                   "ms_per_step": e2e_s / e2e_steps * 1e3, "steps": e2e_steps},
+           "gpu_launches": int(l1 - l0), "allocs_in_timed_region": int(a1 - a0)}
+    if not args.no_cpu_baseline:
+        op = OraclePass(A, P, seed)
+        t = op.run()
+        out["cpu_baseline"] = {"value": op.total_bytes / t["total"] / 1e9, "unit": "GB/s", "cores": omp_threads(),
+                               "kind": "oracle", "sample": "one full pass of the same workload (all four operations)",
+                               "seconds": {k: round(v, 4) for k, v in t.items()}}
+    if world > 1:
+        dist.destroy_process_group()
+    return out
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", type=int, default=3, help="BASELINE.json config (3 = the 128^3 headline grid)")
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--ref-ne", type=int, default=64, help="sample grid of the reference arm (elements per side)")
+    ap.add_argument("--e2e-steps", type=int, default=3)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        if int(os.environ.get("RANK", "0")) != 0:
+            return
+        print(json.dumps(run_reference(args)), flush=True)
+        return
+    out = run_ours(args)
+    if out is not None:
+        print(json.dumps(out), flush=True)
+
+
+if __name__ == "__main__":
+    main()
