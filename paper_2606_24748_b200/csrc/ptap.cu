@@ -12,8 +12,10 @@
 // walked in the plan's fixed order (ascending inner index) and the block is written once.  No atomics, no
 // zero-fill pass, bit-reproducible.
 #include <algorithm>
+#include <cstdlib>
 
 #include "internal.h"
+#include "ptap_stream.h"
 
 struct ptap_plan_s {
   uint64_t magic = 0;
@@ -26,7 +28,9 @@ struct ptap_plan_s {
   int32_t *rowptr_c = nullptr, *colidx_c = nullptr, *rowidx_c = nullptr, *pairptr2 = nullptr, *apstart = nullptr;
   void *pairs1 = nullptr, *pairs2 = nullptr;
   double* vals_ap = nullptr;
+  bsramg::StreamDev s1, s2;  // brick-staged schedules of the two stages (ok == false: gather kernels)
 };
+static const int STREAM_MAX_ITEM = 24;  // longest run of products one lane group sums before handing over a part
 static const uint64_t PLAN_MAGIC = 0x5054415031303030ull;
 
 namespace bsramg {
@@ -116,8 +120,58 @@ static int product_launch(bool wide, int64_t nout, const int32_t* rowidx, const 
   return BSR_OK;
 }
 
+template <typename T>
+static int stream_up(const std::vector<T>& h, const T** d, StreamDev& sd, cudaStream_t st) {
+  T* p = nullptr;
+  BSR_TRY(upload(&p, h, st));
+  sd.owned.push_back(p);
+  sd.bytes += (int64_t)h.size() * sizeof(T);
+  *d = p;
+  return BSR_OK;
+}
+
+int stream_upload(const StreamPlan& sp, StreamDev& sd, cudaStream_t st) {
+  sd = StreamDev();
+  if (!sp.ok) return BSR_OK;
+  StreamArgs& a = sd.args;
+  int rc = stream_up(sp.br_chunk_ptr, &a.br_chunk_ptr, sd, st);
+  if (rc == BSR_OK) rc = stream_up(sp.br_acc_ptr, &a.br_acc_ptr, sd, st);
+  if (rc == BSR_OK) rc = stream_up(sp.acc_slot, &a.acc_slot, sd, st);
+  if (rc == BSR_OK) rc = stream_up(sp.ch_xrun_ptr, &a.ch_xrun_ptr, sd, st);
+  if (rc == BSR_OK) rc = stream_up(sp.ch_yrun_ptr, &a.ch_yrun_ptr, sd, st);
+  if (rc == BSR_OK) rc = stream_up(sp.ch_item_ptr, &a.ch_item_ptr, sd, st);
+  if (rc == BSR_OK) rc = stream_up(sp.ch_red_ptr, &a.ch_red_ptr, sd, st);
+  if (rc == BSR_OK) rc = stream_up(sp.ch_gptr, &a.ch_gptr, sd, st);
+  if (rc == BSR_OK) rc = stream_up(sp.ch_nx, &a.ch_nx, sd, st);
+  if (rc == BSR_OK) rc = stream_up(sp.ch_ny, &a.ch_ny, sd, st);
+  if (rc == BSR_OK) rc = stream_up(sp.ch_nparts, &a.ch_nparts, sd, st);
+  if (rc == BSR_OK) rc = stream_up(sp.ch_code_ptr, &a.ch_code_ptr, sd, st);
+  if (rc == BSR_OK) rc = stream_up(sp.xruns, &a.xruns, sd, st);
+  if (rc == BSR_OK) rc = stream_up(sp.yruns, &a.yruns, sd, st);
+  if (rc == BSR_OK) rc = stream_up(sp.items, &a.items, sd, st);
+  if (rc == BSR_OK) rc = stream_up(sp.reds, &a.reds, sd, st);
+  if (rc == BSR_OK) {
+    if (sp.wide) { const uint32_t* p = nullptr; rc = stream_up(sp.codes32, &p, sd, st); a.codes = p; }
+    else { const uint16_t* p = nullptr; rc = stream_up(sp.codes16, &p, sd, st); a.codes = p; }
+  }
+  if (rc == BSR_OK && cudaStreamSynchronize(st) != cudaSuccess) rc = fail(BSR_ERR_CUDA, "stream plan upload failed");
+  if (rc != BSR_OK) { stream_release(sd); return rc; }
+  sd.ok = true; sd.wide = sp.wide; sd.nbricks = sp.nbricks(); sd.smem = sp.max_smem;
+  return BSR_OK;
+}
+
+void stream_release(StreamDev& sd) {
+  for (void* p : sd.owned) dev_free(p);
+  sd = StreamDev();
+}
+
 static int stage1(ptap_plan_t pl, cudaStream_t st) {
   bsr_t A = pl->A, P = pl->P;
+  if (pl->s1.ok) {
+    StreamArgs a = pl->s1.args;
+    a.xvals = A->d_vals; a.yvals = P->d_vals; a.cvals = pl->vals_ap;
+    return stream_launch(pl->bf, pl->bf, pl->bc, a, pl->s1.wide, pl->s1.nbricks, pl->s1.smem, st);
+  }
 #define S1(BF, BC)                                                                                             \
   return product_launch<BF, BF, BC>(pl->wide1, pl->nnzb_ap, pl->rowidx_ap, A->d_rowptr, pl->pstart, pl->pairptr1, \
                                     pl->pairs1, A->d_vals, P->d_vals, pl->vals_ap, st)
@@ -136,6 +190,11 @@ static int stage1(ptap_plan_t pl, cudaStream_t st) {
 
 static int stage2(ptap_plan_t pl, double* d_vals_c, cudaStream_t st) {
   bsr_t R = pl->P->T;
+  if (pl->s2.ok) {
+    StreamArgs a = pl->s2.args;
+    a.xvals = R->d_vals; a.yvals = pl->vals_ap; a.cvals = d_vals_c;
+    return stream_launch(pl->bc, pl->bf, pl->bc, a, pl->s2.wide, pl->s2.nbricks, pl->s2.smem, st);
+  }
 #define S2(BF, BC)                                                                                              \
   return product_launch<BC, BF, BC>(pl->wide2, pl->nnzb_c, pl->rowidx_c, R->d_rowptr, pl->apstart, pl->pairptr2, \
                                     pl->pairs2, R->d_vals, pl->vals_ap, d_vals_c, st)
@@ -196,6 +255,7 @@ static void plan_release(ptap_plan_t pl) {
   dev_free(pl->rowptr_ap); dev_free(pl->colidx_ap); dev_free(pl->rowidx_ap); dev_free(pl->pairptr1);
   dev_free(pl->pstart); dev_free(pl->rowptr_c); dev_free(pl->colidx_c); dev_free(pl->rowidx_c);
   dev_free(pl->pairptr2); dev_free(pl->apstart); dev_free(pl->pairs1); dev_free(pl->pairs2); dev_free(pl->vals_ap);
+  stream_release(pl->s1); stream_release(pl->s2);
   pl->magic = 0;
   delete pl;
 }
@@ -252,6 +312,23 @@ int ptap_symbolic(ptap_plan_t* out, bsr_t A, bsr_t P, int32_t* nbrows_c, int64_t
   if (rc == BSR_OK) rc = upload_pairs(&pl->pairs1, pl->wide1, hp.k1, hp.q1, st);
   if (rc == BSR_OK) rc = upload_pairs(&pl->pairs2, pl->wide2, hp.t2, hp.s2, st);
   if (rc == BSR_OK) rc = dev_alloc_t(&pl->vals_ap, (size_t)pl->nnzb_ap * pl->bf * pl->bc);
+  if (rc == BSR_OK && !getenv("BSRAMG_NO_STREAM")) {
+    // brick-staged schedules (ptap_stream.cpp); a stage whose shapes do not fit keeps the gather kernel
+    std::vector<StreamBrickDef> bricks;
+    StreamPlan sp;
+    const StreamShape sh1{pl->bf, pl->bf, pl->bc}, sh2{pl->bc, pl->bf, pl->bc};
+    const int ng = stream_groups(pl->bc);
+    stream_bricks_stage1(hp, sh1, ng, STREAM_SMEM_BUDGET, A->h_rowptr.data(), A->h_colidx.data(), P->h_rowptr.data(), bricks);
+    stream_build(sh1, ng, 65535, STREAM_SMEM_BUDGET, bricks, A->h_rowptr.data(), A->h_colidx.data(), P->h_rowptr.data(),
+                 hp.rowptr_ap.data(), hp.pairptr1.data(), hp.k1.data(), hp.q1.data(), sp);
+    rc = stream_upload(sp, pl->s1, st);
+    if (rc == BSR_OK) {
+      stream_bricks_stage2(hp, sh2, ng, STREAM_MAX_ITEM, STREAM_SMEM_BUDGET, R->h_rowptr.data(), R->h_colidx.data(), bricks);
+      stream_build(sh2, ng, STREAM_MAX_ITEM, STREAM_SMEM_BUDGET, bricks, R->h_rowptr.data(), R->h_colidx.data(),
+                   hp.rowptr_ap.data(), hp.rowptr_c.data(), hp.pairptr2.data(), hp.t2.data(), hp.s2.data(), sp);
+      rc = stream_upload(sp, pl->s2, st);
+    }
+  }
   if (rc == BSR_OK && cudaStreamSynchronize(st) != cudaSuccess) rc = fail(BSR_ERR_CUDA, "plan upload failed");
   if (rc != BSR_OK) {
     plan_release(pl);
