@@ -118,69 +118,69 @@ struct bsr_matrix_s {
 };
 static const uint64_t BSR_MAGIC = 0x425352414d473031ull;
 
-// ------------------------------------------------------------------ brick-staged product streams (ptap_stream.cpp)
+// ------------------------------------------------------------------ brick-staged block products (ptap_stream.cpp)
 // One output-stationary block product C = X * Y (stage 1: X = A, Y = P; stage 2: X = R, Y = AP) cut into BRICKS
-// (one CTA each) of CHUNKS.  A chunk stages a set of X blocks and every Y row they reference in shared memory, then
-// lane groups walk ITEMS: an item is a run of products of ONE output block, summed in registers in ascending inner
-// index.  DIRECT items are written straight to C; otherwise the item is one PART of an output block, parts are
-// summed in a fixed order into the brick's shared-memory accumulator and the block is written once at the end
-// (the atomic-free segmented scatter of SURVEY.md 8(a) a7).
+// (one CTA each) of CHUNKS.  A chunk stages a set of X row pieces and every Y row they reference in shared memory.
+// A lane owns one output block C(row, slot) (M x N accumulators in registers).  A warp walks the X blocks of its
+// row piece(s) in order ("k-synchronous"): at step k every lane of the row reads the same X block (a broadcast),
+// and the lanes whose slot receives a product from X(row,k) -- bit `slot` of the block's MASK -- read consecutive
+// blocks of Y's row (lane's block = rank of its bit in the mask), so shared-memory reads are broadcast or
+// contiguous.  DIRECT bricks write each block once from registers at the end of a pass (stage 1).  PERSIST bricks
+// keep the accumulators over all chunks, every warp taking a share of each chunk's X blocks, and add the warps'
+// partial blocks in warp order through shared memory before writing the block once (stage 2) -- the atomic-free
+// segmented scatter of SURVEY.md 8(a) a7.
 namespace bsramg {
 
-struct StreamItem {   // 12 bytes, staged in shared memory
-  int32_t out;        // >= 0: slot of C (direct);  < 0: part -out-1 of this chunk
-  int32_t p0;         // first product, relative to the chunk's code array
-  uint16_t n;         // number of products
-  uint16_t xrow;      // shared-memory X block index of the item's X row piece
+struct StreamEntry {   // 16 bytes: one X row piece inside a pass
+  int32_t out;         // first slot of C's row (direct) / first accumulator of the row (persist)
+  int32_t xbase;       // staged X block index of the piece's first block
+  int32_t len;         // number of X blocks (steps)
+  uint8_t lane0;       // first lane of the row's slots in the warp
+  uint8_t nslots;      // slots of the row (<= 32)
+  uint8_t pad0, pad1;
 };
-struct StreamRun { int32_t src, n, dst; };          // copy n blocks from global block src to staged block dst
-struct StreamRed { int32_t acc, part0, nparts; };   // acc[acc] += part0 + part0+1 + ... (in this order)
+struct StreamPass { int32_t e0, e1, steps, pad; };   // entries [e0, e1) (relative to the chunk), max len
+struct StreamMeta { uint32_t mask, ybase; };          // per staged X block: receiving slots, staged Y row start
+struct StreamRun { int32_t src, n, dst; };            // copy n blocks from global block src to staged block dst
 
 struct StreamPlan {
-  bool ok = false;            // false: shapes / sizes outside the stream format -> caller keeps the gather kernel
+  bool ok = false;            // false: shapes / sizes outside this format -> caller keeps the gather kernel
   std::string why;
-  int ngroups = 0;            // lane groups per CTA the items were scheduled for
-  int oxbits = 0;             // code = ox | (staged Y block index << oxbits); wide -> uint32 codes, else uint16
-  bool wide = false;
+  bool persist = false;
+  int nwarps = 0;
   int64_t max_smem = 0;       // dynamic shared memory of the largest brick
   std::vector<int32_t> br_chunk_ptr;   // nbricks + 1
-  std::vector<int32_t> br_acc_ptr;     // nbricks + 1 -> acc_slot
-  std::vector<int32_t> acc_slot;       // C slot of every accumulator entry
-  std::vector<int32_t> ch_xrun_ptr, ch_yrun_ptr, ch_item_ptr, ch_red_ptr;  // nchunks + 1
-  std::vector<int64_t> ch_code_ptr;                                        // nchunks + 1
-  std::vector<int32_t> ch_gptr;        // nchunks * (ngroups + 1), item index relative to the chunk
-  std::vector<int32_t> ch_nx, ch_ny, ch_nparts;                            // staged X / Y blocks, parts per chunk
+  std::vector<int32_t> br_out;         // persist: first C slot of the brick's row;  br_nslots: its slot count
+  std::vector<int32_t> br_nslots;
+  std::vector<int32_t> ch_xrun_ptr, ch_yrun_ptr, ch_entry_ptr, ch_pass_ptr;  // nchunks + 1
+  std::vector<int64_t> ch_meta_ptr;                                          // nchunks + 1 (staged X blocks)
+  std::vector<int32_t> ch_ny;                                                // staged Y blocks per chunk
   std::vector<StreamRun> xruns, yruns;
-  std::vector<StreamItem> items;
-  std::vector<StreamRed> reds;
-  std::vector<uint16_t> codes16;
-  std::vector<uint32_t> codes32;
+  std::vector<StreamEntry> entries;
+  std::vector<StreamPass> passes;
+  std::vector<StreamMeta> meta;
   int64_t nbricks() const { return (int64_t)br_chunk_ptr.size() - 1; }
-  int64_t nchunks() const { return (int64_t)ch_item_ptr.size() - 1; }
+  int64_t nchunks() const { return (int64_t)ch_ny.size(); }
 };
 
 struct StreamShape { int M, K, N; };   // C blocks M x N, X blocks M x K, Y blocks K x N
 inline int stream_xs(int M, int K) { return (M * K + 1) & ~1; }   // staged X block stride in doubles (16-byte rows)
-int64_t stream_smem_bytes(const StreamShape& sh, int ngroups, bool wide, int64_t nx, int64_t ny, int64_t ncodes,
-                          int64_t nitems, int64_t nparts, int64_t nacc);
+int64_t stream_smem_bytes(const StreamShape& sh, int64_t nx, int64_t ny, int64_t nentries, int64_t npasses);
 
 // piece of an X row: blocks [t0, t1) of row `row`
 struct StreamPiece { int32_t row, t0, t1; };
 struct StreamChunkDef { std::vector<StreamPiece> pieces; };
 struct StreamBrickDef { std::vector<StreamChunkDef> chunks; bool direct = true; };
 
-// builds the flat stream plan of C = X*Y for the given bricks.  pairptr/off_x/off_y: per C slot the ordered products
-// (HostPlan).  max_item: longest item (products); smem_budget: bytes of dynamic shared memory a brick may use.
-void stream_build(const StreamShape& sh, int ngroups, int max_item, int64_t smem_budget,
-                  const std::vector<StreamBrickDef>& bricks, const int32_t* rowptr_x, const int32_t* colidx_x,
-                  const int32_t* rowptr_y, const int32_t* rowptr_c, const int32_t* pairptr, const uint16_t* off_x,
-                  const uint16_t* off_y, StreamPlan& out);
+// builds the flat plan of C = X*Y for the given bricks.  pairptr/off_x: per C slot the ordered products (HostPlan).
+void stream_build(const StreamShape& sh, int nwarps, int64_t smem_budget, const std::vector<StreamBrickDef>& bricks,
+                  const int32_t* rowptr_x, const int32_t* colidx_x, const int32_t* rowptr_y, const int32_t* rowptr_c,
+                  const int32_t* pairptr, const uint16_t* off_x, const uint16_t* off_y, StreamPlan& out);
 
 // brick definitions of the two PtAP stages
-void stream_bricks_stage1(const HostPlan& hp, const StreamShape& sh, int ngroups, int64_t smem_budget,
-                          const int32_t* rowptr_a, const int32_t* colidx_a, const int32_t* rowptr_p,
-                          std::vector<StreamBrickDef>& bricks);
-void stream_bricks_stage2(const HostPlan& hp, const StreamShape& sh, int ngroups, int max_item, int64_t smem_budget,
+void stream_bricks_stage1(const HostPlan& hp, const StreamShape& sh, int64_t smem_budget, const int32_t* rowptr_a,
+                          const int32_t* colidx_a, const int32_t* rowptr_p, std::vector<StreamBrickDef>& bricks);
+void stream_bricks_stage2(const HostPlan& hp, const StreamShape& sh, int nwarps, int64_t smem_budget,
                           const int32_t* rowptr_r, const int32_t* colidx_r, std::vector<StreamBrickDef>& bricks);
 
 }  // namespace bsramg

@@ -30,7 +30,6 @@ struct ptap_plan_s {
   double* vals_ap = nullptr;
   bsramg::StreamDev s1, s2;  // brick-staged schedules of the two stages (ok == false: gather kernels)
 };
-static const int STREAM_MAX_ITEM = 24;  // longest run of products one lane group sums before handing over a part
 static const uint64_t PLAN_MAGIC = 0x5054415031303030ull;
 
 namespace bsramg {
@@ -135,28 +134,22 @@ int stream_upload(const StreamPlan& sp, StreamDev& sd, cudaStream_t st) {
   if (!sp.ok) return BSR_OK;
   StreamArgs& a = sd.args;
   int rc = stream_up(sp.br_chunk_ptr, &a.br_chunk_ptr, sd, st);
-  if (rc == BSR_OK) rc = stream_up(sp.br_acc_ptr, &a.br_acc_ptr, sd, st);
-  if (rc == BSR_OK) rc = stream_up(sp.acc_slot, &a.acc_slot, sd, st);
+  if (rc == BSR_OK) rc = stream_up(sp.br_out, &a.br_out, sd, st);
+  if (rc == BSR_OK) rc = stream_up(sp.br_nslots, &a.br_nslots, sd, st);
   if (rc == BSR_OK) rc = stream_up(sp.ch_xrun_ptr, &a.ch_xrun_ptr, sd, st);
   if (rc == BSR_OK) rc = stream_up(sp.ch_yrun_ptr, &a.ch_yrun_ptr, sd, st);
-  if (rc == BSR_OK) rc = stream_up(sp.ch_item_ptr, &a.ch_item_ptr, sd, st);
-  if (rc == BSR_OK) rc = stream_up(sp.ch_red_ptr, &a.ch_red_ptr, sd, st);
-  if (rc == BSR_OK) rc = stream_up(sp.ch_gptr, &a.ch_gptr, sd, st);
-  if (rc == BSR_OK) rc = stream_up(sp.ch_nx, &a.ch_nx, sd, st);
+  if (rc == BSR_OK) rc = stream_up(sp.ch_entry_ptr, &a.ch_entry_ptr, sd, st);
+  if (rc == BSR_OK) rc = stream_up(sp.ch_pass_ptr, &a.ch_pass_ptr, sd, st);
   if (rc == BSR_OK) rc = stream_up(sp.ch_ny, &a.ch_ny, sd, st);
-  if (rc == BSR_OK) rc = stream_up(sp.ch_nparts, &a.ch_nparts, sd, st);
-  if (rc == BSR_OK) rc = stream_up(sp.ch_code_ptr, &a.ch_code_ptr, sd, st);
+  if (rc == BSR_OK) rc = stream_up(sp.ch_meta_ptr, &a.ch_meta_ptr, sd, st);
   if (rc == BSR_OK) rc = stream_up(sp.xruns, &a.xruns, sd, st);
   if (rc == BSR_OK) rc = stream_up(sp.yruns, &a.yruns, sd, st);
-  if (rc == BSR_OK) rc = stream_up(sp.items, &a.items, sd, st);
-  if (rc == BSR_OK) rc = stream_up(sp.reds, &a.reds, sd, st);
-  if (rc == BSR_OK) {
-    if (sp.wide) { const uint32_t* p = nullptr; rc = stream_up(sp.codes32, &p, sd, st); a.codes = p; }
-    else { const uint16_t* p = nullptr; rc = stream_up(sp.codes16, &p, sd, st); a.codes = p; }
-  }
+  if (rc == BSR_OK) rc = stream_up(sp.entries, &a.entries, sd, st);
+  if (rc == BSR_OK) rc = stream_up(sp.passes, &a.passes, sd, st);
+  if (rc == BSR_OK) rc = stream_up(sp.meta, &a.meta, sd, st);
   if (rc == BSR_OK && cudaStreamSynchronize(st) != cudaSuccess) rc = fail(BSR_ERR_CUDA, "stream plan upload failed");
   if (rc != BSR_OK) { stream_release(sd); return rc; }
-  sd.ok = true; sd.wide = sp.wide; sd.nbricks = sp.nbricks(); sd.smem = sp.max_smem;
+  sd.ok = true; sd.persist = sp.persist; sd.nbricks = sp.nbricks(); sd.smem = sp.max_smem;
   return BSR_OK;
 }
 
@@ -170,7 +163,7 @@ static int stage1(ptap_plan_t pl, cudaStream_t st) {
   if (pl->s1.ok) {
     StreamArgs a = pl->s1.args;
     a.xvals = A->d_vals; a.yvals = P->d_vals; a.cvals = pl->vals_ap;
-    return stream_launch(pl->bf, pl->bf, pl->bc, a, pl->s1.wide, pl->s1.nbricks, pl->s1.smem, st);
+    return stream_launch(pl->bf, pl->bf, pl->bc, a, false, pl->s1.nbricks, pl->s1.smem, st);
   }
 #define S1(BF, BC)                                                                                             \
   return product_launch<BF, BF, BC>(pl->wide1, pl->nnzb_ap, pl->rowidx_ap, A->d_rowptr, pl->pstart, pl->pairptr1, \
@@ -193,7 +186,7 @@ static int stage2(ptap_plan_t pl, double* d_vals_c, cudaStream_t st) {
   if (pl->s2.ok) {
     StreamArgs a = pl->s2.args;
     a.xvals = R->d_vals; a.yvals = pl->vals_ap; a.cvals = d_vals_c;
-    return stream_launch(pl->bc, pl->bf, pl->bc, a, pl->s2.wide, pl->s2.nbricks, pl->s2.smem, st);
+    return stream_launch(pl->bc, pl->bf, pl->bc, a, true, pl->s2.nbricks, pl->s2.smem, st);
   }
 #define S2(BF, BC)                                                                                              \
   return product_launch<BC, BF, BC>(pl->wide2, pl->nnzb_c, pl->rowidx_c, R->d_rowptr, pl->apstart, pl->pairptr2, \
@@ -317,17 +310,21 @@ int ptap_symbolic(ptap_plan_t* out, bsr_t A, bsr_t P, int32_t* nbrows_c, int64_t
     std::vector<StreamBrickDef> bricks;
     StreamPlan sp;
     const StreamShape sh1{pl->bf, pl->bf, pl->bc}, sh2{pl->bc, pl->bf, pl->bc};
-    const int ng = stream_groups(pl->bc);
-    stream_bricks_stage1(hp, sh1, ng, STREAM_SMEM_BUDGET, A->h_rowptr.data(), A->h_colidx.data(), P->h_rowptr.data(), bricks);
-    stream_build(sh1, ng, 65535, STREAM_SMEM_BUDGET, bricks, A->h_rowptr.data(), A->h_colidx.data(), P->h_rowptr.data(),
-                 hp.rowptr_ap.data(), hp.pairptr1.data(), hp.k1.data(), hp.q1.data(), sp);
+    stream_bricks_stage1(hp, sh1, STREAM_SMEM_BUDGET, A->h_rowptr.data(), A->h_colidx.data(), P->h_rowptr.data(), bricks);
+    stream_build(sh1, STREAM_THREADS_DIRECT / 32, STREAM_SMEM_BUDGET, bricks, A->h_rowptr.data(), A->h_colidx.data(),
+                 P->h_rowptr.data(), hp.rowptr_ap.data(), hp.pairptr1.data(), hp.k1.data(), hp.q1.data(), sp);
     rc = stream_upload(sp, pl->s1, st);
     if (rc == BSR_OK) {
-      stream_bricks_stage2(hp, sh2, ng, STREAM_MAX_ITEM, STREAM_SMEM_BUDGET, R->h_rowptr.data(), R->h_colidx.data(), bricks);
-      stream_build(sh2, ng, STREAM_MAX_ITEM, STREAM_SMEM_BUDGET, bricks, R->h_rowptr.data(), R->h_colidx.data(),
-                   hp.rowptr_ap.data(), hp.rowptr_c.data(), hp.pairptr2.data(), hp.t2.data(), hp.s2.data(), sp);
+      const int nw2 = STREAM_THREADS_PERSIST / 32;
+      stream_bricks_stage2(hp, sh2, nw2, STREAM_SMEM_BUDGET, R->h_rowptr.data(), R->h_colidx.data(), bricks);
+      stream_build(sh2, nw2, STREAM_SMEM_BUDGET, bricks, R->h_rowptr.data(), R->h_colidx.data(), hp.rowptr_ap.data(),
+                   hp.rowptr_c.data(), hp.pairptr2.data(), hp.t2.data(), hp.s2.data(), sp);
       rc = stream_upload(sp, pl->s2, st);
     }
+    if (getenv("BSRAMG_VERBOSE"))
+      fprintf(stderr, "ptap_symbolic: stage 1 staged=%d (%lld bricks, %lld B smem), stage 2 staged=%d (%lld bricks, %lld B smem)\n",
+              (int)pl->s1.ok, (long long)pl->s1.nbricks, (long long)pl->s1.smem, (int)pl->s2.ok,
+              (long long)pl->s2.nbricks, (long long)pl->s2.smem);
   }
   if (rc == BSR_OK && cudaStreamSynchronize(st) != cudaSuccess) rc = fail(BSR_ERR_CUDA, "plan upload failed");
   if (rc != BSR_OK) {

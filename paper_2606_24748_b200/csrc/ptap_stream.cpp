@@ -19,16 +19,13 @@ namespace bsramg {
 
 static inline int64_t up16(int64_t b) { return (b + 15) & ~int64_t(15); }
 
-int64_t stream_smem_bytes(const StreamShape& sh, int ngroups, bool wide, int64_t nx, int64_t ny, int64_t ncodes,
-                          int64_t nitems, int64_t nparts, int64_t nacc) {
+int64_t stream_smem_bytes(const StreamShape& sh, int64_t nx, int64_t ny, int64_t nentries, int64_t npasses) {
   int64_t b = 0;
-  b += up16(nacc * sh.M * sh.N * 8);
   b += up16(nx * stream_xs(sh.M, sh.K) * 8);
+  b += up16(nx * (int64_t)sizeof(StreamMeta));
   b += up16(ny * sh.K * sh.N * 8);
-  b += up16(nparts * sh.M * sh.N * 8);
-  b += up16(ncodes * (wide ? 4 : 2));
-  b += up16(nitems * (int64_t)sizeof(StreamItem));
-  b += up16((int64_t)(ngroups + 1) * 4);
+  b += up16(nentries * (int64_t)sizeof(StreamEntry));
+  b += up16(npasses * (int64_t)sizeof(StreamPass));
   return b;
 }
 
@@ -36,53 +33,50 @@ namespace {
 
 struct LocalChunk {
   std::vector<StreamRun> xruns, yruns;
-  std::vector<StreamItem> items;
-  std::vector<int32_t> gptr;
-  std::vector<StreamRed> reds;
-  std::vector<uint32_t> ox, yi;  // per product (unpacked)
-  int32_t nx = 0, ny = 0, nparts = 0;
+  std::vector<StreamEntry> entries;
+  std::vector<StreamPass> passes;
+  std::vector<StreamMeta> meta;
+  int32_t ny = 0;
 };
 struct LocalBrick {
   std::vector<LocalChunk> chunks;
-  std::vector<int32_t> acc_slot;
-  uint32_t max_ox = 0, max_yi = 0;
+  int32_t out = 0, nslots = 0;
   bool bad = false;
 };
 
+inline int popc32(uint32_t v) { return __builtin_popcount(v); }
+
 }  // namespace
 
-void stream_build(const StreamShape& sh, int ngroups, int max_item, int64_t smem_budget,
-                  const std::vector<StreamBrickDef>& bricks, const int32_t* rowptr_x, const int32_t* colidx_x,
-                  const int32_t* rowptr_y, const int32_t* rowptr_c, const int32_t* pairptr, const uint16_t* off_x,
-                  const uint16_t* off_y, StreamPlan& out) {
+void stream_build(const StreamShape& sh, int nwarps, int64_t smem_budget, const std::vector<StreamBrickDef>& bricks,
+                  const int32_t* rowptr_x, const int32_t* colidx_x, const int32_t* rowptr_y, const int32_t* rowptr_c,
+                  const int32_t* pairptr, const uint16_t* off_x, const uint16_t* off_y, StreamPlan& out) {
   out = StreamPlan();
-  out.ngroups = ngroups;
+  out.nwarps = nwarps;
   const int64_t nb = (int64_t)bricks.size();
+  out.persist = nb > 0 && !bricks[0].direct;
   std::vector<LocalBrick> L((size_t)nb);
-  if (max_item < 1) max_item = 1;
-  if (max_item > 65535) max_item = 65535;
 
 #pragma omp parallel
   {
-    std::vector<int32_t> ycols, ydst, order, load_of;
+    std::vector<int32_t> ycols, ydst, order;
 #pragma omp for schedule(dynamic, 16)
     for (int64_t b = 0; b < nb; ++b) {
       const StreamBrickDef& bd = bricks[(size_t)b];
       LocalBrick& lb = L[(size_t)b];
-      // accumulator entries: every C slot of every distinct row of the brick (accumulate mode only)
-      std::vector<int32_t> rows;
-      std::vector<int32_t> acc_base;
+      if (bd.direct == out.persist) { lb.bad = true; continue; }  // one mode per plan
       if (!bd.direct) {
-        for (const auto& cd : bd.chunks)
-          for (const auto& pc : cd.pieces) rows.push_back(pc.row);
-        std::sort(rows.begin(), rows.end());
-        rows.erase(std::unique(rows.begin(), rows.end()), rows.end());
-        acc_base.resize(rows.size());
-        for (size_t r = 0; r < rows.size(); ++r) {
-          acc_base[r] = (int32_t)lb.acc_slot.size();
-          for (int32_t s = rowptr_c[rows[r]]; s < rowptr_c[rows[r] + 1]; ++s) lb.acc_slot.push_back(s);
+        // persist: one C row per brick, one piece per chunk
+        int32_t row = -1;
+        for (const auto& cd : bd.chunks) {
+          if (cd.pieces.size() != 1 || (row >= 0 && cd.pieces[0].row != row)) lb.bad = true;
+          if (!cd.pieces.empty()) row = cd.pieces[0].row;
         }
+        if (row < 0) { lb.bad = true; continue; }
+        lb.out = rowptr_c[row];
+        lb.nslots = rowptr_c[row + 1] - rowptr_c[row];
       }
+      if (lb.bad) continue;
       lb.chunks.resize(bd.chunks.size());
       for (size_t ci = 0; ci < bd.chunks.size(); ++ci) {
         const StreamChunkDef& cd = bd.chunks[ci];
@@ -101,7 +95,6 @@ void stream_build(const StreamShape& sh, int ngroups, int max_item, int64_t smem
           for (int32_t k = src; k < src + n; ++k) ycols.push_back(colidx_x[k]);
           dst += n;
         }
-        lc.nx = dst;
         std::sort(ycols.begin(), ycols.end());
         ycols.erase(std::unique(ycols.begin(), ycols.end()), ycols.end());
         ydst.resize(ycols.size());
@@ -116,135 +109,126 @@ void stream_build(const StreamShape& sh, int ngroups, int max_item, int64_t smem
           yd += n;
         }
         lc.ny = yd;
-        // ---- items (slot-major; a slot's products inside one piece are contiguous because off_x ascends)
+        // ---- per staged X block: which slots of C's row receive a product from it, and where its Y row starts
+        lc.meta.assign((size_t)dst, StreamMeta{0u, 0u});
         for (size_t pi = 0; pi < cd.pieces.size(); ++pi) {
           const StreamPiece& pc = cd.pieces[pi];
-          if (pc.t1 <= pc.t0) continue;
-          const size_t racc = bd.direct ? 0 : (size_t)(std::lower_bound(rows.begin(), rows.end(), pc.row) - rows.begin());
-          for (int32_t s = rowptr_c[pc.row]; s < rowptr_c[pc.row + 1]; ++s) {
-            const uint16_t* ob = off_x + pairptr[s];
-            const uint16_t* oe = off_x + pairptr[s + 1];
-            const int64_t a = pairptr[s] + (std::lower_bound(ob, oe, (uint16_t)pc.t0) - ob);
-            const int64_t e = (pc.t1 > 0xffff) ? pairptr[s + 1]
-                                               : pairptr[s] + (std::lower_bound(ob, oe, (uint16_t)pc.t1) - ob);
-            if (e <= a) continue;
-            const int32_t part_first = lc.nparts;
-            for (int64_t p = a; p < e;) {
-              const int32_t n = (int32_t)std::min<int64_t>(bd.direct ? 65535 : max_item, e - p);
-              StreamItem it;
-              it.p0 = (int32_t)lc.ox.size();
-              it.n = (uint16_t)n;
-              if (piece_xbase[pi] > 0xffff) lb.bad = true;
-              it.xrow = (uint16_t)piece_xbase[pi];
-              if (bd.direct) {
-                if (p != a || n != e - a || pc.t0 != 0) lb.bad = true;  // a direct block must be one item
-                it.out = s;
-              } else {
-                it.out = -(lc.nparts++) - 1;
-              }
-              for (int64_t q = p; q < p + n; ++q) {
-                const uint32_t ox = off_x[q];
-                const int32_t j = colidx_x[rowptr_x[pc.row] + ox];
-                const size_t t = (size_t)(std::lower_bound(ycols.begin(), ycols.end(), j) - ycols.begin());
-                const uint32_t oxr = ox - (uint32_t)pc.t0, yi = (uint32_t)ydst[t] + off_y[q];
-                lc.ox.push_back(oxr);
-                lc.yi.push_back(yi);
-                lb.max_ox = std::max(lb.max_ox, oxr);
-                lb.max_yi = std::max(lb.max_yi, yi);
-              }
-              lc.items.push_back(it);
-              p += n;
+          const int32_t s0 = rowptr_c[pc.row], ns = rowptr_c[pc.row + 1] - s0;
+          if (ns > 32) { lb.bad = true; break; }
+          StreamMeta* mt = lc.meta.data() + piece_xbase[pi];
+          for (int32_t k = pc.t0; k < pc.t1; ++k) {
+            const int32_t j = colidx_x[rowptr_x[pc.row] + k];
+            mt[k - pc.t0].ybase = (uint32_t)ydst[(size_t)(std::lower_bound(ycols.begin(), ycols.end(), j) - ycols.begin())];
+          }
+          for (int32_t s = s0; s < s0 + ns; ++s)
+            for (int64_t p = pairptr[s]; p < pairptr[s + 1]; ++p) {
+              const int32_t ox = off_x[p];
+              if (ox >= pc.t0 && ox < pc.t1) mt[ox - pc.t0].mask |= 1u << (s - s0);
             }
-            if (!bd.direct)
-              lc.reds.push_back({acc_base[racc] + (s - rowptr_c[pc.row]), part_first, lc.nparts - part_first});
+          // the lane of slot s reads block rank(s) of Y's row: must be the product's own Y block
+          for (int32_t s = s0; s < s0 + ns && !lb.bad; ++s)
+            for (int64_t p = pairptr[s]; p < pairptr[s + 1]; ++p) {
+              const int32_t ox = off_x[p];
+              if (ox < pc.t0 || ox >= pc.t1) continue;
+              if (popc32(mt[ox - pc.t0].mask & ((1u << (s - s0)) - 1u)) != (int)off_y[p]) { lb.bad = true; break; }
+            }
+        }
+        if (lb.bad) break;
+        if (lc.meta.size() & 1) lc.meta.push_back(StreamMeta{0u, 0u});  // even count: 16-byte staging
+        // ---- passes
+        if (bd.direct) {
+          // whole rows, packed into warps of 32 lanes: first fit, most slots first
+          const size_t np = cd.pieces.size();
+          order.resize(np);
+          std::iota(order.begin(), order.end(), 0);
+          auto nsl = [&](int32_t pi) { return rowptr_c[cd.pieces[(size_t)pi].row + 1] - rowptr_c[cd.pieces[(size_t)pi].row]; };
+          std::stable_sort(order.begin(), order.end(), [&](int32_t u, int32_t v) { return nsl(u) > nsl(v); });
+          std::vector<std::vector<int32_t>> bins;
+          std::vector<int32_t> used;
+          for (int32_t pi : order) {
+            const int32_t ns = nsl(pi);
+            if (cd.pieces[(size_t)pi].t0 != 0) lb.bad = true;
+            size_t bi = 0;
+            while (bi < bins.size() && used[bi] + ns > 32) ++bi;
+            if (bi == bins.size()) { bins.emplace_back(); used.push_back(0); }
+            bins[bi].push_back(pi);
+            used[bi] += ns;
+          }
+          std::vector<int32_t> steps(bins.size(), 0), border(bins.size());
+          for (size_t bi = 0; bi < bins.size(); ++bi)
+            for (int32_t pi : bins[bi]) steps[bi] = std::max(steps[bi], cd.pieces[(size_t)pi].t1 - cd.pieces[(size_t)pi].t0);
+          std::iota(border.begin(), border.end(), 0);
+          std::stable_sort(border.begin(), border.end(), [&](int32_t u, int32_t v) { return steps[(size_t)u] > steps[(size_t)v]; });
+          for (int32_t bi : border) {
+            StreamPass ps{(int32_t)lc.entries.size(), 0, steps[(size_t)bi], 0};
+            int32_t lane0 = 0;
+            for (int32_t pi : bins[(size_t)bi]) {
+              const StreamPiece& pc = cd.pieces[(size_t)pi];
+              const int32_t ns = nsl(pi);
+              lc.entries.push_back(StreamEntry{rowptr_c[pc.row], piece_xbase[(size_t)pi], pc.t1 - pc.t0, (uint8_t)lane0,
+                                               (uint8_t)ns, 0, 0});
+              lane0 += ns;
+            }
+            ps.e1 = (int32_t)lc.entries.size();
+            lc.passes.push_back(ps);
+          }
+        } else {
+          // the chunk's piece of the row, cut into nwarps contiguous shares: pass w belongs to warp w
+          const StreamPiece& pc = cd.pieces[0];
+          const int32_t len = pc.t1 - pc.t0;
+          for (int w = 0; w < nwarps; ++w) {
+            const int32_t a = (int32_t)((int64_t)len * w / nwarps), e = (int32_t)((int64_t)len * (w + 1) / nwarps);
+            lc.passes.push_back(StreamPass{(int32_t)lc.entries.size(), (int32_t)lc.entries.size() + 1, e - a, 0});
+            lc.entries.push_back(StreamEntry{0, piece_xbase[0] + a, e - a, 0, (uint8_t)lb.nslots, 0, 0});
           }
         }
-        // ---- schedule: longest item first onto the least loaded lane group, then store the items group-major
-        const size_t ni = lc.items.size();
-        order.resize(ni);
-        std::iota(order.begin(), order.end(), 0);
-        std::stable_sort(order.begin(), order.end(),
-                         [&](int32_t u, int32_t v) { return lc.items[(size_t)u].n > lc.items[(size_t)v].n; });
-        typedef std::pair<int64_t, int32_t> LG;  // (load, group)
-        std::priority_queue<LG, std::vector<LG>, std::greater<LG>> pq;
-        for (int g = 0; g < ngroups; ++g) pq.push({0, g});
-        load_of.assign(ni, 0);
-        std::vector<int32_t> cnt((size_t)ngroups + 1, 0);
-        for (size_t t = 0; t < ni; ++t) {
-          LG top = pq.top();
-          pq.pop();
-          load_of[(size_t)order[t]] = top.second;
-          cnt[(size_t)top.second + 1]++;
-          top.first += lc.items[(size_t)order[t]].n + 3;  // + per-item overhead (fetch, flush)
-          pq.push(top);
-        }
-        for (int g = 0; g < ngroups; ++g) cnt[(size_t)g + 1] += cnt[(size_t)g];
-        lc.gptr = cnt;
-        std::vector<StreamItem> sorted(ni);
-        std::vector<int32_t> fill(cnt.begin(), cnt.end() - 1);
-        for (size_t t = 0; t < ni; ++t) sorted[(size_t)fill[(size_t)load_of[(size_t)order[t]]]++] = lc.items[(size_t)order[t]];
-        lc.items.swap(sorted);
       }
     }
   }
-  // ---- code width and limits
-  uint32_t max_ox = 0, max_yi = 0;
-  for (const auto& lb : L) {
-    if (lb.bad) { out.why = "brick outside the stream format"; return; }
-    max_ox = std::max(max_ox, lb.max_ox);
-    max_yi = std::max(max_yi, lb.max_yi);
-  }
-  if (max_ox < 32 && max_yi < 2048) { out.wide = false; out.oxbits = 5; }
-  else if (max_ox < 4096 && max_yi < (1u << 20)) { out.wide = true; out.oxbits = 12; }
-  else { out.why = "row or staged operand too long for the product codes"; return; }
+  for (const auto& lb : L)
+    if (lb.bad) { out.why = "brick outside the staged format (row with more than 32 blocks, or unsorted operand)"; return; }
   // ---- flatten
-  int64_t nchunks = 0, nacc = 0;
-  for (const auto& lb : L) { nchunks += (int64_t)lb.chunks.size(); nacc += (int64_t)lb.acc_slot.size(); }
+  int64_t nchunks = 0;
+  for (const auto& lb : L) nchunks += (int64_t)lb.chunks.size();
   out.br_chunk_ptr.resize((size_t)nb + 1);
-  out.br_acc_ptr.resize((size_t)nb + 1);
-  out.acc_slot.reserve((size_t)nacc);
+  out.br_out.resize((size_t)nb);
+  out.br_nslots.resize((size_t)nb);
   out.ch_xrun_ptr.assign((size_t)nchunks + 1, 0);
   out.ch_yrun_ptr.assign((size_t)nchunks + 1, 0);
-  out.ch_item_ptr.assign((size_t)nchunks + 1, 0);
-  out.ch_red_ptr.assign((size_t)nchunks + 1, 0);
-  out.ch_code_ptr.assign((size_t)nchunks + 1, 0);
-  out.ch_gptr.resize((size_t)nchunks * (ngroups + 1));
-  out.ch_nx.resize((size_t)nchunks);
+  out.ch_entry_ptr.assign((size_t)nchunks + 1, 0);
+  out.ch_pass_ptr.assign((size_t)nchunks + 1, 0);
+  out.ch_meta_ptr.assign((size_t)nchunks + 1, 0);
   out.ch_ny.resize((size_t)nchunks);
-  out.ch_nparts.resize((size_t)nchunks);
-  int64_t c = 0, nxr = 0, nyr = 0, nit = 0, nrd = 0, ncd = 0;
+  int64_t c = 0, nxr = 0, nyr = 0, nen = 0, npa = 0, nme = 0;
   for (int64_t b = 0; b < nb; ++b) {
     const LocalBrick& lb = L[(size_t)b];
     out.br_chunk_ptr[(size_t)b] = (int32_t)c;
-    out.br_acc_ptr[(size_t)b] = (int32_t)out.acc_slot.size();
-    out.acc_slot.insert(out.acc_slot.end(), lb.acc_slot.begin(), lb.acc_slot.end());
+    out.br_out[(size_t)b] = lb.out;
+    out.br_nslots[(size_t)b] = lb.nslots;
+    if (out.persist)
+      out.max_smem = std::max<int64_t>(out.max_smem, up16((int64_t)nwarps * lb.nslots * sh.M * sh.N * 8));
     for (const auto& lc : lb.chunks) {
       out.ch_xrun_ptr[(size_t)c] = (int32_t)nxr; out.ch_yrun_ptr[(size_t)c] = (int32_t)nyr;
-      out.ch_item_ptr[(size_t)c] = (int32_t)nit; out.ch_red_ptr[(size_t)c] = (int32_t)nrd;
-      out.ch_code_ptr[(size_t)c] = ncd;
-      out.ch_nx[(size_t)c] = lc.nx; out.ch_ny[(size_t)c] = lc.ny; out.ch_nparts[(size_t)c] = lc.nparts;
-      std::copy(lc.gptr.begin(), lc.gptr.end(), out.ch_gptr.begin() + c * (ngroups + 1));
-      const int64_t smem = stream_smem_bytes(sh, ngroups, out.wide, lc.nx, lc.ny, (int64_t)lc.ox.size(),
-                                             (int64_t)lc.items.size(), lc.nparts, (int64_t)lb.acc_slot.size());
-      out.max_smem = std::max(out.max_smem, smem);
-      nxr += (int64_t)lc.xruns.size(); nyr += (int64_t)lc.yruns.size(); nit += (int64_t)lc.items.size();
-      nrd += (int64_t)lc.reds.size(); ncd += (int64_t)lc.ox.size();
+      out.ch_entry_ptr[(size_t)c] = (int32_t)nen; out.ch_pass_ptr[(size_t)c] = (int32_t)npa;
+      out.ch_meta_ptr[(size_t)c] = nme;
+      out.ch_ny[(size_t)c] = lc.ny;
+      out.max_smem = std::max(out.max_smem, stream_smem_bytes(sh, (int64_t)lc.meta.size(), lc.ny,
+                                                              (int64_t)lc.entries.size(), (int64_t)lc.passes.size()));
+      nxr += (int64_t)lc.xruns.size(); nyr += (int64_t)lc.yruns.size(); nen += (int64_t)lc.entries.size();
+      npa += (int64_t)lc.passes.size(); nme += ((int64_t)lc.meta.size() + 1) & ~int64_t(1);  // 16-byte aligned
       ++c;
     }
   }
   out.br_chunk_ptr[(size_t)nb] = (int32_t)c;
-  out.br_acc_ptr[(size_t)nb] = (int32_t)out.acc_slot.size();
   out.ch_xrun_ptr[(size_t)c] = (int32_t)nxr; out.ch_yrun_ptr[(size_t)c] = (int32_t)nyr;
-  out.ch_item_ptr[(size_t)c] = (int32_t)nit; out.ch_red_ptr[(size_t)c] = (int32_t)nrd;
-  out.ch_code_ptr[(size_t)c] = ncd;
-  if (nit >= (1LL << 31) || out.max_smem > smem_budget) {
-    out.why = out.max_smem > smem_budget ? "a brick does not fit the shared memory budget" : "too many items";
+  out.ch_entry_ptr[(size_t)c] = (int32_t)nen; out.ch_pass_ptr[(size_t)c] = (int32_t)npa;
+  out.ch_meta_ptr[(size_t)c] = nme;
+  if (nen >= (1LL << 31) || out.max_smem > smem_budget) {
+    out.why = out.max_smem > smem_budget ? "a brick does not fit the shared memory budget" : "too many entries";
     return;
   }
-  out.xruns.resize((size_t)nxr); out.yruns.resize((size_t)nyr); out.items.resize((size_t)nit);
-  out.reds.resize((size_t)nrd);
-  if (out.wide) out.codes32.resize((size_t)ncd); else out.codes16.resize((size_t)ncd);
-  const int oxb = out.oxbits;
+  out.xruns.resize((size_t)nxr); out.yruns.resize((size_t)nyr); out.entries.resize((size_t)nen);
+  out.passes.resize((size_t)npa); out.meta.assign((size_t)nme, StreamMeta{0u, 0u});
 #pragma omp parallel for schedule(dynamic, 16)
   for (int64_t b = 0; b < nb; ++b) {
     const LocalBrick& lb = L[(size_t)b];
@@ -252,13 +236,9 @@ void stream_build(const StreamShape& sh, int ngroups, int max_item, int64_t smem
     for (const auto& lc : lb.chunks) {
       std::copy(lc.xruns.begin(), lc.xruns.end(), out.xruns.begin() + out.ch_xrun_ptr[(size_t)cc]);
       std::copy(lc.yruns.begin(), lc.yruns.end(), out.yruns.begin() + out.ch_yrun_ptr[(size_t)cc]);
-      std::copy(lc.items.begin(), lc.items.end(), out.items.begin() + out.ch_item_ptr[(size_t)cc]);
-      std::copy(lc.reds.begin(), lc.reds.end(), out.reds.begin() + out.ch_red_ptr[(size_t)cc]);
-      const int64_t c0 = out.ch_code_ptr[(size_t)cc];
-      for (size_t p = 0; p < lc.ox.size(); ++p) {
-        const uint32_t code = lc.ox[p] | (lc.yi[p] << oxb);
-        if (out.wide) out.codes32[(size_t)c0 + p] = code; else out.codes16[(size_t)c0 + p] = (uint16_t)code;
-      }
+      std::copy(lc.entries.begin(), lc.entries.end(), out.entries.begin() + out.ch_entry_ptr[(size_t)cc]);
+      std::copy(lc.passes.begin(), lc.passes.end(), out.passes.begin() + out.ch_pass_ptr[(size_t)cc]);
+      std::copy(lc.meta.begin(), lc.meta.end(), out.meta.begin() + out.ch_meta_ptr[(size_t)cc]);
       ++cc;
     }
   }
@@ -270,9 +250,8 @@ void stream_build(const StreamShape& sh, int ngroups, int max_item, int64_t smem
 // receives the most products, i.e. argmax_J |N(i) ∩ supp P(:,J)| -- for an aggregation-based P that is i's own
 // aggregate, and the P rows the brick references are the aggregate's neighbourhood.  Purely structural; it only
 // decides scheduling.  A group that does not fit the shared-memory budget is halved (by row order) until it does.
-void stream_bricks_stage1(const HostPlan& hp, const StreamShape& sh, int ngroups, int64_t smem_budget,
-                          const int32_t* rowptr_a, const int32_t* colidx_a, const int32_t* rowptr_p,
-                          std::vector<StreamBrickDef>& bricks) {
+void stream_bricks_stage1(const HostPlan& hp, const StreamShape& sh, int64_t smem_budget, const int32_t* rowptr_a,
+                          const int32_t* colidx_a, const int32_t* rowptr_p, std::vector<StreamBrickDef>& bricks) {
   const int32_t n = hp.nbrows_a, nc = hp.nbcols_p;
   std::vector<int32_t> home((size_t)n, 0);
 #pragma omp parallel for schedule(static)
@@ -304,20 +283,18 @@ void stream_bricks_stage1(const HostPlan& hp, const StreamShape& sh, int ngroups
       while (!stack.empty()) {
         const auto r = stack.back();
         stack.pop_back();
-        int64_t nx = 0, ny = 0, ncodes = 0, nitems = 0;
+        int64_t nx = 0, ny = 0;
         cols.clear();
         for (int32_t t = r.first; t < r.second; ++t) {
           const int32_t i = grows[t];
           nx += rowptr_a[i + 1] - rowptr_a[i];
-          nitems += hp.rowptr_ap[i + 1] - hp.rowptr_ap[i];
-          ncodes += hp.pairptr1[hp.rowptr_ap[i + 1]] - hp.pairptr1[hp.rowptr_ap[i]];
           cols.insert(cols.end(), colidx_a + rowptr_a[i], colidx_a + rowptr_a[i + 1]);
         }
         std::sort(cols.begin(), cols.end());
         cols.erase(std::unique(cols.begin(), cols.end()), cols.end());
         for (int32_t j : cols) ny += rowptr_p[j + 1] - rowptr_p[j];
-        const int64_t bytes = stream_smem_bytes(sh, ngroups, /*wide=*/ny >= 2048, nx, ny, ncodes, nitems, 0, 0);
-        if (bytes > smem_budget && r.second - r.first > 1) {
+        const int64_t bytes = stream_smem_bytes(sh, nx, ny, r.second - r.first, r.second - r.first);
+        if (bytes > smem_budget - 512 && r.second - r.first > 1) {
           const int32_t mid = r.first + (r.second - r.first) / 2;
           stack.push_back({mid, r.second});   // popped after the first half: keeps row order
           stack.push_back({r.first, mid});
@@ -342,36 +319,27 @@ void stream_bricks_stage1(const HostPlan& hp, const StreamShape& sh, int ngroups
 // ------------------------------------------------------------------ stage 2 bricks: A_c = R*(AP)
 // One brick per coarse row I.  Its R row is cut into chunks of consecutive blocks such that the chunk's R blocks, the
 // AP rows they reference, the codes, items and parts fit the budget next to the row's accumulator.
-void stream_bricks_stage2(const HostPlan& hp, const StreamShape& sh, int ngroups, int max_item, int64_t smem_budget,
+void stream_bricks_stage2(const HostPlan& hp, const StreamShape& sh, int nwarps, int64_t smem_budget,
                           const int32_t* rowptr_r, const int32_t* colidx_r, std::vector<StreamBrickDef>& bricks) {
   const int32_t nc = hp.nbcols_p;
   bricks.assign((size_t)nc, StreamBrickDef());
-#pragma omp parallel
-  {
-    std::vector<int32_t> cnt;
-#pragma omp for schedule(dynamic, 64)
-    for (int32_t I = 0; I < nc; ++I) {
-      StreamBrickDef& bd = bricks[(size_t)I];
-      bd.direct = false;
-      const int32_t len = rowptr_r[I + 1] - rowptr_r[I];
-      const int64_t nslots = hp.rowptr_c[I + 1] - hp.rowptr_c[I];
-      cnt.assign((size_t)len + 1, 0);
-      for (int64_t p = hp.pairptr2[hp.rowptr_c[I]]; p < hp.pairptr2[hp.rowptr_c[I + 1]]; ++p) cnt[hp.t2[(size_t)p]]++;
-      int32_t t0 = 0;
-      int64_t nx = 0, ny = 0, ncodes = 0;
-      for (int32_t t = 0; t < len; ++t) {
-        const int32_t i = colidx_r[rowptr_r[I] + t];
-        const int64_t ay = hp.rowptr_ap[i + 1] - hp.rowptr_ap[i], ac = cnt[(size_t)t];
-        const int64_t est_items = nslots + (ncodes + ac) / std::max(1, max_item);
-        const int64_t bytes = stream_smem_bytes(sh, ngroups, true, nx + 1, ny + ay, ncodes + ac, est_items, est_items, nslots);
-        if (bytes > smem_budget && t > t0) {
-          bd.chunks.push_back(StreamChunkDef{{StreamPiece{I, t0, t}}});
-          t0 = t; nx = 0; ny = 0; ncodes = 0;
-        }
-        nx += 1; ny += ay; ncodes += ac;
+#pragma omp parallel for schedule(dynamic, 64)
+  for (int32_t I = 0; I < nc; ++I) {
+    StreamBrickDef& bd = bricks[(size_t)I];
+    bd.direct = false;
+    const int32_t len = rowptr_r[I + 1] - rowptr_r[I];
+    int32_t t0 = 0;
+    int64_t nx = 0, ny = 0;
+    for (int32_t t = 0; t < len; ++t) {
+      const int32_t i = colidx_r[rowptr_r[I] + t];
+      const int64_t ay = hp.rowptr_ap[i + 1] - hp.rowptr_ap[i];
+      if (stream_smem_bytes(sh, nx + 1, ny + ay, nwarps, nwarps) > smem_budget - 512 && t > t0) {
+        bd.chunks.push_back(StreamChunkDef{{StreamPiece{I, t0, t}}});
+        t0 = t; nx = 0; ny = 0;
       }
-      if (len > t0 || bd.chunks.empty()) bd.chunks.push_back(StreamChunkDef{{StreamPiece{I, t0, len}}});
+      nx += 1; ny += ay;
     }
+    if (len > t0 || bd.chunks.empty()) bd.chunks.push_back(StreamChunkDef{{StreamPiece{I, t0, len}}});
   }
 }
 

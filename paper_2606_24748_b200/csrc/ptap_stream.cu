@@ -1,17 +1,18 @@
-// ptap_stream.cu -- the hot kernels of ptap_numeric: brick-staged, output-stationary block products.
+// ptap_stream.cu -- the hot kernels of ptap_numeric: brick-staged, output-stationary, k-synchronous block products.
 //
 // PAPER.md:219 (the dominant kernel is the numeric A*P with block sizes <3,3,6>), PAPER.md:103 ("local blocked triple
 // product"), PAPER.md:97-99, 248-250 (coarse blocks summed through a precomputed block plan, contiguous bs_r*bs_c
 // runs).  Schedule format: internal.h / ptap_stream.cpp.
 //
-// One CTA = one brick.  Per chunk it stages, with coalesced loads, the X blocks (A rows / a piece of an R row), every
-// Y row they reference (P rows / AP rows), the product codes and the item table in shared memory.  Then lane groups
-// of N lanes (lane = column c of the output block) walk their items: per product a group reads its X block by
-// broadcast (M*K doubles, 16-byte loads) and column c of the Y block (K doubles), and keeps the M x N output block in
-// M registers per lane.  HBM sees each operand once per brick (Y again from L2 for neighbouring bricks); the
-// gathers that made the one-thread-per-block version L1-bound (profiles/r1a_first_path.md) are shared-memory reads.
-// No atomics: a block is either written once from registers (stage 1) or its parts are added in plan order into the
-// brick's shared-memory accumulator and written once (stage 2).
+// One CTA = one brick.  Per chunk it stages, with asynchronous coalesced copies, the X blocks (A rows / a piece of an
+// R row), every Y row they reference (P rows / AP rows) and the per-block masks in shared memory.  A lane owns one
+// output block (M x N accumulators in registers); its warp walks the X blocks of the row in order.  At step k all
+// lanes of a row read X(row,k) -- one shared-memory broadcast -- and the lanes whose bit is set in the block's mask
+// read consecutive blocks of Y's row, so every shared-memory access is a broadcast or contiguous (the gathers that
+// made the one-thread-per-block version L1-bound, profiles/r1a_first_path.md, are gone) and HBM sees each operand
+// once per brick (Y again from L2 for neighbouring bricks).  No atomics: stage 1 writes each AP block once from
+// registers; stage 2 adds the warps' partial coarse blocks in warp order through shared memory and writes each A_c
+// block once.
 #include "internal.h"
 #include "ptap_stream.h"
 
@@ -19,181 +20,218 @@ namespace bsramg {
 
 __device__ __forceinline__ int64_t up16d(int64_t b) { return (b + 15) & ~int64_t(15); }
 
-template <int M, int K, int N, typename CodeT, int OXBITS>
-__global__ void __launch_bounds__(STREAM_THREADS, 2)
+// asynchronous global -> shared copies (LDGSTS): every thread issues all of its copies back to back and the CTA
+// waits once, so a chunk pays the memory latency once instead of once per loop trip
+template <int BYTES>
+__device__ __forceinline__ void cp_async(void* dst_smem, const void* src) {
+  const unsigned d = (unsigned)__cvta_generic_to_shared(dst_smem);
+  if (BYTES == 16) asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(d), "l"(src));
+  else if (BYTES == 8) asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(d), "l"(src));
+  else asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(d), "l"(src));
+}
+__device__ __forceinline__ void cp_async_wait_all() {
+  asm volatile("cp.async.commit_group;\n\tcp.async.wait_group 0;" ::: "memory");
+}
+
+template <int NE>
+__device__ __forceinline__ void lds_block(const double* __restrict__ p, double (&v)[NE]) {  // p 16-byte aligned if NE even
+  if (NE % 2 == 0) {
+#pragma unroll
+    for (int e = 0; e < NE / 2; ++e) {
+      const double2 t = reinterpret_cast<const double2*>(p)[e];
+      v[2 * e] = t.x;
+      v[2 * e + 1] = t.y;
+    }
+  } else {
+#pragma unroll
+    for (int e = 0; e < NE; ++e) v[e] = p[e];
+  }
+}
+
+template <int M, int K, int N, int NT, bool PERSIST>
+__global__ void __launch_bounds__(NT, 2)
 stream_product_kernel(const StreamArgs a) {
-  constexpr int MK = M * K, KN = K * N, MN = M * N, XS = (MK + 1) & ~1;
-  constexpr int G = 32 / N;                      // lane groups per warp
-  constexpr int NG = (STREAM_THREADS / 32) * G;  // lane groups per CTA
+  constexpr int MK = M * K, KN = K * N, MN = M * N, XS = (MK + 1) & ~1, NW = NT / 32;
   extern __shared__ __align__(16) unsigned char smem[];
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int b = blockIdx.x;
-  const int g = lane / N, c = lane % N;
-  const bool glive = g < G;
-  const int gid = warp * G + g;
+  const int br_nslots = PERSIST ? a.br_nslots[b] : 0;
 
-  const int acc0 = a.br_acc_ptr[b], nacc = a.br_acc_ptr[b + 1] - acc0;
-  double* accs = reinterpret_cast<double*>(smem);
-  unsigned char* chunk_base = smem + up16d((int64_t)nacc * MN * 8);
-  for (int e = tid; e < nacc * MN; e += STREAM_THREADS) accs[e] = 0.0;
+  double acc[MN];
+#pragma unroll
+  for (int e = 0; e < MN; ++e) acc[e] = 0.0;
 
   for (int ch = a.br_chunk_ptr[b]; ch < a.br_chunk_ptr[b + 1]; ++ch) {
-    const int nx = a.ch_nx[ch], ny = a.ch_ny[ch], nparts = a.ch_nparts[ch];
-    const int item0 = a.ch_item_ptr[ch], nitems = a.ch_item_ptr[ch + 1] - item0;
-    const int64_t code0 = a.ch_code_ptr[ch];
-    const int ncodes = (int)(a.ch_code_ptr[ch + 1] - code0);
-    double* Xs = reinterpret_cast<double*>(chunk_base);
-    double* Ys = reinterpret_cast<double*>(chunk_base + up16d((int64_t)nx * XS * 8));
-    double* parts = Ys + (up16d((int64_t)ny * KN * 8) >> 3);
-    CodeT* codes = reinterpret_cast<CodeT*>(reinterpret_cast<unsigned char*>(parts) + up16d((int64_t)nparts * MN * 8));
-    int32_t* items = reinterpret_cast<int32_t*>(reinterpret_cast<unsigned char*>(codes) + up16d((int64_t)ncodes * sizeof(CodeT)));
-    int32_t* gptr = items + (up16d((int64_t)nitems * 12) >> 2);
-    // ---- stage X (padded to XS doubles per block), Y, codes, items, group pointers
-    for (int r = a.ch_xrun_ptr[ch]; r < a.ch_xrun_ptr[ch + 1]; ++r) {
-      const StreamRun run = a.xruns[r];
-      if (MK % 2 == 0) {
-        const double2* src = reinterpret_cast<const double2*>(a.xvals + (int64_t)run.src * MK);
-        double2* dst = reinterpret_cast<double2*>(Xs + (int64_t)run.dst * XS);
-        for (int e = tid; e < run.n * (MK / 2); e += STREAM_THREADS) dst[e] = __ldcs(src + e);
-      } else {
-        const double* src = a.xvals + (int64_t)run.src * MK;
-        double* dst = Xs + (int64_t)run.dst * XS;
-        for (int e = tid; e < run.n * MK; e += STREAM_THREADS) {
-          const int blk = e / MK;
-          dst[blk * XS + (e - blk * MK)] = __ldcs(src + e);
-        }
-      }
-    }
-    for (int r = a.ch_yrun_ptr[ch]; r < a.ch_yrun_ptr[ch + 1]; ++r) {
-      const StreamRun run = a.yruns[r];
-      if (KN % 2 == 0) {
-        const double2* src = reinterpret_cast<const double2*>(a.yvals + (int64_t)run.src * KN);
-        double2* dst = reinterpret_cast<double2*>(Ys + (int64_t)run.dst * KN);
-        for (int e = tid; e < run.n * (KN / 2); e += STREAM_THREADS) dst[e] = __ldg(src + e);
-      } else {
-        const double* src = a.yvals + (int64_t)run.src * KN;
-        double* dst = Ys + (int64_t)run.dst * KN;
-        for (int e = tid; e < run.n * KN; e += STREAM_THREADS) dst[e] = __ldg(src + e);
-      }
-    }
+    const int64_t meta0 = a.ch_meta_ptr[ch];
+    const int nx = (int)(a.ch_meta_ptr[ch + 1] - meta0);  // even (padded by the plan)
+    const int ny = a.ch_ny[ch];
+    const int ent0 = a.ch_entry_ptr[ch], nent = a.ch_entry_ptr[ch + 1] - ent0;
+    const int pass0 = a.ch_pass_ptr[ch], npass = a.ch_pass_ptr[ch + 1] - pass0;
+    double* Xs = reinterpret_cast<double*>(smem);
+    StreamMeta* metas = reinterpret_cast<StreamMeta*>(smem + up16d((int64_t)nx * XS * 8));
+    double* Ys = reinterpret_cast<double*>(reinterpret_cast<unsigned char*>(metas) + up16d((int64_t)nx * 8));
+    StreamEntry* entries = reinterpret_cast<StreamEntry*>(reinterpret_cast<unsigned char*>(Ys) + up16d((int64_t)ny * KN * 8));
+    StreamPass* passes = reinterpret_cast<StreamPass*>(entries + nent);
+    // ---- stage X (padded to XS doubles per block), masks, Y, entries, passes.  Runs are dealt to the warps; a warp
+    // fetches the descriptors of up to 32 of its runs with one load per lane (one memory latency for all of them)
     {
-      const CodeT* src = reinterpret_cast<const CodeT*>(a.codes) + code0;
-      for (int e = tid; e < ncodes; e += STREAM_THREADS) codes[e] = __ldcs(src + e);
-      const int32_t* isrc = reinterpret_cast<const int32_t*>(a.items + item0);
-      for (int e = tid; e < nitems * 3; e += STREAM_THREADS) items[e] = __ldcs(isrc + e);
-      const int32_t* gsrc = a.ch_gptr + (int64_t)ch * (NG + 1);
-      for (int e = tid; e <= NG; e += STREAM_THREADS) gptr[e] = __ldcs(gsrc + e);
-    }
-    __syncthreads();
-    // ---- the product streams
-    {
-      int it = glive ? gptr[gid] : 0;
-      const int it_end = glive ? gptr[gid + 1] : 0;
-      int rem = 0, out = 0, xb = 0;
-      const CodeT* cp = codes;
-      double acc[M];
-#pragma unroll
-      for (int r = 0; r < M; ++r) acc[r] = 0.0;
-      while (true) {
-        const bool have = rem > 0 || it < it_end;
-        if (!__any_sync(0xffffffffu, have)) break;
-        if (have) {
-          if (rem == 0) {
-            out = items[3 * it];
-            cp = codes + items[3 * it + 1];
-            const uint32_t w = (uint32_t)items[3 * it + 2];
-            rem = (int)(w & 0xffffu);
-            xb = (int)(w >> 16);
-            ++it;
-#pragma unroll
-            for (int r = 0; r < M; ++r) acc[r] = 0.0;
-          }
-          const uint32_t code = (uint32_t)(*cp++);
-          const double* xp = Xs + (xb + (int)(code & ((1u << OXBITS) - 1u))) * XS;
-          const double* yp = Ys + (int)(code >> OXBITS) * KN + c;
-          double y[K], x[XS];
-#pragma unroll
-          for (int m = 0; m < K; ++m) y[m] = yp[m * N];
-#pragma unroll
-          for (int e = 0; e < XS / 2; ++e) {
-            const double2 t = reinterpret_cast<const double2*>(xp)[e];
-            x[2 * e] = t.x;
-            x[2 * e + 1] = t.y;
-          }
-#pragma unroll
-          for (int r = 0; r < M; ++r)
-#pragma unroll
-            for (int m = 0; m < K; ++m) acc[r] = fma(x[r * K + m], y[m], acc[r]);
-          if (--rem == 0) {
-            double* dst = (out >= 0) ? a.cvals + (int64_t)out * MN + c : parts + (-out - 1) * MN + c;
-#pragma unroll
-            for (int r = 0; r < M; ++r) dst[r * N] = acc[r];
+      const int xr0 = a.ch_xrun_ptr[ch], nxr = a.ch_xrun_ptr[ch + 1] - xr0;
+      const int yr0 = a.ch_yrun_ptr[ch], nyr = a.ch_yrun_ptr[ch + 1] - yr0;
+      const int nruns = nxr + nyr;  // X runs first
+      for (int base = warp; base < nruns; base += NW * 32) {
+        const int mine = base + lane * NW;
+        StreamRun run = {0, 0, 0};
+        if (mine < nruns) run = (mine < nxr) ? a.xruns[xr0 + mine] : a.yruns[yr0 + (mine - nxr)];
+        const int cnt = min(32, (nruns - base + NW - 1) / NW);
+        for (int t = 0; t < cnt; ++t) {
+          const int src = __shfl_sync(0xffffffffu, run.src, t), n = __shfl_sync(0xffffffffu, run.n, t);
+          const int dst = __shfl_sync(0xffffffffu, run.dst, t);
+          if (base + t * NW < nxr) {
+            if (MK % 2 == 0) {
+              const double2* gs = reinterpret_cast<const double2*>(a.xvals + (int64_t)src * MK);
+              double2* sd = reinterpret_cast<double2*>(Xs + (int64_t)dst * XS);
+              for (int e = lane; e < n * (MK / 2); e += 32) cp_async<16>(sd + e, gs + e);
+            } else {
+              const double* gs = a.xvals + (int64_t)src * MK;
+              double* sd = Xs + (int64_t)dst * XS;
+              for (int e = lane; e < n * MK; e += 32) {
+                const int blk = e / MK;
+                cp_async<8>(sd + blk * XS + (e - blk * MK), gs + e);
+              }
+            }
+          } else {
+            if (KN % 2 == 0) {
+              const double2* gs = reinterpret_cast<const double2*>(a.yvals + (int64_t)src * KN);
+              double2* sd = reinterpret_cast<double2*>(Ys + (int64_t)dst * KN);
+              for (int e = lane; e < n * (KN / 2); e += 32) cp_async<16>(sd + e, gs + e);
+            } else {
+              const double* gs = a.yvals + (int64_t)src * KN;
+              double* sd = Ys + (int64_t)dst * KN;
+              for (int e = lane; e < n * KN; e += 32) cp_async<8>(sd + e, gs + e);
+            }
           }
         }
       }
     }
-    __syncthreads();
-    // ---- parts -> brick accumulator, in plan order
     {
-      const int red0 = a.ch_red_ptr[ch], nred = a.ch_red_ptr[ch + 1] - red0;
-      for (int e = tid; e < nred * MN; e += STREAM_THREADS) {
-        const int ri = e / MN, el = e - ri * MN;
-        const StreamRed rd = a.reds[red0 + ri];
-        double v = accs[rd.acc * MN + el];
-        for (int q = 0; q < rd.nparts; ++q) v += parts[(rd.part0 + q) * MN + el];
-        accs[rd.acc * MN + el] = v;
+      const uint4* msrc = reinterpret_cast<const uint4*>(a.meta + meta0);
+      for (int e = tid; e < nx / 2; e += NT) cp_async<16>(reinterpret_cast<uint4*>(metas) + e, msrc + e);
+      const uint4* esrc = reinterpret_cast<const uint4*>(a.entries + ent0);
+      for (int e = tid; e < nent; e += NT) cp_async<16>(reinterpret_cast<uint4*>(entries) + e, esrc + e);
+      const uint4* psrc = reinterpret_cast<const uint4*>(a.passes + pass0);
+      for (int e = tid; e < npass; e += NT) cp_async<16>(reinterpret_cast<uint4*>(passes) + e, psrc + e);
+    }
+    cp_async_wait_all();
+    __syncthreads();
+    // ---- the passes of this warp
+    for (int p = warp; p < npass; p += NW) {
+      const StreamPass ps = passes[p];
+      int xbase = 0, len = 0, out = 0, slot = -1;
+      for (int e = ps.e0; e < ps.e1; ++e) {
+        const StreamEntry en = entries[e];
+        if (lane >= en.lane0 && lane < en.lane0 + en.nslots) {
+          xbase = en.xbase; len = en.len; out = en.out; slot = lane - en.lane0;
+        }
+      }
+      if (!PERSIST) {
+#pragma unroll
+        for (int e = 0; e < MN; ++e) acc[e] = 0.0;
+      }
+      const uint32_t below = slot >= 0 ? ((1u << slot) - 1u) : 0u;
+      for (int k = 0; k < ps.steps; ++k) {
+        if (slot >= 0 && k < len) {
+          const StreamMeta mt = metas[xbase + k];
+          if ((mt.mask >> slot) & 1u) {
+            const double* xp = Xs + (int64_t)(xbase + k) * XS;
+            const double* yp = Ys + (int64_t)(mt.ybase + __popc(mt.mask & below)) * KN;
+            double x[XS];
+            lds_block<XS>(xp, x);
+#pragma unroll
+            for (int m = 0; m < K; ++m) {
+              double y[N];
+              if ((N % 2 == 0)) lds_block<N>(yp + m * N, y);
+              else {
+#pragma unroll
+                for (int c = 0; c < N; ++c) y[c] = yp[m * N + c];
+              }
+#pragma unroll
+              for (int r = 0; r < M; ++r)
+#pragma unroll
+                for (int c = 0; c < N; ++c) acc[r * N + c] = fma(x[r * K + m], y[c], acc[r * N + c]);
+            }
+          }
+        }
+      }
+      if (!PERSIST && slot >= 0) {
+        double* dst = a.cvals + (int64_t)(out + slot) * MN;
+        if (MN % 2 == 0) {
+#pragma unroll
+          for (int e = 0; e < MN / 2; ++e) reinterpret_cast<double2*>(dst)[e] = make_double2(acc[2 * e], acc[2 * e + 1]);
+        } else {
+#pragma unroll
+          for (int e = 0; e < MN; ++e) dst[e] = acc[e];
+        }
       }
     }
     __syncthreads();
   }
-  // ---- the brick's accumulated blocks, written once
-  for (int e = tid; e < nacc * MN; e += STREAM_THREADS) {
-    const int ai = e / MN, el = e - ai * MN;
-    a.cvals[(int64_t)a.acc_slot[acc0 + ai] * MN + el] = accs[e];
+  if (PERSIST) {
+    // partial blocks of the NW warps, added in warp order; every coarse block is written once
+    double* part = reinterpret_cast<double*>(smem);
+    if (lane < br_nslots) {
+#pragma unroll
+      for (int e = 0; e < MN; ++e) part[((int64_t)warp * br_nslots + lane) * MN + e] = acc[e];
+    }
+    __syncthreads();
+    double* dst = a.cvals + (int64_t)a.br_out[b] * MN;
+    for (int e = tid; e < br_nslots * MN; e += NT) {
+      double v = part[e];
+#pragma unroll
+      for (int w = 1; w < NW; ++w) v += part[(int64_t)w * br_nslots * MN + e];
+      dst[e] = v;
+    }
   }
 }
 
 template <int M, int K, int N>
-static int stream_launch_mkn(const StreamArgs& a, bool wide, int64_t nbricks, int64_t smem, cudaStream_t st) {
+static int stream_launch_mkn(const StreamArgs& a, bool persist, int64_t nbricks, int64_t smem, cudaStream_t st) {
   if (nbricks == 0) return BSR_OK;
-  if (wide) {
-    auto kern = stream_product_kernel<M, K, N, uint32_t, 12>;
+  if (persist) {
+    auto kern = stream_product_kernel<M, K, N, STREAM_THREADS_PERSIST, true>;
     static int64_t set_smem = -1;
     if (smem > set_smem) {
       CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
       set_smem = smem;
     }
-    LAUNCH(kern, (unsigned)nbricks, STREAM_THREADS, (size_t)smem, st, a);
+    LAUNCH(kern, (unsigned)nbricks, STREAM_THREADS_PERSIST, (size_t)smem, st, a);
   } else {
-    auto kern = stream_product_kernel<M, K, N, uint16_t, 5>;
+    auto kern = stream_product_kernel<M, K, N, STREAM_THREADS_DIRECT, false>;
     static int64_t set_smem = -1;
     if (smem > set_smem) {
       CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
       set_smem = smem;
     }
-    LAUNCH(kern, (unsigned)nbricks, STREAM_THREADS, (size_t)smem, st, a);
+    LAUNCH(kern, (unsigned)nbricks, STREAM_THREADS_DIRECT, (size_t)smem, st, a);
   }
   return BSR_OK;
 }
 
-int stream_launch(int M, int K, int N, const StreamArgs& a, bool wide, int64_t nbricks, int64_t smem, cudaStream_t st) {
+int stream_launch(int M, int K, int N, const StreamArgs& a, bool persist, int64_t nbricks, int64_t smem, cudaStream_t st) {
   const int key = M * 100 + K * 10 + N;
   switch (key) {
-    case 222: return stream_launch_mkn<2, 2, 2>(a, wide, nbricks, smem, st);
-    case 223: return stream_launch_mkn<2, 2, 3>(a, wide, nbricks, smem, st);
-    case 323: return stream_launch_mkn<3, 2, 3>(a, wide, nbricks, smem, st);
-    case 332: return stream_launch_mkn<3, 3, 2>(a, wide, nbricks, smem, st);
-    case 232: return stream_launch_mkn<2, 3, 2>(a, wide, nbricks, smem, st);
-    case 333: return stream_launch_mkn<3, 3, 3>(a, wide, nbricks, smem, st);
-    case 336: return stream_launch_mkn<3, 3, 6>(a, wide, nbricks, smem, st);
-    case 636: return stream_launch_mkn<6, 3, 6>(a, wide, nbricks, smem, st);
-    case 663: return stream_launch_mkn<6, 6, 3>(a, wide, nbricks, smem, st);
-    case 363: return stream_launch_mkn<3, 6, 3>(a, wide, nbricks, smem, st);
-    case 666: return stream_launch_mkn<6, 6, 6>(a, wide, nbricks, smem, st);
+    case 222: return stream_launch_mkn<2, 2, 2>(a, persist, nbricks, smem, st);
+    case 223: return stream_launch_mkn<2, 2, 3>(a, persist, nbricks, smem, st);
+    case 323: return stream_launch_mkn<3, 2, 3>(a, persist, nbricks, smem, st);
+    case 332: return stream_launch_mkn<3, 3, 2>(a, persist, nbricks, smem, st);
+    case 232: return stream_launch_mkn<2, 3, 2>(a, persist, nbricks, smem, st);
+    case 333: return stream_launch_mkn<3, 3, 3>(a, persist, nbricks, smem, st);
+    case 336: return stream_launch_mkn<3, 3, 6>(a, persist, nbricks, smem, st);
+    case 636: return stream_launch_mkn<6, 3, 6>(a, persist, nbricks, smem, st);
+    case 663: return stream_launch_mkn<6, 6, 3>(a, persist, nbricks, smem, st);
+    case 363: return stream_launch_mkn<3, 6, 3>(a, persist, nbricks, smem, st);
+    case 666: return stream_launch_mkn<6, 6, 6>(a, persist, nbricks, smem, st);
   }
-  return fail(BSR_ERR_BLOCK, "no stream kernel for <%d,%d,%d>", M, K, N);
+  return fail(BSR_ERR_BLOCK, "no staged product kernel for <%d,%d,%d>", M, K, N);
 }
-
-int stream_groups(int N) { return (STREAM_THREADS / 32) * (32 / N); }
 
 }  // namespace bsramg
