@@ -142,6 +142,13 @@ struct StreamEntry {   // 16 bytes: one X row piece inside a pass
 struct StreamPass { int32_t e0, e1, steps, pad; };   // entries [e0, e1) (relative to the chunk), max len
 struct StreamMeta { uint32_t mask, ybase; };          // per staged X block: receiving slots, staged Y row start
 struct StreamRun { int32_t src, n, dst; };            // copy n blocks from global block src to staged block dst
+struct StreamBrickHdr { int32_t chunk0, nchunks, out, nslots; };   // out / nslots: persist bricks (C row of the brick)
+struct StreamChunkHdr {   // 64 bytes: everything a CTA needs to know about a chunk, fetched with one load
+  int64_t meta0;          // first staged X block in StreamPlan::meta
+  int32_t nx, ny;         // staged X blocks (even, padded) and Y blocks
+  int32_t ent0, nent, pass0, npass, xr0, nxr, yr0, nyr;
+  int32_t pad[4];
+};
 
 struct StreamPlan {
   bool ok = false;            // false: shapes / sizes outside this format -> caller keeps the gather kernel
@@ -149,18 +156,14 @@ struct StreamPlan {
   bool persist = false;
   int nwarps = 0;
   int64_t max_smem = 0;       // dynamic shared memory of the largest brick
-  std::vector<int32_t> br_chunk_ptr;   // nbricks + 1
-  std::vector<int32_t> br_out;         // persist: first C slot of the brick's row;  br_nslots: its slot count
-  std::vector<int32_t> br_nslots;
-  std::vector<int32_t> ch_xrun_ptr, ch_yrun_ptr, ch_entry_ptr, ch_pass_ptr;  // nchunks + 1
-  std::vector<int64_t> ch_meta_ptr;                                          // nchunks + 1 (staged X blocks)
-  std::vector<int32_t> ch_ny;                                                // staged Y blocks per chunk
+  std::vector<StreamBrickHdr> bricks;
+  std::vector<StreamChunkHdr> chunks;
   std::vector<StreamRun> xruns, yruns;
   std::vector<StreamEntry> entries;
   std::vector<StreamPass> passes;
   std::vector<StreamMeta> meta;
-  int64_t nbricks() const { return (int64_t)br_chunk_ptr.size() - 1; }
-  int64_t nchunks() const { return (int64_t)ch_ny.size(); }
+  int64_t nbricks() const { return (int64_t)bricks.size(); }
+  int64_t nchunks() const { return (int64_t)chunks.size(); }
 };
 
 struct StreamShape { int M, K, N; };   // C blocks M x N, X blocks M x K, Y blocks K x N

@@ -133,15 +133,8 @@ int stream_upload(const StreamPlan& sp, StreamDev& sd, cudaStream_t st) {
   sd = StreamDev();
   if (!sp.ok) return BSR_OK;
   StreamArgs& a = sd.args;
-  int rc = stream_up(sp.br_chunk_ptr, &a.br_chunk_ptr, sd, st);
-  if (rc == BSR_OK) rc = stream_up(sp.br_out, &a.br_out, sd, st);
-  if (rc == BSR_OK) rc = stream_up(sp.br_nslots, &a.br_nslots, sd, st);
-  if (rc == BSR_OK) rc = stream_up(sp.ch_xrun_ptr, &a.ch_xrun_ptr, sd, st);
-  if (rc == BSR_OK) rc = stream_up(sp.ch_yrun_ptr, &a.ch_yrun_ptr, sd, st);
-  if (rc == BSR_OK) rc = stream_up(sp.ch_entry_ptr, &a.ch_entry_ptr, sd, st);
-  if (rc == BSR_OK) rc = stream_up(sp.ch_pass_ptr, &a.ch_pass_ptr, sd, st);
-  if (rc == BSR_OK) rc = stream_up(sp.ch_ny, &a.ch_ny, sd, st);
-  if (rc == BSR_OK) rc = stream_up(sp.ch_meta_ptr, &a.ch_meta_ptr, sd, st);
+  int rc = stream_up(sp.bricks, &a.bricks, sd, st);
+  if (rc == BSR_OK) rc = stream_up(sp.chunks, &a.chunks, sd, st);
   if (rc == BSR_OK) rc = stream_up(sp.xruns, &a.xruns, sd, st);
   if (rc == BSR_OK) rc = stream_up(sp.yruns, &a.yruns, sd, st);
   if (rc == BSR_OK) rc = stream_up(sp.entries, &a.entries, sd, st);
@@ -310,14 +303,17 @@ int ptap_symbolic(ptap_plan_t* out, bsr_t A, bsr_t P, int32_t* nbrows_c, int64_t
     std::vector<StreamBrickDef> bricks;
     StreamPlan sp;
     const StreamShape sh1{pl->bf, pl->bf, pl->bc}, sh2{pl->bc, pl->bf, pl->bc};
-    stream_bricks_stage1(hp, sh1, STREAM_SMEM_BUDGET, A->h_rowptr.data(), A->h_colidx.data(), P->h_rowptr.data(), bricks);
-    stream_build(sh1, STREAM_THREADS_DIRECT / 32, STREAM_SMEM_BUDGET, bricks, A->h_rowptr.data(), A->h_colidx.data(),
+    // shared-memory budgets per brick (tuning knobs; defaults: two stage-1 bricks and three stage-2 bricks per SM)
+    const int64_t budget1 = getenv("BSRAMG_S1_SMEM") ? atoll(getenv("BSRAMG_S1_SMEM")) : STREAM_SMEM_BUDGET;
+    const int64_t budget2 = getenv("BSRAMG_S2_SMEM") ? atoll(getenv("BSRAMG_S2_SMEM")) : STREAM_SMEM_BUDGET_PERSIST;
+    stream_bricks_stage1(hp, sh1, budget1, A->h_rowptr.data(), A->h_colidx.data(), P->h_rowptr.data(), bricks);
+    stream_build(sh1, STREAM_THREADS_DIRECT / 32, budget1, bricks, A->h_rowptr.data(), A->h_colidx.data(),
                  P->h_rowptr.data(), hp.rowptr_ap.data(), hp.pairptr1.data(), hp.k1.data(), hp.q1.data(), sp);
     rc = stream_upload(sp, pl->s1, st);
     if (rc == BSR_OK) {
       const int nw2 = STREAM_THREADS_PERSIST / 32;
-      stream_bricks_stage2(hp, sh2, nw2, STREAM_SMEM_BUDGET, R->h_rowptr.data(), R->h_colidx.data(), bricks);
-      stream_build(sh2, nw2, STREAM_SMEM_BUDGET, bricks, R->h_rowptr.data(), R->h_colidx.data(), hp.rowptr_ap.data(),
+      stream_bricks_stage2(hp, sh2, nw2, budget2, R->h_rowptr.data(), R->h_colidx.data(), bricks);
+      stream_build(sh2, nw2, budget2, bricks, R->h_rowptr.data(), R->h_colidx.data(), hp.rowptr_ap.data(),
                    hp.rowptr_c.data(), hp.pairptr2.data(), hp.t2.data(), hp.s2.data(), sp);
       rc = stream_upload(sp, pl->s2, st);
     }

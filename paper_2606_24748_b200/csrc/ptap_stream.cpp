@@ -190,40 +190,31 @@ void stream_build(const StreamShape& sh, int nwarps, int64_t smem_budget, const 
   // ---- flatten
   int64_t nchunks = 0;
   for (const auto& lb : L) nchunks += (int64_t)lb.chunks.size();
-  out.br_chunk_ptr.resize((size_t)nb + 1);
-  out.br_out.resize((size_t)nb);
-  out.br_nslots.resize((size_t)nb);
-  out.ch_xrun_ptr.assign((size_t)nchunks + 1, 0);
-  out.ch_yrun_ptr.assign((size_t)nchunks + 1, 0);
-  out.ch_entry_ptr.assign((size_t)nchunks + 1, 0);
-  out.ch_pass_ptr.assign((size_t)nchunks + 1, 0);
-  out.ch_meta_ptr.assign((size_t)nchunks + 1, 0);
-  out.ch_ny.resize((size_t)nchunks);
+  out.bricks.resize((size_t)nb);
+  out.chunks.resize((size_t)nchunks);
   int64_t c = 0, nxr = 0, nyr = 0, nen = 0, npa = 0, nme = 0;
   for (int64_t b = 0; b < nb; ++b) {
     const LocalBrick& lb = L[(size_t)b];
-    out.br_chunk_ptr[(size_t)b] = (int32_t)c;
-    out.br_out[(size_t)b] = lb.out;
-    out.br_nslots[(size_t)b] = lb.nslots;
+    out.bricks[(size_t)b] = StreamBrickHdr{(int32_t)c, (int32_t)lb.chunks.size(), lb.out, lb.nslots};
     if (out.persist)
       out.max_smem = std::max<int64_t>(out.max_smem, up16((int64_t)nwarps * lb.nslots * sh.M * sh.N * 8));
     for (const auto& lc : lb.chunks) {
-      out.ch_xrun_ptr[(size_t)c] = (int32_t)nxr; out.ch_yrun_ptr[(size_t)c] = (int32_t)nyr;
-      out.ch_entry_ptr[(size_t)c] = (int32_t)nen; out.ch_pass_ptr[(size_t)c] = (int32_t)npa;
-      out.ch_meta_ptr[(size_t)c] = nme;
-      out.ch_ny[(size_t)c] = lc.ny;
+      StreamChunkHdr h;
+      memset(&h, 0, sizeof h);
+      h.meta0 = nme; h.nx = (int32_t)lc.meta.size(); h.ny = lc.ny;
+      h.ent0 = (int32_t)nen; h.nent = (int32_t)lc.entries.size();
+      h.pass0 = (int32_t)npa; h.npass = (int32_t)lc.passes.size();
+      h.xr0 = (int32_t)nxr; h.nxr = (int32_t)lc.xruns.size();
+      h.yr0 = (int32_t)nyr; h.nyr = (int32_t)lc.yruns.size();
+      out.chunks[(size_t)c] = h;
       out.max_smem = std::max(out.max_smem, stream_smem_bytes(sh, (int64_t)lc.meta.size(), lc.ny,
                                                               (int64_t)lc.entries.size(), (int64_t)lc.passes.size()));
       nxr += (int64_t)lc.xruns.size(); nyr += (int64_t)lc.yruns.size(); nen += (int64_t)lc.entries.size();
-      npa += (int64_t)lc.passes.size(); nme += ((int64_t)lc.meta.size() + 1) & ~int64_t(1);  // 16-byte aligned
+      npa += (int64_t)lc.passes.size(); nme += (int64_t)lc.meta.size();  // even per chunk: 16-byte aligned
       ++c;
     }
   }
-  out.br_chunk_ptr[(size_t)nb] = (int32_t)c;
-  out.ch_xrun_ptr[(size_t)c] = (int32_t)nxr; out.ch_yrun_ptr[(size_t)c] = (int32_t)nyr;
-  out.ch_entry_ptr[(size_t)c] = (int32_t)nen; out.ch_pass_ptr[(size_t)c] = (int32_t)npa;
-  out.ch_meta_ptr[(size_t)c] = nme;
-  if (nen >= (1LL << 31) || out.max_smem > smem_budget) {
+  if (nen >= (1LL << 31) || nxr >= (1LL << 31) || nyr >= (1LL << 31) || out.max_smem > smem_budget) {
     out.why = out.max_smem > smem_budget ? "a brick does not fit the shared memory budget" : "too many entries";
     return;
   }
@@ -232,13 +223,14 @@ void stream_build(const StreamShape& sh, int nwarps, int64_t smem_budget, const 
 #pragma omp parallel for schedule(dynamic, 16)
   for (int64_t b = 0; b < nb; ++b) {
     const LocalBrick& lb = L[(size_t)b];
-    int64_t cc = out.br_chunk_ptr[(size_t)b];
+    int64_t cc = out.bricks[(size_t)b].chunk0;
     for (const auto& lc : lb.chunks) {
-      std::copy(lc.xruns.begin(), lc.xruns.end(), out.xruns.begin() + out.ch_xrun_ptr[(size_t)cc]);
-      std::copy(lc.yruns.begin(), lc.yruns.end(), out.yruns.begin() + out.ch_yrun_ptr[(size_t)cc]);
-      std::copy(lc.entries.begin(), lc.entries.end(), out.entries.begin() + out.ch_entry_ptr[(size_t)cc]);
-      std::copy(lc.passes.begin(), lc.passes.end(), out.passes.begin() + out.ch_pass_ptr[(size_t)cc]);
-      std::copy(lc.meta.begin(), lc.meta.end(), out.meta.begin() + out.ch_meta_ptr[(size_t)cc]);
+      const StreamChunkHdr& h = out.chunks[(size_t)cc];
+      std::copy(lc.xruns.begin(), lc.xruns.end(), out.xruns.begin() + h.xr0);
+      std::copy(lc.yruns.begin(), lc.yruns.end(), out.yruns.begin() + h.yr0);
+      std::copy(lc.entries.begin(), lc.entries.end(), out.entries.begin() + h.ent0);
+      std::copy(lc.passes.begin(), lc.passes.end(), out.passes.begin() + h.pass0);
+      std::copy(lc.meta.begin(), lc.meta.end(), out.meta.begin() + h.meta0);
       ++cc;
     }
   }

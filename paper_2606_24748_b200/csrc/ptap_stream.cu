@@ -49,24 +49,29 @@ __device__ __forceinline__ void lds_block(const double* __restrict__ p, double (
 }
 
 template <int M, int K, int N, int NT, bool PERSIST>
-__global__ void __launch_bounds__(NT, 2)
+__global__ void __launch_bounds__(NT, PERSIST ? 3 : (NT >= 512 ? 1 : 2))
 stream_product_kernel(const StreamArgs a) {
   constexpr int MK = M * K, KN = K * N, MN = M * N, XS = (MK + 1) & ~1, NW = NT / 32;
   extern __shared__ __align__(16) unsigned char smem[];
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int b = blockIdx.x;
-  const int br_nslots = PERSIST ? a.br_nslots[b] : 0;
+  // brick and chunk headers: one 16-byte and one 64-byte broadcast load (a direct brick is its own single chunk, so
+  // both loads are issued together)
+  const int4 bh = __ldg(reinterpret_cast<const int4*>(a.bricks + b));  // chunk0, nchunks, out, nslots
+  const int br_nslots = bh.w;
 
   double acc[MN];
 #pragma unroll
   for (int e = 0; e < MN; ++e) acc[e] = 0.0;
 
-  for (int ch = a.br_chunk_ptr[b]; ch < a.br_chunk_ptr[b + 1]; ++ch) {
-    const int64_t meta0 = a.ch_meta_ptr[ch];
-    const int nx = (int)(a.ch_meta_ptr[ch + 1] - meta0);  // even (padded by the plan)
-    const int ny = a.ch_ny[ch];
-    const int ent0 = a.ch_entry_ptr[ch], nent = a.ch_entry_ptr[ch + 1] - ent0;
-    const int pass0 = a.ch_pass_ptr[ch], npass = a.ch_pass_ptr[ch + 1] - pass0;
+  for (int ci = 0; ci < (PERSIST ? bh.y : 1); ++ci) {
+    const int ch = PERSIST ? bh.x + ci : b;
+    const int4* hp = reinterpret_cast<const int4*>(a.chunks + ch);
+    const int4 h0 = __ldg(hp), h1 = __ldg(hp + 1), h2 = __ldg(hp + 2);
+    const int64_t meta0 = ((int64_t)(uint32_t)h0.x) | ((int64_t)h0.y << 32);
+    const int nx = h0.z, ny = h0.w;              // nx even (padded by the plan)
+    const int ent0 = h1.x, nent = h1.y, pass0 = h1.z, npass = h1.w;
+    const int xr0 = h2.x, nxr = h2.y, yr0 = h2.z, nyr = h2.w;
     double* Xs = reinterpret_cast<double*>(smem);
     StreamMeta* metas = reinterpret_cast<StreamMeta*>(smem + up16d((int64_t)nx * XS * 8));
     double* Ys = reinterpret_cast<double*>(reinterpret_cast<unsigned char*>(metas) + up16d((int64_t)nx * 8));
@@ -75,8 +80,6 @@ stream_product_kernel(const StreamArgs a) {
     // ---- stage X (padded to XS doubles per block), masks, Y, entries, passes.  Runs are dealt to the warps; a warp
     // fetches the descriptors of up to 32 of its runs with one load per lane (one memory latency for all of them)
     {
-      const int xr0 = a.ch_xrun_ptr[ch], nxr = a.ch_xrun_ptr[ch + 1] - xr0;
-      const int yr0 = a.ch_yrun_ptr[ch], nyr = a.ch_yrun_ptr[ch + 1] - yr0;
       const int nruns = nxr + nyr;  // X runs first
       for (int base = warp; base < nruns; base += NW * 32) {
         const int mine = base + lane * NW;
@@ -138,9 +141,12 @@ stream_product_kernel(const StreamArgs a) {
         for (int e = 0; e < MN; ++e) acc[e] = 0.0;
       }
       const uint32_t below = slot >= 0 ? ((1u << slot) - 1u) : 0u;
+      // the mask of step k+1 is fetched while step k computes (one shared-memory latency off the critical path)
+      StreamMeta nxt = metas[xbase];
       for (int k = 0; k < ps.steps; ++k) {
+        const StreamMeta mt = nxt;
+        nxt = metas[xbase + min(k + 1, max(len - 1, 0))];
         if (slot >= 0 && k < len) {
-          const StreamMeta mt = metas[xbase + k];
           if ((mt.mask >> slot) & 1u) {
             const double* xp = Xs + (int64_t)(xbase + k) * XS;
             const double* yp = Ys + (int64_t)(mt.ybase + __popc(mt.mask & below)) * KN;
@@ -183,7 +189,7 @@ stream_product_kernel(const StreamArgs a) {
       for (int e = 0; e < MN; ++e) part[((int64_t)warp * br_nslots + lane) * MN + e] = acc[e];
     }
     __syncthreads();
-    double* dst = a.cvals + (int64_t)a.br_out[b] * MN;
+    double* dst = a.cvals + (int64_t)bh.z * MN;
     for (int e = tid; e < br_nslots * MN; e += NT) {
       double v = part[e];
 #pragma unroll

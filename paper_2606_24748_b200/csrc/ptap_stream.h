@@ -7,11 +7,11 @@ namespace bsramg {
 constexpr int STREAM_THREADS_DIRECT = 256;           // stage 1: 8 warps per brick, two bricks per SM
 constexpr int STREAM_THREADS_PERSIST = 128;          // stage 2: 4 warps per coarse row (36 accumulators per lane)
 constexpr int64_t STREAM_SMEM_BUDGET = 112 * 1024;   // dynamic shared memory a brick may use (2 x (112+1) KB <= 228 KB)
+constexpr int64_t STREAM_SMEM_BUDGET_PERSIST = 75000;  // stage 2: three coarse rows per SM (register-limited)
 
 struct StreamArgs {  // all device pointers
-  const int32_t *br_chunk_ptr, *br_out, *br_nslots;
-  const int32_t *ch_xrun_ptr, *ch_yrun_ptr, *ch_entry_ptr, *ch_pass_ptr, *ch_ny;
-  const int64_t* ch_meta_ptr;
+  const StreamBrickHdr* bricks;
+  const StreamChunkHdr* chunks;
   const StreamRun *xruns, *yruns;
   const StreamEntry* entries;
   const StreamPass* passes;
