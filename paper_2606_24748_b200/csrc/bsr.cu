@@ -65,8 +65,11 @@ struct Shape {
 // y (op)= A x.  TEAM = number of lane groups that share one block row (1 or GPW).  U = blocks in flight per group.
 // Loads are unconditional (the block index is clamped to the row's last block, the product of a clamped step is
 // discarded) so that all U index, value and x loads of a step are issued before the first FMA.
-template <int BR, int BC, int TEAM, int U, int EPI>
-__global__ void __launch_bounds__(256, 4)  // a minimum CTA count makes ptxas keep the batched loads (56 regs)
+// MINB = resident CTAs per SM the register allocation is held to: stating it at all makes ptxas keep the batched loads;
+// 6 (40 registers, 48 warps per SM) is best for rows of a few steps (A, P), 4 (56 registers) for long rows (R) --
+// measured, profiles/r1e_spmv.md.
+template <int BR, int BC, int TEAM, int U, int EPI, int MINB>
+__global__ void __launch_bounds__(256, MINB)
 spmv_kernel(int32_t nbrows, const int32_t* __restrict__ rowptr, const int32_t* __restrict__ colidx,
             const double* __restrict__ vals, const double* __restrict__ x, double* __restrict__ y,
             const double* __restrict__ b) {
@@ -179,7 +182,7 @@ spmv_kernel(int32_t nbrows, const int32_t* __restrict__ rowptr, const int32_t* _
   }
 }
 
-template <int BR, int BC, int TEAM, int U>
+template <int BR, int BC, int TEAM, int U, int MINB>
 static int spmv_dispatch_epi(bsr_t A, const double* x, double* y, const double* b, Epilogue epi, cudaStream_t st) {
   using S = Shape<BR, BC>;
   constexpr int ROWS_PER_WARP = S::GPW / TEAM;
@@ -190,34 +193,38 @@ static int spmv_dispatch_epi(bsr_t A, const double* x, double* y, const double* 
   const dim3 grid((unsigned)blocks), block(256);
   switch (epi) {
     case EPI_ASSIGN:
-      LAUNCH((spmv_kernel<BR, BC, TEAM, U, EPI_ASSIGN>), grid, block, 0, st, A->nbrows, A->d_rowptr, A->d_colidx,
+      LAUNCH((spmv_kernel<BR, BC, TEAM, U, EPI_ASSIGN, MINB>), grid, block, 0, st, A->nbrows, A->d_rowptr, A->d_colidx,
              A->d_vals, x, y, b);
       break;
     case EPI_RESID:
-      LAUNCH((spmv_kernel<BR, BC, TEAM, U, EPI_RESID>), grid, block, 0, st, A->nbrows, A->d_rowptr, A->d_colidx,
+      LAUNCH((spmv_kernel<BR, BC, TEAM, U, EPI_RESID, MINB>), grid, block, 0, st, A->nbrows, A->d_rowptr, A->d_colidx,
              A->d_vals, x, y, b);
       break;
     case EPI_SUB:
-      LAUNCH((spmv_kernel<BR, BC, TEAM, U, EPI_SUB>), grid, block, 0, st, A->nbrows, A->d_rowptr, A->d_colidx,
+      LAUNCH((spmv_kernel<BR, BC, TEAM, U, EPI_SUB, MINB>), grid, block, 0, st, A->nbrows, A->d_rowptr, A->d_colidx,
              A->d_vals, x, y, b);
       break;
     default:
-      LAUNCH((spmv_kernel<BR, BC, TEAM, U, EPI_ADD>), grid, block, 0, st, A->nbrows, A->d_rowptr, A->d_colidx,
+      LAUNCH((spmv_kernel<BR, BC, TEAM, U, EPI_ADD, MINB>), grid, block, 0, st, A->nbrows, A->d_rowptr, A->d_colidx,
              A->d_vals, x, y, b);
       break;
   }
   return BSR_OK;
 }
 
+#ifndef SPMV_ROW_U
+#define SPMV_ROW_U 4
+#endif
 template <int BR, int BC>
 static int spmv_dispatch_team(bsr_t A, const double* x, double* y, const double* b, Epilogue epi, cudaStream_t st) {
   using S = Shape<BR, BC>;
   if (A->team_mode == 1) {
     // the whole warp on one block row: U steps of GPW blocks cover a 27-block row of A in one pass
     constexpr int U = (S::GPW >= 8) ? 2 : (S::GPW == 1 ? 8 : 9);
-    return spmv_dispatch_epi<BR, BC, S::GPW, U>(A, x, y, b, epi, st);
+    if (A->avg_row_len >= 2.0 * S::GPW * U) return spmv_dispatch_epi<BR, BC, S::GPW, U, 4>(A, x, y, b, epi, st);
+    return spmv_dispatch_epi<BR, BC, S::GPW, U, 6>(A, x, y, b, epi, st);
   }
-  return spmv_dispatch_epi<BR, BC, 1, 4>(A, x, y, b, epi, st);
+  return spmv_dispatch_epi<BR, BC, 1, SPMV_ROW_U, 6>(A, x, y, b, epi, st);
 }
 
 int spmv_launch(bsr_t A, const double* x, double* y, const double* b, Epilogue epi, cudaStream_t st) {
