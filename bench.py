@@ -64,7 +64,7 @@ class ClockSampler:
     def start(self):
         try:
             self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}",
-                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                          "--format=csv,noheader,nounits", "-lms", "20"],
                                          stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
             self.thread = threading.Thread(target=self._read, daemon=True)
             self.thread.start()
@@ -181,15 +181,35 @@ def run_reference(args) -> dict:
             "e2e": {"value": val, "unit": "GB/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
 
 
+# ------------------------------------------------------------------ ranks (one process per GPU, weak scaling)
+def rank_env():
+    return (int(os.environ.get("RANK", "0")), int(os.environ.get("WORLD_SIZE", "1")),
+            int(os.environ.get("LOCAL_RANK", "0")))
+
+
+def max_over_ranks(value: float, world: int, device) -> float:
+    """The job's time is the slowest rank's (every rank runs its own independent problem; no data-path collective)."""
+    if world <= 1:
+        return float(value)
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([value], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def job_value(bytes_per_rank: int, world: int, seconds: float) -> float:
+    """Whole-job GB/s: the units all ranks processed divided by the max-over-ranks time."""
+    return bytes_per_rank * world / seconds / 1e9
+
+
 # ------------------------------------------------------------------ the CUDA arm
 def run_ours(args) -> dict | None:
     import torch
     import torch.distributed as dist
     from paper_2606_24748_b200 import bsr, problems as pr
 
-    rank = int(os.environ.get("RANK", "0"))
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    local = int(os.environ.get("LOCAL_RANK", "0"))
+    rank, world, local = rank_env()
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device -- the product path has no CPU fallback")
     torch.cuda.set_device(local)
@@ -254,12 +274,9 @@ def run_ours(args) -> dict | None:
     ms_total = t_start.elapsed_time(t_end)
     per = {n: float(np.mean([evs[k][i].elapsed_time(evs[k][i + 1]) for k in range(args.steps)]))
            for i, n in enumerate(names)}
-    if world > 1:
-        t = torch.tensor([ms_total], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms_total = float(t.item())
+    ms_total = max_over_ranks(ms_total, world, dev)
     ms_step = ms_total / args.steps
-    value = total_bytes * world / (ms_step * 1e-3) / 1e9
+    value = job_value(total_bytes, world, ms_step * 1e-3)
     peak, peak_src = measured_peak()
 
     # ---- e2e: the same step through the C ABI's host-buffer calls (pinned host memory, copies inside the timed region)
@@ -285,11 +302,8 @@ def run_ours(args) -> dict | None:
         step_host()
     barrier()
     e2e_s = time.perf_counter() - t0
-    if world > 1:
-        t = torch.tensor([e2e_s], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        e2e_s = float(t.item())
-    e2e_val = total_bytes * world * e2e_steps / e2e_s / 1e9
+    e2e_s = max_over_ranks(e2e_s, world, dev)
+    e2e_val = job_value(total_bytes * e2e_steps, world, e2e_s)
 
     if rank != 0:
         if world > 1:
@@ -334,6 +348,11 @@ def run_ours(args) -> dict | None:
            "e2e": {"value": e2e_val, "unit": "GB/s", "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                    "ms_per_step": e2e_s / e2e_steps * 1e3, "steps": e2e_steps},
            "gpu_launches": int(l1 - l0), "allocs_in_timed_region": int(a1 - a0)}
+    if not args.no_vcycle:
+        # release the config-3 device arrays first (config 4 is a second, smaller problem)
+        del plan, GA, GP, x, xc, y, yc, vals_c
+        torch.cuda.empty_cache()
+        out["vcycle"] = run_vcycle(peak)
     if not args.no_cpu_baseline:
         op = OraclePass(A, P, seed)
         t = op.run()
@@ -343,6 +362,65 @@ def run_ours(args) -> dict | None:
     if world > 1:
         dist.destroy_process_group()
     return out
+
+
+def run_vcycle(peak: float, cfg: int = 4, reps: int = 10) -> dict:
+    """BASELINE.json's third number: V-cycle ms at config 4 (96^3, three levels, V(2,2) degree-2 Chebyshev / block
+    Jacobi, dense coarsest solve), plus the full hierarchy recompute and one PCG iteration.  The hierarchy is built
+    through the library (two ptap plans); the generator only needs the level-1 operator back on the host to form the
+    level-2 prolongator (cold setup)."""
+    import torch
+    from paper_2606_24748_b200 import bsr, problems as pr
+    g = pr.make_generator(cfg)
+    g.build_prolongator(0)
+    A0, P0 = g.A(0), g.P(0)
+    G0, GP0 = bsr.Bsr.from_host(A0), bsr.Bsr.from_host(P0)
+    plan0 = bsr.PtapPlan(G0, GP0)
+    v1 = plan0.numeric()
+    A1 = pr.HostBSR(plan0.nbrows_c, plan0.nbrows_c, P0.bs_c, P0.bs_c, plan0.rowptr_c.cpu().numpy(),
+                    plan0.colidx_c.cpu().numpy(), v1.cpu().numpy().reshape(-1, P0.bs_c, P0.bs_c))
+    g.set_operator(1, A1)
+    g.build_prolongator(1)
+    P1 = g.P(1)
+    G1, GP1 = plan0.coarse_matrix(v1), bsr.Bsr.from_host(P1)
+    plan1 = bsr.PtapPlan(G1, GP1)
+    v2 = plan1.numeric()
+    G2 = plan1.coarse_matrix(v2)
+    lams = [g.level_info(0)["lam"], g.level_info(1)["lam"]]
+    vc = bsr.VCycle([G0, G1, G2], [GP0, GP1], lams)
+    b = torch.from_numpy(pr.uniform(pr.CONFIGS[cfg]["seed"], pr.PURPOSE_RHS, A0.nbrows * A0.bs_r)).cuda()
+    xv = torch.empty_like(b)
+
+    def timed(fn, n):
+        for _ in range(3):
+            fn()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        e0.record()
+        for _ in range(n):
+            fn()
+        e1.record()
+        torch.cuda.synchronize()
+        return e0.elapsed_time(e1) / n
+
+    ms_v = timed(lambda: vc.apply(b, xv), reps)
+
+    def recompute():
+        plan0.numeric(v1); plan1.numeric(v2); vc.refresh(check=False)
+    ms_r = timed(recompute, 3)
+    ms_pcg = timed(lambda: vc.pcg(b, 5), 2) / 5
+    # algorithmic bytes of one application (SURVEY.md 8(d)): per non-coarsest level 4 A-SpMVs + restriction +
+    # prolongation and four reads of D^-1, plus the two triangular sweeps of the dense coarsest solve
+    nbytes = 0
+    for Al, Pl in ((A0, P0), (A1, P1)):
+        Rl = pr.HostBSR(Pl.nbcols, Pl.nbrows, Pl.bs_c, Pl.bs_r, None, Pl.colidx, None)
+        nbytes += 4 * spmv_bytes(Al) + spmv_bytes(Pl) + spmv_bytes(Rl) + 4 * 8 * Al.nbrows * Al.bs_r * Al.bs_r
+    nc = plan1.nbrows_c * P1.bs_c
+    nbytes += 8 * nc * nc
+    gbs = nbytes / (ms_v * 1e-3) / 1e9
+    return {"workload": pr.CONFIGS[cfg]["name"], "vcycle_ms": ms_v, "algorithmic_GB": nbytes / 1e9, "GB/s": gbs,
+            "frac_of_measured_hbm": gbs / peak, "frac_of_nominal_8TBs": gbs / NOMINAL_HBM_GBS,
+            "hierarchy_recompute_ms": ms_r, "pcg_iteration_ms": ms_pcg, "coarsest_unknowns": nc}
 
 
 def main():
@@ -355,6 +433,7 @@ def main():
     ap.add_argument("--ref-ne", type=int, default=64, help="sample grid of the reference arm (elements per side)")
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-vcycle", action="store_true", help="skip the config-4 V-cycle timing")
     args = ap.parse_args()
     if args.impl == "reference":
         if int(os.environ.get("RANK", "0")) != 0:
