@@ -49,7 +49,7 @@ __device__ __forceinline__ void lds_block(const double* __restrict__ p, double (
 }
 
 template <int M, int K, int N, int NT, bool PERSIST>
-__global__ void __launch_bounds__(NT, PERSIST ? 3 : (NT >= 512 ? 1 : 2))
+__global__ void __launch_bounds__(NT, PERSIST ? 3 : STREAM_MINB1)
 stream_product_kernel(const StreamArgs a) {
   constexpr int MK = M * K, KN = K * N, MN = M * N, XS = (MK + 1) & ~1, NW = NT / 32;
   extern __shared__ __align__(16) unsigned char smem[];

@@ -4,7 +4,13 @@
 
 namespace bsramg {
 
-constexpr int STREAM_THREADS_DIRECT = 256;           // stage 1: 8 warps per brick, two bricks per SM
+#ifndef STREAM_NT1
+#define STREAM_NT1 256
+#endif
+#ifndef STREAM_MINB1
+#define STREAM_MINB1 2
+#endif
+constexpr int STREAM_THREADS_DIRECT = STREAM_NT1;           // stage 1: 8 warps per brick, two bricks per SM
 constexpr int STREAM_THREADS_PERSIST = 128;          // stage 2: 4 warps per coarse row (36 accumulators per lane)
 constexpr int64_t STREAM_SMEM_BUDGET = 112 * 1024;   // dynamic shared memory a brick may use (2 x (112+1) KB <= 228 KB)
 constexpr int64_t STREAM_SMEM_BUDGET_PERSIST = 75000;  // stage 2: three coarse rows per SM (register-limited)
