@@ -327,10 +327,13 @@ def run_ours(args) -> dict | None:
     dom = max(names, key=lambda n: per[n])
     ach = kb[dom] / (per[dom] * 1e-3) / 1e9
     traffic = None
-    tp = os.path.join(ROOT, "profiles", "ncu_traffic.json")  # written by hand from the ncu --set full capture
+    tp = os.path.join(ROOT, "profiles", "ncu_traffic.csv")  # copied by hand from the ncu --set full capture
     if os.path.exists(tp):
         try:
-            traffic = json.load(open(tp)).get(dom)
+            for ln in open(tp).read().splitlines()[1:]:
+                k, v = ln.split(",")
+                if k.strip() == dom:
+                    traffic = int(v)
         except Exception:
             traffic = None
     roofline = {"bound": "hbm", "kernel": dom, "achieved": ach, "peak": peak, "peak_source": peak_src, "unit": "GB/s",
