@@ -422,6 +422,7 @@ int bsr_destroy(bsr_t A) {
     delete A->T;
   }
   dev_free(A->T_perm);
+  dev_free(A->stage_x); dev_free(A->stage_y);
   A->magic = 0;
   delete A;
   return BSR_OK;
@@ -473,16 +474,17 @@ int bsr_spmv_host(bsr_t A, int32_t trans, const double* h_x, double* h_y, void* 
   cudaStream_t st = (cudaStream_t)stream;
   const size_t nx = (size_t)(trans ? A->nbrows * (int64_t)A->bs_r : A->nbcols * (int64_t)A->bs_c);
   const size_t ny = (size_t)(trans ? A->nbcols * (int64_t)A->bs_c : A->nbrows * (int64_t)A->bs_r);
-  double *dx = nullptr, *dy = nullptr;
-  int rc = dev_alloc_t(&dx, nx);
-  if (rc == BSR_OK) rc = dev_alloc_t(&dy, ny);
+  // staging vectors live on the handle: allocated at first use (cold), reused afterwards
+  int rc = BSR_OK;
+  if (A->stage_nx < nx) { dev_free(A->stage_x); A->stage_x = nullptr; A->stage_nx = 0; rc = dev_alloc_t(&A->stage_x, nx); if (rc == BSR_OK) A->stage_nx = nx; }
+  if (rc == BSR_OK && A->stage_ny < ny) { dev_free(A->stage_y); A->stage_y = nullptr; A->stage_ny = 0; rc = dev_alloc_t(&A->stage_y, ny); if (rc == BSR_OK) A->stage_ny = ny; }
+  double *dx = A->stage_x, *dy = A->stage_y;
   if (rc == BSR_OK && cudaMemcpyAsync(dx, h_x, nx * 8, cudaMemcpyHostToDevice, st) != cudaSuccess)
     rc = fail(BSR_ERR_CUDA, "H2D copy failed");
   if (rc == BSR_OK) rc = trans ? bsr_spmv_t(A, dx, dy, stream) : bsr_spmv(A, dx, dy, stream);
   if (rc == BSR_OK && cudaMemcpyAsync(h_y, dy, ny * 8, cudaMemcpyDeviceToHost, st) != cudaSuccess)
     rc = fail(BSR_ERR_CUDA, "D2H copy failed");
   if (rc == BSR_OK && cudaStreamSynchronize(st) != cudaSuccess) rc = fail(BSR_ERR_CUDA, "stream synchronise failed");
-  dev_free(dx); dev_free(dy);
   return rc;
 }
 

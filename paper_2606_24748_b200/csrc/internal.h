@@ -115,6 +115,9 @@ struct bsr_matrix_s {
   int64_t T_state = -1;       // state of this matrix when T's values were last built
   int64_t T_builds = 0;
   bool owns_arrays = false;  // true for library-created matrices (the transposes)
+  // staging vectors of the *_host convenience calls (allocated at first use, kept)
+  double *stage_x = nullptr, *stage_y = nullptr;
+  size_t stage_nx = 0, stage_ny = 0;
 };
 static const uint64_t BSR_MAGIC = 0x425352414d473031ull;
 
