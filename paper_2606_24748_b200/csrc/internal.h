@@ -152,6 +152,7 @@ struct StreamChunkHdr {   // 64 bytes: everything a CTA needs to know about a ch
   int32_t ent0, nent, pass0, npass, xr0, nxr, yr0, nyr;
   int32_t pad[4];
 };
+static_assert(sizeof(StreamChunkHdr) == 64 && sizeof(StreamBrickHdr) == 16, "headers are fetched with 16-byte loads");
 
 struct StreamPlan {
   bool ok = false;            // false: shapes / sizes outside this format -> caller keeps the gather kernel
