@@ -13,6 +13,7 @@
 //   All index / value / x loads of U steps are issued before the first FMA.  The row sum is finished with warp
 //   shuffles in a fixed order (deterministic); the epilogue (y = Ax, b - Ax, y -= Ax, y += Ax) is fused in.
 #include <algorithm>
+#include <cstdlib>
 #include <cstring>
 
 #include "internal.h"
@@ -212,6 +213,95 @@ static int spmv_dispatch_epi(bsr_t A, const double* x, double* y, const double* 
   return BSR_OK;
 }
 
+// ------------------------------------------------------------------ short rows: flat value stream (ROWPAIR shapes)
+// Rows of a handful of blocks (the prolongator: 1-8 blocks of 3x6) leave the row-per-lane-group kernel waiting on the
+// chain rowptr -> (colidx, values) -> x for every three rows.  Here a CTA takes FLAT_ROWS consecutive block rows, whose
+// values are ONE contiguous run: every thread streams 16-byte pairs of that run (perfectly coalesced, no clamped
+// steps, loads independent of the row pointers), multiplies by the matching x pair and parks the partial product in
+// shared memory; then one thread per output entry adds its row's partials in a fixed order (block by block, pair by
+// pair) and applies the epilogue.  Deterministic, no atomics.
+constexpr int FLAT_ROWS = 64;
+constexpr int FLAT_THREADS = 256;
+constexpr int FLAT_U = 4;
+
+template <int BR, int BC, int EPI>
+__global__ void __launch_bounds__(FLAT_THREADS, 4)
+spmv_flat_kernel(int32_t nbrows, const int32_t* __restrict__ rowptr, const int32_t* __restrict__ colidx,
+                 const double* __restrict__ vals, const double* __restrict__ x, double* __restrict__ y,
+                 const double* __restrict__ b) {
+  using S = Shape<BR, BC>;
+  static_assert(S::ROWPAIR, "flat kernel needs 16-byte pairs inside one block row");
+  constexpr int LB = S::LB, LPR = S::LPR;
+  extern __shared__ __align__(16) unsigned char flat_smem[];
+  int32_t* rp = reinterpret_cast<int32_t*>(flat_smem);                 // FLAT_ROWS + 1 row pointers
+  double* part = reinterpret_cast<double*>(flat_smem + ((FLAT_ROWS + 1) * 4 + 15) / 16 * 16);
+  const int tid = threadIdx.x;
+  const int32_t r0 = blockIdx.x * FLAT_ROWS, r1 = min(r0 + FLAT_ROWS, nbrows);
+  if (tid <= r1 - r0) rp[tid] = __ldg(rowptr + r0 + tid);
+  const int32_t k0 = __ldg(rowptr + r0), k1 = __ldg(rowptr + r1);
+  const int32_t T = (k1 - k0) * LB;                                    // 16-byte pairs of the CTA's run
+  const double2* v2 = reinterpret_cast<const double2*>(vals) + (int64_t)k0 * LB;
+  for (int32_t c = tid; c < T; c += FLAT_THREADS * FLAT_U) {
+    int32_t cu[FLAT_U], col[FLAT_U];
+    double2 v[FLAT_U], xv[FLAT_U];
+#pragma unroll
+    for (int u = 0; u < FLAT_U; ++u) {
+      cu[u] = min(c + u * FLAT_THREADS, T - 1);                        // clamped: the tail repeats the last pair
+      col[u] = __ldg(colidx + k0 + cu[u] / LB);
+    }
+#pragma unroll
+    for (int u = 0; u < FLAT_U; ++u) v[u] = __ldcs(v2 + cu[u]);
+#pragma unroll
+    for (int u = 0; u < FLAT_U; ++u)
+      xv[u] = __ldg(reinterpret_cast<const double2*>(x + (int64_t)col[u] * BC) + (cu[u] % LB) % LPR);
+#pragma unroll
+    for (int u = 0; u < FLAT_U; ++u)
+      if (c + u * FLAT_THREADS < T) part[cu[u]] = fma(v[u].y, xv[u].y, v[u].x * xv[u].x);
+  }
+  __syncthreads();
+  for (int o = tid; o < (r1 - r0) * BR; o += FLAT_THREADS) {
+    const int rl = o / BR, r = o - rl * BR;
+    const int32_t ks = rp[rl] - k0, ke = rp[rl + 1] - k0;
+    double sum = 0.0;
+    for (int32_t kk = ks; kk < ke; ++kk) {
+#pragma unroll
+      for (int cv = 0; cv < LPR; ++cv) sum += part[kk * LB + r * LPR + cv];
+    }
+    const int64_t oi = (int64_t)(r0 + rl) * BR + r;
+    if (EPI == EPI_ASSIGN) y[oi] = sum;
+    else if (EPI == EPI_RESID) y[oi] = b[oi] - sum;
+    else if (EPI == EPI_SUB) y[oi] = y[oi] - sum;
+    else y[oi] = y[oi] + sum;
+  }
+}
+
+template <int BR, int BC>
+static int spmv_flat_launch(bsr_t A, const double* x, double* y, const double* b, Epilogue epi, cudaStream_t st) {
+  using S = Shape<BR, BC>;
+  const int64_t blocks = ((int64_t)A->nbrows + FLAT_ROWS - 1) / FLAT_ROWS;
+  if (blocks == 0) return BSR_OK;
+  const size_t smem = ((FLAT_ROWS + 1) * 4 + 15) / 16 * 16 + (size_t)A->flat_max_blocks * S::LB * 8;
+  const dim3 grid((unsigned)blocks), block(FLAT_THREADS);
+#define FLAT_CASE(E)                                                                                          \
+  {                                                                                                           \
+    auto kern = spmv_flat_kernel<BR, BC, E>;                                                                  \
+    static size_t set_smem = 0;                                                                               \
+    if (smem > 48 * 1024 && smem > set_smem) {                                                                \
+      CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));           \
+      set_smem = smem;                                                                                        \
+    }                                                                                                         \
+    LAUNCH(kern, grid, block, smem, st, A->nbrows, A->d_rowptr, A->d_colidx, A->d_vals, x, y, b);             \
+  }
+  switch (epi) {
+    case EPI_ASSIGN: FLAT_CASE(EPI_ASSIGN) break;
+    case EPI_RESID: FLAT_CASE(EPI_RESID) break;
+    case EPI_SUB: FLAT_CASE(EPI_SUB) break;
+    default: FLAT_CASE(EPI_ADD) break;
+  }
+#undef FLAT_CASE
+  return BSR_OK;
+}
+
 #ifndef SPMV_ROW_U
 #define SPMV_ROW_U 4
 #endif
@@ -223,6 +313,11 @@ static int spmv_dispatch_team(bsr_t A, const double* x, double* y, const double*
     constexpr int U = (S::GPW >= 8) ? 2 : (S::GPW == 1 ? 8 : 9);
     if (A->avg_row_len >= 2.0 * S::GPW * U) return spmv_dispatch_epi<BR, BC, S::GPW, U, 4>(A, x, y, b, epi, st);
     return spmv_dispatch_epi<BR, BC, S::GPW, U, 6>(A, x, y, b, epi, st);
+  }
+  if constexpr (S::ROWPAIR) {
+    // short rows of a pair-able shape: the flat stream kernel, if a CTA's partials fit in shared memory
+    if (!getenv("BSRAMG_NO_FLAT") && (size_t)A->flat_max_blocks * S::LB * 8 <= 96 * 1024)
+      return spmv_flat_launch<BR, BC>(A, x, y, b, epi, st);
   }
   return spmv_dispatch_epi<BR, BC, 1, SPMV_ROW_U, 6>(A, x, y, b, epi, st);
 }
@@ -275,6 +370,13 @@ transpose_values_kernel(int64_t nvals, int br, int bc, const int32_t* __restrict
   tvals[e] = __ldg(vals + (int64_t)__ldg(perm + t) * bb + r * bc + c);
 }
 
+// most blocks any run of FLAT_ROWS consecutive rows (one CTA of the flat SpMV) holds
+static int32_t flat_max_blocks_of(const std::vector<int32_t>& rp, int32_t nbrows) {
+  int32_t mx = 0;
+  for (int32_t r0 = 0; r0 < nbrows; r0 += FLAT_ROWS) mx = std::max(mx, rp[(size_t)std::min(r0 + FLAT_ROWS, nbrows)] - rp[(size_t)r0]);
+  return mx;
+}
+
 static void choose_team_mode(bsr_t A) {
   // the whole warp shares a row only when the row keeps every lane group busy for a few steps
   int gpw = 1;
@@ -315,6 +417,7 @@ int transpose_ensure(bsr_t A, cudaStream_t st) {
     for (int32_t j = 0; j < T->nbrows; ++j) mx = std::max(mx, rp[(size_t)j + 1] - rp[j]);
     T->max_row_len = mx;
     T->avg_row_len = T->nbrows ? (double)T->nnzb / T->nbrows : 0.0;
+    T->flat_max_blocks = flat_max_blocks_of(rp, T->nbrows);
     T->h_rowptr.swap(rp);
     T->h_colidx.swap(ci);
     choose_team_mode(T);
@@ -402,6 +505,7 @@ int bsr_create(bsr_t* out, int32_t nbrows, int32_t nbcols, int32_t bs_r, int32_t
   A->magic = BSR_MAGIC;
   A->max_row_len = mx;
   A->avg_row_len = nbrows ? (double)nnzb / nbrows : 0.0;
+  A->flat_max_blocks = flat_max_blocks_of(A->h_rowptr, nbrows);
   choose_team_mode(A);
   *out = A;
   return BSR_OK;

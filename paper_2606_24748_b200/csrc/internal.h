@@ -109,6 +109,7 @@ struct bsr_matrix_s {
   int32_t max_row_len = 0;
   double avg_row_len = 0;
   int team_mode = 0;  // 0: one lane group per row, 1: the whole warp per row
+  int32_t flat_max_blocks = 0;  // most blocks in any run of 64 consecutive rows (flat SpMV shared-memory size)
   // cached explicit transpose (library-owned)
   bsr_matrix_s* T = nullptr;
   int32_t* T_perm = nullptr;  // device: source slot per transposed slot
