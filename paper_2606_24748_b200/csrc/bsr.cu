@@ -220,12 +220,21 @@ static int spmv_dispatch_epi(bsr_t A, const double* x, double* y, const double* 
 // steps, loads independent of the row pointers), multiplies by the matching x pair and parks the partial product in
 // shared memory; then one thread per output entry adds its row's partials in a fixed order (block by block, pair by
 // pair) and applies the epilogue.  Deterministic, no atomics.
-constexpr int FLAT_ROWS = 64;
+#ifndef FLAT_ROWS_N
+#define FLAT_ROWS_N 64
+#endif
+#ifndef FLAT_U_N
+#define FLAT_U_N 4
+#endif
+#ifndef FLAT_MINB
+#define FLAT_MINB 6
+#endif
+constexpr int FLAT_ROWS = FLAT_ROWS_N;
 constexpr int FLAT_THREADS = 256;
-constexpr int FLAT_U = 4;
+constexpr int FLAT_U = FLAT_U_N;
 
 template <int BR, int BC, int EPI>
-__global__ void __launch_bounds__(FLAT_THREADS, 4)
+__global__ void __launch_bounds__(FLAT_THREADS, FLAT_MINB)
 spmv_flat_kernel(int32_t nbrows, const int32_t* __restrict__ rowptr, const int32_t* __restrict__ colidx,
                  const double* __restrict__ vals, const double* __restrict__ x, double* __restrict__ y,
                  const double* __restrict__ b) {
