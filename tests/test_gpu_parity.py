@@ -100,6 +100,29 @@ def test_spmv_edge_structures(bsr):
     assert G.spmv(torch.empty(0, dtype=torch.float64, device="cuda")).numel() == 0
 
 
+def test_spmv_flat_short_rows(bsr):
+    """Short-row matrices of pair-able shapes take the flat value-stream kernel: many CTAs, empty rows, a ragged last
+    CTA, rows of 1..8 blocks, and an all-empty matrix."""
+    import torch
+    rng = np.random.default_rng(11)
+    for (br, bc) in [(3, 6), (2, 2), (6, 6)]:
+        nbrows, nbcols = 1003, 400
+        lens = rng.integers(0, 9, size=nbrows)
+        lens[5:70] = 0                                           # a whole CTA's worth of empty rows
+        if (br, bc) == (6, 6):
+            lens = np.minimum(lens, 1)                           # keeps 6x6 in row mode (average below 2)
+        rowptr = np.concatenate([[0], np.cumsum(lens)]).astype(np.int32)
+        cols = np.concatenate([np.sort(rng.choice(nbcols, n, replace=False)) for n in lens] + [np.zeros(0, int)]).astype(np.int32)
+        vals = rng.uniform(-1, 1, (cols.shape[0], br, bc))
+        M = pr.HostBSR(nbrows, nbcols, br, bc, rowptr, cols, vals)
+        G = check_spmv(bsr, M, 21)
+        x = dev(pr.uniform(2, pr.PURPOSE_FINE, nbcols * bc))
+        assert torch.equal(G.spmv(x), G.spmv(x))
+    Z = pr.HostBSR(300, 10, 3, 6, np.zeros(301, np.int32), np.zeros(0, np.int32), np.zeros((0, 3, 6)))
+    y = bsr.Bsr.from_host(Z).spmv(dev(np.ones(60)))
+    assert float(y.abs().max()) == 0.0
+
+
 def test_bsr_create_rejects_malformed(bsr):
     import torch
     ok = pr.HostBSR(2, 3, 3, 3, np.array([0, 2, 3], np.int32), np.array([0, 2, 1], np.int32), np.ones((3, 3, 3)))
