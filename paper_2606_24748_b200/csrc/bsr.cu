@@ -68,7 +68,7 @@ struct Shape {
 // discarded) so that all U index, value and x loads of a step are issued before the first FMA.
 // MINB = resident CTAs per SM the register allocation is held to: stating it at all makes ptxas keep the batched loads;
 // 6 (40 registers, 48 warps per SM) is best for rows of a few steps (A, P), 4 (56 registers) for long rows (R) --
-// measured, profiles/r1e_spmv.md.
+// measured, profiles/r1f_staged_ptap.md.
 template <int BR, int BC, int TEAM, int U, int EPI, int MINB>
 __global__ void __launch_bounds__(256, MINB)
 spmv_kernel(int32_t nbrows, const int32_t* __restrict__ rowptr, const int32_t* __restrict__ colidx,
