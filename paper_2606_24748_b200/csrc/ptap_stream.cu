@@ -33,6 +33,34 @@ __device__ __forceinline__ void cp_async_wait_all() {
   asm volatile("cp.async.commit_group;\n\tcp.async.wait_group 0;" ::: "memory");
 }
 
+// ---- bulk (TMA) copies: one thread moves a whole run of blocks global -> shared; completion is counted in bytes on
+// an mbarrier.  Used for every operand whose blocks are a multiple of 16 bytes (everything but 3x3 X blocks, which
+// are padded on the way in); the shared-memory side is written in full lines by the copy engine instead of one
+// 16-byte LDGSTS wavefront per sector (profiles/r1g_final.md: 11.5 wavefronts per 512-byte LDGSTS.128).
+__device__ __forceinline__ void mbar_init(uint64_t* bar, int count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"((unsigned)__cvta_generic_to_shared(bar)), "r"(count));
+  asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, unsigned bytes) {
+  asm volatile("mbarrier.expect_tx.relaxed.cta.shared::cta.b64 [%0], %1;" ::"r"((unsigned)__cvta_generic_to_shared(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint64_t* bar) {
+  asm volatile("{ .reg .b64 st; mbarrier.arrive.shared::cta.b64 st, [%0]; }" ::"r"((unsigned)__cvta_generic_to_shared(bar)) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, unsigned phase) {
+  unsigned done;
+  do {
+    asm volatile("{ .reg .pred p; mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2; selp.u32 %0, 1, 0, p; }"
+                 : "=r"(done) : "r"((unsigned)__cvta_generic_to_shared(bar)), "r"(phase) : "memory");
+  } while (!done);
+}
+__device__ __forceinline__ void bulk_g2s(void* dst_smem, const void* src, unsigned bytes, uint64_t* bar) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+               ::"r"((unsigned)__cvta_generic_to_shared(dst_smem)), "l"(src), "r"(bytes),
+                 "r"((unsigned)__cvta_generic_to_shared(bar)) : "memory");
+}
+__device__ __forceinline__ void fence_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+
 template <int NE>
 __device__ __forceinline__ void lds_block(const double* __restrict__ p, double (&v)[NE]) {  // p 16-byte aligned if NE even
   if (NE % 2 == 0) {
@@ -59,6 +87,12 @@ stream_product_kernel(const StreamArgs a) {
   // both loads are issued together)
   const int4 bh = __ldg(reinterpret_cast<const int4*>(a.bricks + b));  // chunk0, nchunks, out, nslots
   const int br_nslots = bh.w;
+  constexpr bool XBULK = (MK % 2 == 0), YBULK = (KN % 2 == 0);   // runs of whole 16-byte multiples
+  __shared__ uint64_t bulk_bar;
+  if (XBULK || YBULK) {
+    if (tid == 0) mbar_init(&bulk_bar, NT);
+    __syncthreads();
+  }
 
   double acc[MN];
 #pragma unroll
@@ -84,17 +118,24 @@ stream_product_kernel(const StreamArgs a) {
       for (int base = warp; base < nruns; base += NW * 32) {
         const int mine = base + lane * NW;
         StreamRun run = {0, 0, 0};
-        if (mine < nruns) run = (mine < nxr) ? a.xruns[xr0 + mine] : a.yruns[yr0 + (mine - nxr)];
+        const bool have = mine < nruns, isx = mine < nxr;
+        if (have) run = isx ? a.xruns[xr0 + mine] : a.yruns[yr0 + (mine - nxr)];
+        // runs of 16-byte-multiple blocks: this lane hands its run to the copy engine
+        if (have && isx && XBULK && run.n > 0) {
+          mbar_expect_tx(&bulk_bar, (unsigned)run.n * MK * 8);
+          bulk_g2s(Xs + (int64_t)run.dst * XS, a.xvals + (int64_t)run.src * MK, (unsigned)run.n * MK * 8, &bulk_bar);
+        }
+        if (have && !isx && YBULK && run.n > 0) {
+          mbar_expect_tx(&bulk_bar, (unsigned)run.n * KN * 8);
+          bulk_g2s(Ys + (int64_t)run.dst * KN, a.yvals + (int64_t)run.src * KN, (unsigned)run.n * KN * 8, &bulk_bar);
+        }
+        if ((XBULK || nxr == 0) && YBULK) continue;   // nothing left for the LDGSTS path
         const int cnt = min(32, (nruns - base + NW - 1) / NW);
         for (int t = 0; t < cnt; ++t) {
           const int src = __shfl_sync(0xffffffffu, run.src, t), n = __shfl_sync(0xffffffffu, run.n, t);
           const int dst = __shfl_sync(0xffffffffu, run.dst, t);
           if (base + t * NW < nxr) {
-            if (MK % 2 == 0) {
-              const double2* gs = reinterpret_cast<const double2*>(a.xvals + (int64_t)src * MK);
-              double2* sd = reinterpret_cast<double2*>(Xs + (int64_t)dst * XS);
-              for (int e = lane; e < n * (MK / 2); e += 32) cp_async<16>(sd + e, gs + e);
-            } else {
+            if (!XBULK) {   // padded blocks: element by element
               const double* gs = a.xvals + (int64_t)src * MK;
               double* sd = Xs + (int64_t)dst * XS;
               for (int e = lane; e < n * MK; e += 32) {
@@ -102,16 +143,10 @@ stream_product_kernel(const StreamArgs a) {
                 cp_async<8>(sd + blk * XS + (e - blk * MK), gs + e);
               }
             }
-          } else {
-            if (KN % 2 == 0) {
-              const double2* gs = reinterpret_cast<const double2*>(a.yvals + (int64_t)src * KN);
-              double2* sd = reinterpret_cast<double2*>(Ys + (int64_t)dst * KN);
-              for (int e = lane; e < n * (KN / 2); e += 32) cp_async<16>(sd + e, gs + e);
-            } else {
-              const double* gs = a.yvals + (int64_t)src * KN;
-              double* sd = Ys + (int64_t)dst * KN;
-              for (int e = lane; e < n * KN; e += 32) cp_async<8>(sd + e, gs + e);
-            }
+          } else if (!YBULK) {
+            const double* gs = a.yvals + (int64_t)src * KN;
+            double* sd = Ys + (int64_t)dst * KN;
+            for (int e = lane; e < n * KN; e += 32) cp_async<8>(sd + e, gs + e);
           }
         }
       }
@@ -125,6 +160,10 @@ stream_product_kernel(const StreamArgs a) {
       for (int e = tid; e < npass; e += NT) cp_async<16>(reinterpret_cast<uint4*>(passes) + e, psrc + e);
     }
     cp_async_wait_all();
+    if (XBULK || YBULK) {
+      mbar_arrive(&bulk_bar);              // every thread has posted the bytes of its runs
+      mbar_wait(&bulk_bar, (unsigned)(ci & 1));
+    }
     __syncthreads();
     // ---- the passes of this warp
     for (int p = warp; p < npass; p += NW) {
@@ -179,6 +218,7 @@ stream_product_kernel(const StreamArgs a) {
         }
       }
     }
+    if (XBULK || YBULK) fence_async_smem();   // generic-proxy reads of this chunk before the next chunk's bulk writes
     __syncthreads();
   }
   if (PERSIST) {
