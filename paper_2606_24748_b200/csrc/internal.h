@@ -139,9 +139,10 @@ struct StreamEntry {   // 16 bytes: one X row piece inside a pass
   int32_t out;         // first slot of C's row (direct) / first accumulator of the row (persist)
   int32_t xbase;       // staged X block index of the piece's first block
   int32_t len;         // number of X blocks (steps)
-  uint8_t lane0;       // first lane of the row's slots in the warp
-  uint8_t nslots;      // slots of the row (<= 32)
-  uint8_t pad0, pad1;
+  uint8_t lane0;       // first lane of this entry in the warp
+  uint8_t nslots;      // output blocks of the row held by this entry's lanes
+  uint8_t slot0;       // first of them inside the row (a row's blocks may be split over two passes)
+  uint8_t pad1;
 };
 struct StreamPass { int32_t e0, e1, steps, pad; };   // entries [e0, e1) (relative to the chunk), max len
 struct StreamMeta { uint32_t mask, ybase; };          // per staged X block: receiving slots, staged Y row start

@@ -137,41 +137,40 @@ void stream_build(const StreamShape& sh, int nwarps, int64_t smem_budget, const 
         if (lc.meta.size() & 1) lc.meta.push_back(StreamMeta{0u, 0u});  // even count: 16-byte staging
         // ---- passes
         if (bd.direct) {
-          // whole rows, packed into warps of 32 lanes: first fit, most slots first
+          // the output blocks of all rows, longest rows first, laid end to end and cut every 32 lanes: a pass holds
+          // whole rows and at most two row fragments (a row split over two warps is walked by both)
           const size_t np = cd.pieces.size();
           order.resize(np);
           std::iota(order.begin(), order.end(), 0);
           auto nsl = [&](int32_t pi) { return rowptr_c[cd.pieces[(size_t)pi].row + 1] - rowptr_c[cd.pieces[(size_t)pi].row]; };
-          std::stable_sort(order.begin(), order.end(), [&](int32_t u, int32_t v) { return nsl(u) > nsl(v); });
-          std::vector<std::vector<int32_t>> bins;
-          std::vector<int32_t> used;
-          for (int32_t pi : order) {
-            const int32_t ns = nsl(pi);
-            if (cd.pieces[(size_t)pi].t0 != 0) lb.bad = true;
-            size_t bi = 0;
-            while (bi < bins.size() && used[bi] + ns > 32) ++bi;
-            if (bi == bins.size()) { bins.emplace_back(); used.push_back(0); }
-            bins[bi].push_back(pi);
-            used[bi] += ns;
-          }
-          std::vector<int32_t> steps(bins.size(), 0), border(bins.size());
-          for (size_t bi = 0; bi < bins.size(); ++bi)
-            for (int32_t pi : bins[bi]) steps[bi] = std::max(steps[bi], cd.pieces[(size_t)pi].t1 - cd.pieces[(size_t)pi].t0);
-          std::iota(border.begin(), border.end(), 0);
-          std::stable_sort(border.begin(), border.end(), [&](int32_t u, int32_t v) { return steps[(size_t)u] > steps[(size_t)v]; });
-          for (int32_t bi : border) {
-            StreamPass ps{(int32_t)lc.entries.size(), 0, steps[(size_t)bi], 0};
-            int32_t lane0 = 0;
-            for (int32_t pi : bins[(size_t)bi]) {
-              const StreamPiece& pc = cd.pieces[(size_t)pi];
-              const int32_t ns = nsl(pi);
-              lc.entries.push_back(StreamEntry{rowptr_c[pc.row], piece_xbase[(size_t)pi], pc.t1 - pc.t0, (uint8_t)lane0,
-                                               (uint8_t)ns, 0, 0});
-              lane0 += ns;
+          auto plen = [&](int32_t pi) { return cd.pieces[(size_t)pi].t1 - cd.pieces[(size_t)pi].t0; };
+          std::stable_sort(order.begin(), order.end(), [&](int32_t u, int32_t v) { return plen(u) > plen(v); });
+          StreamPass ps{0, 0, 0, 0};
+          int32_t lane0 = 0;
+          auto close_pass = [&]() {
+            if ((int32_t)lc.entries.size() > ps.e0) {
+              ps.e1 = (int32_t)lc.entries.size();
+              lc.passes.push_back(ps);
             }
-            ps.e1 = (int32_t)lc.entries.size();
-            lc.passes.push_back(ps);
+            ps = StreamPass{(int32_t)lc.entries.size(), 0, 0, 0};
+            lane0 = 0;
+          };
+          for (int32_t pi : order) {
+            const StreamPiece& pc = cd.pieces[(size_t)pi];
+            if (pc.t0 != 0) lb.bad = true;
+            int32_t s0 = 0;
+            const int32_t ns = nsl(pi);
+            while (s0 < ns) {
+              const int32_t take = std::min(ns - s0, 32 - lane0);
+              lc.entries.push_back(StreamEntry{rowptr_c[pc.row], piece_xbase[(size_t)pi], plen(pi), (uint8_t)lane0,
+                                               (uint8_t)take, (uint8_t)s0, 0});
+              ps.steps = std::max(ps.steps, plen(pi));
+              lane0 += take;
+              s0 += take;
+              if (lane0 == 32) close_pass();
+            }
           }
+          close_pass();
         } else {
           // the chunk's piece of the row, cut into nwarps contiguous shares: pass w belongs to warp w
           const StreamPiece& pc = cd.pieces[0];

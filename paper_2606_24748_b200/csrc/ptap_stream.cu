@@ -172,7 +172,7 @@ stream_product_kernel(const StreamArgs a) {
       for (int e = ps.e0; e < ps.e1; ++e) {
         const StreamEntry en = entries[e];
         if (lane >= en.lane0 && lane < en.lane0 + en.nslots) {
-          xbase = en.xbase; len = en.len; out = en.out; slot = lane - en.lane0;
+          xbase = en.xbase; len = en.len; out = en.out; slot = en.slot0 + lane - en.lane0;
         }
       }
       if (!PERSIST) {
