@@ -4,8 +4,9 @@
 // product"), PAPER.md:97-99, 248-250 (coarse blocks summed through a precomputed block plan, contiguous bs_r*bs_c
 // runs).  Schedule format: internal.h / ptap_stream.cpp.
 //
-// One CTA = one brick.  Per chunk it stages, with asynchronous coalesced copies, the X blocks (A rows / a piece of an
-// R row), every Y row they reference (P rows / AP rows) and the per-block masks in shared memory.  A lane owns one
+// One CTA = one brick.  Per chunk it stages the X blocks (A rows / a piece of an R row), every Y row they reference
+// (P rows / AP rows) and the per-block masks in shared memory: runs of 16-byte-multiple blocks by TMA bulk copies
+// (cp.async.bulk, bytes counted on an mbarrier), padded 3x3 blocks and the small tables by cp.async.  A lane owns one
 // output block (M x N accumulators in registers); its warp walks the X blocks of the row in order.  At step k all
 // lanes of a row read X(row,k) -- one shared-memory broadcast -- and the lanes whose bit is set in the block's mask
 // read consecutive blocks of Y's row, so every shared-memory access is a broadcast or contiguous (the gathers that

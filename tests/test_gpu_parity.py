@@ -229,6 +229,34 @@ def test_ptap_recompute_reuse_and_state_gate(bsr, probs):
     assert e.value.code == 7
 
 
+def _random_bsr(rng, nbrows, nbcols, br, bc, row_len):
+    lens = np.minimum(rng.integers(1, row_len + 1, size=nbrows), nbcols)
+    rowptr = np.concatenate([[0], np.cumsum(lens)]).astype(np.int32)
+    cols = np.concatenate([np.sort(rng.choice(nbcols, n, replace=False)) for n in lens]).astype(np.int32)
+    return pr.HostBSR(nbrows, nbcols, br, bc, rowptr, cols, rng.uniform(-1, 1, (cols.shape[0], br, bc)))
+
+
+def test_ptap_unstructured_falls_back_to_gather_kernels(bsr):
+    """A product outside the staged format (AP / A_c rows with more than 32 blocks: random A and P) keeps the gather
+    kernels; results must be the same definition."""
+    rng = np.random.default_rng(5)
+    A = _random_bsr(rng, 120, 120, 3, 3, 12)
+    P = _random_bsr(rng, 120, 60, 3, 6, 9)
+    (rap, cap), (rc, cc) = orc.ptap_symbolic(A, P)
+    assert np.diff(rap).max() > 32 or np.diff(rc).max() > 32
+    ptap_check(bsr, A, P)
+
+
+def test_ptap_gather_path_matches_staged_path(bsr, probs, monkeypatch):
+    """BSRAMG_NO_STREAM forces the gather kernels on a structured problem: same structure, values within rounding."""
+    g = probs["hex13"]
+    A, P = g.A(0), g.P(0)
+    _, _, _, staged, ref, mag = ptap_check(bsr, A, P)
+    monkeypatch.setenv("BSRAMG_NO_STREAM", "1")
+    _, _, _, gathered, _, _ = ptap_check(bsr, A, P)
+    assert blockwise_rel_err(gathered, staged, mag) < 1e-13
+
+
 def test_ptap_shape_errors(bsr, probs):
     g = probs["cfg0"]
     A, P = g.A(0), g.P(0)
