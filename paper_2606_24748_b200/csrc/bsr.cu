@@ -69,7 +69,7 @@ struct Shape {
 // MINB = resident CTAs per SM the register allocation is held to: stating it at all makes ptxas keep the batched loads;
 // 6 (40 registers, 48 warps per SM) is best for rows of a few steps (A, P), 4 (56 registers) for long rows (R) --
 // measured, profiles/r1f_staged_ptap.md.
-template <int BR, int BC, int TEAM, int U, int EPI, int MINB>
+template <int BR, int BC, int TEAM, int U, int EPI, int MINB, int RB>
 __global__ void __launch_bounds__(256, MINB)
 spmv_kernel(int32_t nbrows, const int32_t* __restrict__ rowptr, const int32_t* __restrict__ colidx,
             const double* __restrict__ vals, const double* __restrict__ x, double* __restrict__ y,
@@ -81,16 +81,25 @@ spmv_kernel(int32_t nbrows, const int32_t* __restrict__ rowptr, const int32_t* _
   const int g = lane / S::LB;  // lane group
   const int q = lane % S::LB;  // lane inside the group
   const int team = g / TEAM, member = g % TEAM;
-  const int64_t row = warp * ROWS_PER_WARP + team;
-  const bool live = (g < ROWS_PER_WARP * TEAM) && (row < nbrows);
+  const bool glive = g < ROWS_PER_WARP * TEAM;
   // element(s) of the block this lane owns
   const int eA = S::PAIR ? 2 * q : q;
   const int cA = eA % BC;
   const int cB = (eA + 1) % BC;  // PAIR && !ROWPAIR only
-
+  // A warp takes RB consecutive row groups; their row pointers come in with ONE load per lane, so only the first
+  // group of a warp pays the rowptr -> values dependency with a cold row pointer.
+  static_assert(RB * ROWS_PER_WARP + 1 <= 32, "row pointers of a batch must fit one load per lane");
+  const int64_t row_first = warp * (RB * ROWS_PER_WARP);
+  if (row_first >= nbrows) return;  // warp-uniform
+  const int32_t rp_lane = __ldg(rowptr + min(row_first + lane, (int64_t)nbrows));
+#pragma unroll 1
+  for (int j = 0; j < RB; ++j) {
+  const int ri = j * ROWS_PER_WARP + (glive ? team : 0);
+  const int64_t row = row_first + ri;
+  const bool live = glive && (row < nbrows);
+  const int32_t k0 = __shfl_sync(0xffffffffu, rp_lane, ri), k1 = __shfl_sync(0xffffffffu, rp_lane, ri + 1);
   double accA = 0.0, accB = 0.0;
   if (live) {
-    const int32_t k0 = __ldg(rowptr + row), k1 = __ldg(rowptr + row + 1);
     for (int32_t k = k0 + member; k < k1; k += TEAM * U) {
       bool ok[U];
       int32_t kc[U], col[U];
@@ -181,12 +190,13 @@ spmv_kernel(int32_t nbrows, const int32_t* __restrict__ rowptr, const int32_t* _
     else if (EPI == EPI_SUB) y[o] = y[o] - out;
     else y[o] = y[o] + out;
   }
+  }  // batch of row groups
 }
 
-template <int BR, int BC, int TEAM, int U, int MINB>
+template <int BR, int BC, int TEAM, int U, int MINB, int RB>
 static int spmv_dispatch_epi(bsr_t A, const double* x, double* y, const double* b, Epilogue epi, cudaStream_t st) {
   using S = Shape<BR, BC>;
-  constexpr int ROWS_PER_WARP = S::GPW / TEAM;
+  constexpr int ROWS_PER_WARP = (S::GPW / TEAM) * RB;
   const int64_t warps = ((int64_t)A->nbrows + ROWS_PER_WARP - 1) / ROWS_PER_WARP;
   const int64_t blocks = (warps + 7) / 8;
   if (blocks == 0) return BSR_OK;
@@ -194,19 +204,19 @@ static int spmv_dispatch_epi(bsr_t A, const double* x, double* y, const double* 
   const dim3 grid((unsigned)blocks), block(256);
   switch (epi) {
     case EPI_ASSIGN:
-      LAUNCH((spmv_kernel<BR, BC, TEAM, U, EPI_ASSIGN, MINB>), grid, block, 0, st, A->nbrows, A->d_rowptr, A->d_colidx,
+      LAUNCH((spmv_kernel<BR, BC, TEAM, U, EPI_ASSIGN, MINB, RB>), grid, block, 0, st, A->nbrows, A->d_rowptr, A->d_colidx,
              A->d_vals, x, y, b);
       break;
     case EPI_RESID:
-      LAUNCH((spmv_kernel<BR, BC, TEAM, U, EPI_RESID, MINB>), grid, block, 0, st, A->nbrows, A->d_rowptr, A->d_colidx,
+      LAUNCH((spmv_kernel<BR, BC, TEAM, U, EPI_RESID, MINB, RB>), grid, block, 0, st, A->nbrows, A->d_rowptr, A->d_colidx,
              A->d_vals, x, y, b);
       break;
     case EPI_SUB:
-      LAUNCH((spmv_kernel<BR, BC, TEAM, U, EPI_SUB, MINB>), grid, block, 0, st, A->nbrows, A->d_rowptr, A->d_colidx,
+      LAUNCH((spmv_kernel<BR, BC, TEAM, U, EPI_SUB, MINB, RB>), grid, block, 0, st, A->nbrows, A->d_rowptr, A->d_colidx,
              A->d_vals, x, y, b);
       break;
     default:
-      LAUNCH((spmv_kernel<BR, BC, TEAM, U, EPI_ADD, MINB>), grid, block, 0, st, A->nbrows, A->d_rowptr, A->d_colidx,
+      LAUNCH((spmv_kernel<BR, BC, TEAM, U, EPI_ADD, MINB, RB>), grid, block, 0, st, A->nbrows, A->d_rowptr, A->d_colidx,
              A->d_vals, x, y, b);
       break;
   }
@@ -314,21 +324,30 @@ static int spmv_flat_launch(bsr_t A, const double* x, double* y, const double* b
 #ifndef SPMV_ROW_U
 #define SPMV_ROW_U 4
 #endif
+#ifndef SPMV_RB_LONG
+#define SPMV_RB_LONG 1
+#endif
 template <int BR, int BC>
 static int spmv_dispatch_team(bsr_t A, const double* x, double* y, const double* b, Epilogue epi, cudaStream_t st) {
   using S = Shape<BR, BC>;
   if (A->team_mode == 1) {
     // the whole warp on one block row: U steps of GPW blocks cover a 27-block row of A in one pass
     constexpr int U = (S::GPW >= 8) ? 2 : (S::GPW == 1 ? 8 : 9);
-    if (A->avg_row_len >= 2.0 * S::GPW * U) return spmv_dispatch_epi<BR, BC, S::GPW, U, 4>(A, x, y, b, epi, st);
-    return spmv_dispatch_epi<BR, BC, S::GPW, U, 6>(A, x, y, b, epi, st);
+    if (A->avg_row_len >= 2.0 * S::GPW * U) return spmv_dispatch_epi<BR, BC, S::GPW, U, 4, SPMV_RB_LONG>(A, x, y, b, epi, st);
+#ifndef SPMV_RB
+#define SPMV_RB 4
+#endif
+#ifndef SPMV_MINB_SHORT
+#define SPMV_MINB_SHORT 6
+#endif
+    return spmv_dispatch_epi<BR, BC, S::GPW, U, SPMV_MINB_SHORT, SPMV_RB>(A, x, y, b, epi, st);
   }
   if constexpr (S::ROWPAIR) {
     // short rows of a pair-able shape: the flat stream kernel, if a CTA's partials fit in shared memory
     if (!getenv("BSRAMG_NO_FLAT") && (size_t)A->flat_max_blocks * S::LB * 8 <= 96 * 1024)
       return spmv_flat_launch<BR, BC>(A, x, y, b, epi, st);
   }
-  return spmv_dispatch_epi<BR, BC, 1, SPMV_ROW_U, 6>(A, x, y, b, epi, st);
+  return spmv_dispatch_epi<BR, BC, 1, SPMV_ROW_U, 6, 1>(A, x, y, b, epi, st);
 }
 
 int spmv_launch(bsr_t A, const double* x, double* y, const double* b, Epilogue epi, cudaStream_t st) {
