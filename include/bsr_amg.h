@@ -146,6 +146,12 @@ int ptap_destroy(ptap_plan_t plan);
 void* ptap_host_plan_build(int32_t nbrows_a, const int32_t* rowptr_a, const int32_t* colidx_a, int32_t nbcols_p,
                            const int32_t* rowptr_p, const int32_t* colidx_p);
 int ptap_host_plan_get(void* handle, const char* name, const void** ptr, int64_t* count, int32_t* elem_bytes);
+/* Host side of the staged numeric schedule (cold part of ptap_symbolic), for tests: builds the brick / chunk / pass
+ * plan of stage 1 (AP = A*P) or stage 2 (A_c = R*AP) for fine / coarse block sizes bs_f / bs_c under a shared-memory
+ * budget and reports out8 = { plan usable (1/0), bricks, chunks, largest brick's shared memory in bytes, set mask bits
+ * (= block products covered, each exactly once), lanes over all entries, passes, steps over all passes }. */
+int ptap_host_stream_stats(void* handle, int32_t bs_f, int32_t bs_c, int32_t stage, int64_t smem_budget,
+                           int64_t* out8);
 void ptap_host_plan_free(void* handle);
 
 /* ------------------------------------------------------------------ V-cycle and PCG

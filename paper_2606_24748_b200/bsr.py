@@ -42,6 +42,7 @@ SYMBOLS = {
     "ptap_destroy": (C.c_int, [_V]),
     "ptap_host_plan_build": (C.c_void_p, [_I32, _V, _V, _I32, _V, _V]),
     "ptap_host_plan_get": (C.c_int, [_V, C.c_char_p, _PV, _PI64, _PI32]),
+    "ptap_host_stream_stats": (C.c_int, [_V, _I32, _I32, _I32, _I64, _PI64]),
     "ptap_host_plan_free": (None, [_V]),
     "vcycle_create": (C.c_int, [_PV, _I32, _PV, _PV, C.POINTER(_D), _I32, _D, _D, _V]),
     "vcycle_refresh": (C.c_int, [_V, _V]),
@@ -270,6 +271,13 @@ class HostPlan:
                 else:
                     arr = np.empty(0, dt)
                 setattr(self, name, arr)
+            self.stream_stats = {}
+            if getattr(A, "bs_r", None) and getattr(P, "bs_c", None):
+                for stage, budget in ((1, 112 * 1024), (2, 75000)):
+                    o = (C.c_int64 * 8)()
+                    _check(lib().ptap_host_stream_stats(h, A.bs_r, P.bs_c, stage, budget, o))
+                    self.stream_stats[stage] = dict(zip(["ok", "bricks", "chunks", "max_smem", "mask_bits", "lanes",
+                                                         "passes", "steps"], [int(v) for v in o]))
         finally:
             lib().ptap_host_plan_free(h)
 

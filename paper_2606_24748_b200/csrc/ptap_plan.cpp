@@ -158,6 +158,7 @@ extern "C" {
 struct ptap_host_plan_s {
   HostPlan plan;
   std::vector<int32_t> rowptr_r, colidx_r, perm_r;
+  std::vector<int32_t> rowptr_a, colidx_a, rowptr_p;   // copies, for ptap_host_stream_stats
 };
 
 void* ptap_host_plan_build(int32_t nbrows_a, const int32_t* rowptr_a, const int32_t* colidx_a, int32_t nbcols_p,
@@ -169,6 +170,9 @@ void* ptap_host_plan_build(int32_t nbrows_a, const int32_t* rowptr_a, const int3
   ptap_host_plan_s* h = new (std::nothrow) ptap_host_plan_s();
   if (!h) { fail(BSR_ERR_ALLOC, "host allocation failed"); return nullptr; }
   host_transpose_structure(nbrows_a, nbcols_p, rowptr_p, colidx_p, h->rowptr_r, h->colidx_r, h->perm_r);
+  h->rowptr_a.assign(rowptr_a, rowptr_a + nbrows_a + 1);
+  h->colidx_a.assign(colidx_a, colidx_a + rowptr_a[nbrows_a]);
+  h->rowptr_p.assign(rowptr_p, rowptr_p + nbrows_a + 1);
   int rc = h->plan.build(nbrows_a, rowptr_a, colidx_a, nbcols_p, rowptr_p, colidx_p, h->rowptr_r.data(),
                          h->colidx_r.data());
   if (rc != BSR_OK) {
@@ -193,6 +197,33 @@ int ptap_host_plan_get(void* handle, const char* name, const void** ptr, int64_t
 #undef I32
 #undef U16
   return fail(BSR_ERR_NULL, "ptap_host_plan_get: unknown array '%s'", name);
+}
+
+int ptap_host_stream_stats(void* handle, int32_t bs_f, int32_t bs_c, int32_t stage, int64_t smem_budget,
+                           int64_t* out8) {
+  if (!handle || !out8 || (stage != 1 && stage != 2)) return fail(BSR_ERR_NULL, "ptap_host_stream_stats: bad argument");
+  ptap_host_plan_s* h = (ptap_host_plan_s*)handle;
+  const HostPlan& hp = h->plan;
+  std::vector<StreamBrickDef> bricks;
+  StreamPlan sp;
+  if (stage == 1) {
+    const StreamShape sh{bs_f, bs_f, bs_c};
+    stream_bricks_stage1(hp, sh, smem_budget, h->rowptr_a.data(), h->colidx_a.data(), h->rowptr_p.data(), bricks);
+    stream_build(sh, 8, smem_budget, bricks, h->rowptr_a.data(), h->colidx_a.data(), h->rowptr_p.data(),
+                 hp.rowptr_ap.data(), hp.pairptr1.data(), hp.k1.data(), hp.q1.data(), sp);
+  } else {
+    const StreamShape sh{bs_c, bs_f, bs_c};
+    stream_bricks_stage2(hp, sh, 4, smem_budget, h->rowptr_r.data(), h->colidx_r.data(), bricks);
+    stream_build(sh, 4, smem_budget, bricks, h->rowptr_r.data(), h->colidx_r.data(), hp.rowptr_ap.data(),
+                 hp.rowptr_c.data(), hp.pairptr2.data(), hp.t2.data(), hp.s2.data(), sp);
+  }
+  int64_t bits = 0, lanes = 0, steps = 0;
+  for (const StreamMeta& m : sp.meta) bits += __builtin_popcount(m.mask);
+  for (const StreamEntry& e : sp.entries) lanes += e.nslots;
+  for (const StreamPass& p : sp.passes) steps += p.steps;
+  out8[0] = sp.ok ? 1 : 0; out8[1] = sp.nbricks(); out8[2] = sp.nchunks(); out8[3] = sp.max_smem;
+  out8[4] = bits; out8[5] = lanes; out8[6] = (int64_t)sp.passes.size(); out8[7] = steps;
+  return BSR_OK;
 }
 
 void ptap_host_plan_free(void* handle) { delete (ptap_host_plan_s*)handle; }

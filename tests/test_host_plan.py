@@ -101,3 +101,22 @@ def test_host_plan_rejects_nothing_silently_on_empty_rows():
     assert np.array_equal(hp.rowptr_ap, rap) and np.array_equal(hp.colidx_ap, cap)
     assert np.array_equal(hp.rowptr_c, rc) and np.array_equal(hp.colidx_c, cc)
     assert hp.rowptr_c.tolist() == [0, 1, 1]
+
+
+def test_staged_schedule_covers_every_product_once():
+    """Host logic of the staged numeric PtAP (ptap_stream.cpp): the per-block masks of both stages must hold exactly
+    one bit per block product of the gather plan, every brick must fit its shared-memory budget, and stage 2 has one
+    brick per coarse row."""
+    from paper_2606_24748_b200 import bsr, problems as pr
+    for g in (pr.make_generator(0), pr.Generator(2, 24, seed=3), pr.Generator(3, 13, seed=5)):
+        g.build_prolongator(0)
+        A, P = g.A(0), g.P(0)
+        hp = bsr.HostPlan(A, P)
+        s1, s2 = hp.stream_stats[1], hp.stream_stats[2]
+        assert s1["ok"] == 1 and s2["ok"] == 1
+        assert s1["mask_bits"] == hp.k1.shape[0]          # stage 1: every A(i,j)*P(j,J) product once
+        assert s2["mask_bits"] == hp.t2.shape[0]          # stage 2: every R(I,i)*AP(i,K) product once
+        assert s1["max_smem"] <= 112 * 1024 and s2["max_smem"] <= 75000
+        assert s2["bricks"] == P.nbcols and s2["chunks"] >= s2["bricks"]
+        assert s1["lanes"] == hp.colidx_ap.shape[0]       # one lane per AP block
+        assert s1["passes"] * 32 >= s1["lanes"] and s1["steps"] > 0
