@@ -91,9 +91,11 @@ def test_structure_counts(d, ne):
 
 
 def test_nnz_per_row_matches_paper():
-    # PAPER.md:210-217 (Table 4): Q1 operator has ~76 nonzeros per row at the 1-GPU size (32^3 node grid)
-    m = 32
-    assert 3 * (3 * m - 2) ** 3 / m ** 3 == pytest.approx(76.0, abs=0.1)
+    # PAPER.md:210-217 (Table 4): the Q1 operator has ~76 scalar nonzeros per row at the 1-GPU size (32^3 node
+    # grid): counted on the generated matrix itself
+    A = pr.Generator(3, 31, seed=1).A(0)
+    assert A.nbrows == 32 ** 3
+    assert 9 * A.nnzb / (3 * A.nbrows) == pytest.approx(76.0, abs=0.1)
 
 
 @pytest.mark.parametrize("fix", ["cfg0", "grid2d"])
@@ -138,9 +140,11 @@ def test_smoothed_prolongator_definition(cfg0):
 
 
 def test_aggregate_counts():
-    # O5 / R6 (merge rule): 27 aggregates at cfg0; 21^3 at 65^3 nodes; 32^3 at 97^3 nodes (counted without
-    # building those grids: na = floor(n/3))
-    assert (9 // 3) ** 3 == 27 and (65 // 3) ** 3 == 9261 and (97 // 3) ** 3 == 32768 and (129 // 3) ** 3 == 79507
+    # O5 / R6 (merge rule): na = floor(n/3) boxes per side, the remainder merged into the last box
+    for ne, na in ((8, 3), (10, 3), (12, 4)):      # n = ne+1 nodes per side -> floor(n/3) boxes per side
+        gg = pr.Generator(3, ne, seed=0)
+        gg.build_prolongator(0)
+        assert gg.level_info(1)["nnodes"] == na ** 3 and gg.P(0).nbcols == na ** 3
     g = pr.Generator(3, 7, seed=0)   # 8 nodes per side: boxes of 3 and 5
     g.build_prolongator(0)
     agg = g.level_arrays(0)["agg"]
@@ -155,3 +159,51 @@ def test_uniform_stream_reproducible():
     c = pr.uniform(3, pr.PURPOSE_COARSE, 1000)
     assert (a == b).all() and not (a == c).any()
     assert a.min() >= -1 and a.max() < 1 and abs(a.mean()) < 0.1
+
+
+# ---------------------------------------------------------------- level 2 (O9, readings R9, R20; pin I5 second half)
+def _coarse_modes(coords, rfac, d):
+    nb = 6 if d == 3 else 3
+    B = np.zeros((coords.shape[0] * nb, nb))
+    for J in range(coords.shape[0]):
+        Mfull = np.eye(nb)
+        Mfull[:d, :] = rigid_modes(coords[J:J + 1], d)     # M(c_J - 0) = [[I, W(c_J)], [0, I]]
+        B[J * nb:(J + 1) * nb] = rfac[J] @ Mfull
+    return B
+
+
+@pytest.mark.parametrize("d,ne", [(3, 17), (2, 26)])
+def test_level2_tentative_prolongator(d, ne):
+    """The level-2 tentative prolongator (6x6 / 3x3 blocks from the restricted rigid-body modes): orthonormal
+    columns, and the fine rigid-body modes are reproduced through BOTH levels: P1_tent P2_tent B_2 = B_0."""
+    from oracle import oracle as orc
+    g = pr.Generator(d, ne, seed=9)
+    g.build_prolongator(0)
+    A0, P0 = g.A(0), g.P(0)
+    Ac = orc.ptap(A0, P0)
+    g.set_operator(1, pr.HostBSR(Ac.nbrows, Ac.nbcols, Ac.bs_r, Ac.bs_c, Ac.rowptr, Ac.colidx, Ac.vals))
+    g.build_prolongator(1)
+    nb = 6 if d == 3 else 3
+    Pt1, Pt2 = g.P_tent(0).to_scipy().tocsr(), g.P_tent(1)
+    assert (Pt2.bs_r, Pt2.bs_c) == (nb, nb) and Pt2.nbcols == g.level_info(2)["nnodes"] > 1
+    Pt2 = Pt2.to_dense()
+    assert np.abs(Pt2.T @ Pt2 - np.eye(Pt2.shape[1])).max() < 1e-14
+    c1, c2 = g.level_arrays(1), g.level_arrays(2)
+    B0 = rigid_modes(g.level_arrays(0)["coords"], d)
+    B1 = _coarse_modes(c1["coords"], c1["rfac"], d)
+    B2 = _coarse_modes(c2["coords"], c2["rfac"], d)
+    assert np.abs(Pt2 @ B2 - B1).max() < 1e-13 * max(1.0, np.abs(B1).max())
+    assert np.abs(Pt1 @ (Pt2 @ B2) - B0).max() < 1e-13
+    # level-2 centroids are the unweighted means of their members' level-1 centroids (R20)
+    agg = c1["agg"]
+    for K in range(c2["coords"].shape[0]):
+        assert np.allclose(c2["coords"][K], c1["coords"][agg == K].mean(axis=0), rtol=0, atol=1e-15)
+    # smoothed level-2 prolongator against the dense formula with the 6x6 (3x3) block diagonal (O7 on A_1)
+    A1 = g.A(1).to_dense()
+    info = g.level_info(1)
+    D = np.zeros_like(A1)
+    for i in range(0, A1.shape[0], nb):
+        D[i:i + nb, i:i + nb] = A1[i:i + nb, i:i + nb]
+    ref = Pt2 - info["omega"] * np.linalg.solve(D, A1 @ Pt2)
+    assert np.abs(g.P(1).to_dense() - ref).max() < 1e-13 * np.abs(ref).max()
+    assert info["omega"] == pytest.approx(4 / (3 * info["lam"]), rel=1e-15)

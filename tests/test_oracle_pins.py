@@ -283,7 +283,88 @@ def test_pcg_history_vs_dense_reference(cfg0):
     assert np.linalg.norm(Ad @ x - b) == pytest.approx(hist[-1], rel=1e-6)
 
 
-def test_byte_model_matches_paper():
-    # a 3x3 block moves 72 B of values + 4 B of index = 76 B (scalar CSR: 108 B)
-    assert 8 * 3 * 3 + 4 == 76 and 9 * (8 + 4) == 108
-    assert 108 / 76 == pytest.approx(1.42, abs=0.005)
+# ---------------------------------------------------------------- three levels (O9, O10): the intermediate level
+def _three_level(d, ne, seed):
+    """A small three-level hierarchy built the way config 4 is (O9): A_1 = P_0^T A_0 P_0, level-2 prolongator from
+    the restricted rigid-body modes, A_2 = P_1^T A_1 P_1."""
+    g = pr.Generator(d, ne, seed=seed)
+    g.build_prolongator(0)
+    A0, P0 = g.A(0), g.P(0)
+    Ac = orc.ptap(A0, P0)
+    A1 = pr.HostBSR(Ac.nbrows, Ac.nbcols, Ac.bs_r, Ac.bs_c, Ac.rowptr, Ac.colidx, Ac.vals)
+    g.set_operator(1, A1)
+    g.build_prolongator(1)
+    P1 = g.P(1)
+    Ac2 = orc.ptap(A1, P1)
+    A2 = pr.HostBSR(Ac2.nbrows, Ac2.nbcols, Ac2.bs_r, Ac2.bs_c, Ac2.rowptr, Ac2.colidx, Ac2.vals)
+    lams = [g.level_info(0)["lam"], g.level_info(1)["lam"]]
+    return g, [A0, A1, A2], [P0, P1], lams
+
+
+def _dense_smoother(Ad, bs, lam):
+    n = Ad.shape[0]
+    Dinv = np.zeros_like(Ad)
+    for i in range(0, n, bs):
+        Dinv[i:i + bs, i:i + bs] = np.linalg.inv(Ad[i:i + bs, i:i + bs])     # library inverse of each bs x bs block
+    return (np.eye(n) - cheb_poly_closed_form(Ad, Dinv, lam)) @ np.linalg.inv(Ad), Dinv
+
+
+@pytest.mark.parametrize("d,ne", [(3, 8), (2, 26)])
+def test_three_grid_operator_dense(d, ne):
+    """PAPER.md:42 written out densely for THREE grids: the middle level both smooths (6x6 / 3x3 block-Jacobi,
+    blocks inverted by numpy) and recurses.  Fails if vcycle() takes a level's operator, prolongator, lambda or
+    D^-1 from the wrong level, or if the 6x6 block inverse is wrong."""
+    g, As, Ps, lams = _three_level(d, ne, seed=21)
+    assert As[1].bs_r == (6 if d == 3 else 3) and As[2].nbrows >= 1
+    H = orc.Hierarchy(As, Ps, lams)
+    A0, A1, A2 = (M.to_dense() for M in As)
+    P0, P1 = (M.to_dense() for M in Ps)
+    S0, _ = _dense_smoother(A0, As[0].bs_r, lams[0])
+    S1, Dinv1 = _dense_smoother(A1, As[1].bs_r, lams[1])
+    assert abs(lams[0] - lams[1]) > 1e-3 * lams[0]          # the two levels are distinguishable
+
+    def level1(rc):                                          # V-cycle on level 1 from a zero guess
+        y1 = S1 @ rc
+        y2 = y1 + P1 @ np.linalg.solve(A2, P1.T @ (rc - A1 @ y1))
+        return y2 + S1 @ (rc - A1 @ y2)
+
+    b = pr.uniform(21, pr.PURPOSE_RHS, A0.shape[0])
+    x1 = S0 @ b
+    x2 = x1 + P0 @ level1(P0.T @ (b - A0 @ x1))
+    x3 = x2 + S0 @ (b - A0 @ x2)
+    got = H.vcycle(b)
+    assert np.linalg.norm(got - x3) < 1e-10 * np.linalg.norm(x3)
+    # the level-1 smoother on its own: error propagation p(D_1^-1 A_1) with numpy's 6x6 (3x3) inverses
+    bc = pr.uniform(21, pr.PURPOSE_COARSE, A1.shape[0])
+    y0 = pr.uniform(22, pr.PURPOSE_COARSE, A1.shape[0])
+    ys = np.linalg.solve(A1, bc)
+    ref = ys - cheb_poly_closed_form(A1, Dinv1, lams[1]) @ (ys - y0)
+    y1 = H.smooth(1, bc, y0)
+    assert np.linalg.norm(y1 - ref) < 1e-11 * np.linalg.norm(ref)
+    # symmetric operator (I12), three levels
+    u = pr.uniform(23, pr.PURPOSE_FINE, A0.shape[0])
+    assert np.dot(u, got) == pytest.approx(np.dot(b, H.vcycle(u)), rel=1e-9)
+
+
+def test_three_level_pcg_vs_dense_reference():
+    g, As, Ps, lams = _three_level(2, 26, seed=5)
+    H = orc.Hierarchy(As, Ps, lams)
+    Ad = As[0].to_dense()
+    n = Ad.shape[0]
+    Minv = np.column_stack([H.vcycle(e) for e in np.eye(n)])
+    assert np.abs(Minv - Minv.T).max() < 1e-9 * np.abs(Minv).max()
+    b = pr.uniform(5, pr.PURPOSE_RHS, n)
+    x, hist = H.pcg(b, 10)
+    r = b.copy(); z = Minv @ r; p = z.copy(); rz = r @ z
+    ref = [np.linalg.norm(r)]
+    for _ in range(10):
+        q = Ad @ p
+        a = rz / (p @ q)
+        r -= a * q
+        ref.append(np.linalg.norm(r))
+        z = Minv @ r
+        rz_new = r @ z
+        p = z + (rz_new / rz) * p
+        rz = rz_new
+    assert np.allclose(hist, ref, rtol=1e-7)
+    assert (np.diff(hist) < 0).all()
