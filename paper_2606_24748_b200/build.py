@@ -53,8 +53,6 @@ def cuda_headers() -> list[str]:
 
 
 def build_cuda(force: bool = False, verbose: bool = False) -> str:
-    if os.environ.get("BSRAMG_LIB"):  # a prebuilt library (e.g. an instrumented build) instead of the in-tree one
-        return os.environ["BSRAMG_LIB"]
     srcs = cuda_sources()
     if not srcs:
         raise RuntimeError("no CUDA sources under " + CSRC)

@@ -230,18 +230,11 @@ static int spmv_dispatch_epi(bsr_t A, const double* x, double* y, const double* 
 // steps, loads independent of the row pointers), multiplies by the matching x pair and parks the partial product in
 // shared memory; then one thread per output entry adds its row's partials in a fixed order (block by block, pair by
 // pair) and applies the epilogue.  Deterministic, no atomics.
-#ifndef FLAT_ROWS_N
-#define FLAT_ROWS_N 64
-#endif
-#ifndef FLAT_U_N
-#define FLAT_U_N 4
-#endif
-#ifndef FLAT_MINB
-#define FLAT_MINB 6
-#endif
-constexpr int FLAT_ROWS = FLAT_ROWS_N;
+// 64 rows per CTA, 4 loads in flight per thread, 6 resident CTAs: the best of the sweep in profiles/r1g_final.md
+constexpr int FLAT_ROWS = 64;
 constexpr int FLAT_THREADS = 256;
-constexpr int FLAT_U = FLAT_U_N;
+constexpr int FLAT_U = 4;
+constexpr int FLAT_MINB = 6;
 
 template <int BR, int BC, int EPI>
 __global__ void __launch_bounds__(FLAT_THREADS, FLAT_MINB)
@@ -294,22 +287,31 @@ spmv_flat_kernel(int32_t nbrows, const int32_t* __restrict__ rowptr, const int32
   }
 }
 
+// shared memory a CTA of the flat kernel may ask for (its partials; above that the row kernel runs instead)
+constexpr int FLAT_SMEM_MAX = 100 * 1024;
+
+// prepare = true (cold, from bsr_create): opts the four epilogue instantiations in to FLAT_SMEM_MAX bytes of dynamic
+// shared memory on the current device; false: the hot launch
 template <int BR, int BC>
-static int spmv_flat_launch(bsr_t A, const double* x, double* y, const double* b, Epilogue epi, cudaStream_t st) {
+static int spmv_flat_launch(bsr_t A, const double* x, double* y, const double* b, Epilogue epi, cudaStream_t st,
+                            bool prepare = false) {
   using S = Shape<BR, BC>;
   const int64_t blocks = ((int64_t)A->nbrows + FLAT_ROWS - 1) / FLAT_ROWS;
-  if (blocks == 0) return BSR_OK;
+  if (blocks == 0 && !prepare) return BSR_OK;
   const size_t smem = ((FLAT_ROWS + 1) * 4 + 15) / 16 * 16 + (size_t)A->flat_max_blocks * S::LB * 8;
   const dim3 grid((unsigned)blocks), block(FLAT_THREADS);
 #define FLAT_CASE(E)                                                                                          \
   {                                                                                                           \
     auto kern = spmv_flat_kernel<BR, BC, E>;                                                                  \
-    static size_t set_smem = 0;                                                                               \
-    if (smem > 48 * 1024 && smem > set_smem) {                                                                \
-      CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));           \
-      set_smem = smem;                                                                                        \
+    if (prepare) {                                                                                            \
+      CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, FLAT_SMEM_MAX));       \
+    } else {                                                                                                  \
+      LAUNCH(kern, grid, block, smem, st, A->nbrows, A->d_rowptr, A->d_colidx, A->d_vals, x, y, b);           \
     }                                                                                                         \
-    LAUNCH(kern, grid, block, smem, st, A->nbrows, A->d_rowptr, A->d_colidx, A->d_vals, x, y, b);             \
+  }
+  if (prepare) {
+    FLAT_CASE(EPI_ASSIGN) FLAT_CASE(EPI_RESID) FLAT_CASE(EPI_SUB) FLAT_CASE(EPI_ADD)
+    return BSR_OK;
   }
   switch (epi) {
     case EPI_ASSIGN: FLAT_CASE(EPI_ASSIGN) break;
@@ -321,12 +323,17 @@ static int spmv_flat_launch(bsr_t A, const double* x, double* y, const double* b
   return BSR_OK;
 }
 
-#ifndef SPMV_ROW_U
-#define SPMV_ROW_U 4
-#endif
-#ifndef SPMV_RB_LONG
-#define SPMV_RB_LONG 1
-#endif
+// row-kernel parameters frozen from the sweeps in profiles/r1i_end_of_round.md: 4 loads in flight in ROW mode; a warp
+// takes 4 consecutive short rows per row-pointer load (6 resident CTAs), 1 long row (4 resident CTAs)
+constexpr int SPMV_ROW_U = 4, SPMV_RB_LONG = 1, SPMV_RB = 4, SPMV_MINB_SHORT = 6;
+
+template <int BR, int BC>
+static bool spmv_uses_flat(bsr_t A) {
+  using S = Shape<BR, BC>;
+  if constexpr (S::ROWPAIR) return A->team_mode != 1 && !A->no_flat && ((FLAT_ROWS + 1) * 4 + 15) / 16 * 16 + (size_t)A->flat_max_blocks * S::LB * 8 <= (size_t)FLAT_SMEM_MAX;
+  return false;
+}
+
 template <int BR, int BC>
 static int spmv_dispatch_team(bsr_t A, const double* x, double* y, const double* b, Epilogue epi, cudaStream_t st) {
   using S = Shape<BR, BC>;
@@ -334,20 +341,36 @@ static int spmv_dispatch_team(bsr_t A, const double* x, double* y, const double*
     // the whole warp on one block row: U steps of GPW blocks cover a 27-block row of A in one pass
     constexpr int U = (S::GPW >= 8) ? 2 : (S::GPW == 1 ? 8 : 9);
     if (A->avg_row_len >= 2.0 * S::GPW * U) return spmv_dispatch_epi<BR, BC, S::GPW, U, 4, SPMV_RB_LONG>(A, x, y, b, epi, st);
-#ifndef SPMV_RB
-#define SPMV_RB 4
-#endif
-#ifndef SPMV_MINB_SHORT
-#define SPMV_MINB_SHORT 6
-#endif
     return spmv_dispatch_epi<BR, BC, S::GPW, U, SPMV_MINB_SHORT, SPMV_RB>(A, x, y, b, epi, st);
   }
   if constexpr (S::ROWPAIR) {
     // short rows of a pair-able shape: the flat stream kernel, if a CTA's partials fit in shared memory
-    if (!getenv("BSRAMG_NO_FLAT") && (size_t)A->flat_max_blocks * S::LB * 8 <= 96 * 1024)
-      return spmv_flat_launch<BR, BC>(A, x, y, b, epi, st);
+    if (spmv_uses_flat<BR, BC>(A)) return spmv_flat_launch<BR, BC>(A, x, y, b, epi, st);
   }
   return spmv_dispatch_epi<BR, BC, 1, SPMV_ROW_U, 6, 1>(A, x, y, b, epi, st);
+}
+
+// cold (bsr_create / first transpose): opt the flat kernels of A's shape in to their shared memory on this device
+template <int BR, int BC>
+static int spmv_prepare_shape(bsr_t A) {
+  if constexpr (Shape<BR, BC>::ROWPAIR) {
+    if (spmv_uses_flat<BR, BC>(A)) return spmv_flat_launch<BR, BC>(A, nullptr, nullptr, nullptr, EPI_ASSIGN, 0, true);
+  }
+  return BSR_OK;
+}
+static int spmv_prepare(bsr_t A) {
+#define PREP(BR, BC) return spmv_prepare_shape<BR, BC>(A)
+  switch (A->bs_r * 10 + A->bs_c) {
+    case 22: PREP(2, 2);
+    case 23: PREP(2, 3);
+    case 32: PREP(3, 2);
+    case 33: PREP(3, 3);
+    case 36: PREP(3, 6);
+    case 63: PREP(6, 3);
+    case 66: PREP(6, 6);
+  }
+#undef PREP
+  return BSR_OK;
 }
 
 int spmv_launch(bsr_t A, const double* x, double* y, const double* b, Epilogue epi, cudaStream_t st) {
@@ -449,6 +472,7 @@ int transpose_ensure(bsr_t A, cudaStream_t st) {
     T->h_rowptr.swap(rp);
     T->h_colidx.swap(ci);
     choose_team_mode(T);
+    if (spmv_prepare(T) != BSR_OK) T->no_flat = true;   // a device without the shared memory: row kernel
     A->T = T;
     A->T_state = -1;
   }
@@ -535,6 +559,7 @@ int bsr_create(bsr_t* out, int32_t nbrows, int32_t nbcols, int32_t bs_r, int32_t
   A->avg_row_len = nbrows ? (double)nnzb / nbrows : 0.0;
   A->flat_max_blocks = flat_max_blocks_of(A->h_rowptr, nbrows);
   choose_team_mode(A);
+  if (spmv_prepare(A) != BSR_OK) A->no_flat = true;   // no device yet / too little shared memory: row kernel
   *out = A;
   return BSR_OK;
 }

@@ -236,24 +236,34 @@ def _random_bsr(rng, nbrows, nbcols, br, bc, row_len):
     return pr.HostBSR(nbrows, nbcols, br, bc, rowptr, cols, rng.uniform(-1, 1, (cols.shape[0], br, bc)))
 
 
-def test_ptap_unstructured_falls_back_to_gather_kernels(bsr):
-    """A product outside the staged format (AP / A_c rows with more than 32 blocks: random A and P) keeps the gather
-    kernels; results must be the same definition."""
+@pytest.mark.parametrize("shape", [(3, 6), (2, 3), (6, 6), (3, 3), (2, 2), (6, 3), (3, 2)])
+def test_ptap_unstructured(bsr, shape):
+    """Random sparsity (AP / A_c rows with far more than 32 blocks, empty rows): the lane programs have no row-length
+    limit; same definition, same tolerance, every block shape of the supported set."""
     rng = np.random.default_rng(5)
-    A = _random_bsr(rng, 120, 120, 3, 3, 12)
-    P = _random_bsr(rng, 120, 60, 3, 6, 9)
+    bf, bc = shape
+    A = _random_bsr(rng, 120, 120, bf, bf, 12)
+    P = _random_bsr(rng, 120, 60, bf, bc, 9)
     (rap, cap), (rc, cc) = orc.ptap_symbolic(A, P)
     assert np.diff(rap).max() > 32 or np.diff(rc).max() > 32
-    ptap_check(bsr, A, P)
+    GA, GP, plan, got, ref, mag = ptap_check(bsr, A, P)
+    sch = plan.schedule()
+    assert sch[1]["programs"] == 1 and sch[2]["programs"] == 1
 
 
-def test_ptap_gather_path_matches_staged_path(bsr, probs, monkeypatch):
-    """BSRAMG_NO_STREAM forces the gather kernels on a structured problem: same structure, values within rounding."""
+def test_ptap_gather_path_matches_program_path(bsr, probs):
+    """bsr_set_option("ptap_force_gather") keeps the one-thread-per-block gather kernels (the path a matrix outside
+    the program format takes) on a structured problem: same structure, values within rounding."""
     g = probs["hex13"]
     A, P = g.A(0), g.P(0)
-    _, _, _, staged, ref, mag = ptap_check(bsr, A, P)
-    monkeypatch.setenv("BSRAMG_NO_STREAM", "1")
-    _, _, _, gathered, _, _ = ptap_check(bsr, A, P)
+    _, _, plan, staged, ref, mag = ptap_check(bsr, A, P)
+    assert plan.schedule()[1]["programs"] == 1 and plan.schedule()[2]["programs"] == 1
+    bsr.set_option("ptap_force_gather", 1)
+    try:
+        _, _, plan2, gathered, _, _ = ptap_check(bsr, A, P)
+        assert plan2.schedule()[1]["programs"] == 0 and plan2.schedule()[2]["programs"] == 0
+    finally:
+        bsr.set_option("ptap_force_gather", 0)
     assert blockwise_rel_err(gathered, staged, mag) < 1e-13
 
 
