@@ -119,8 +119,8 @@ int ptap_structure(ptap_plan_t plan, int32_t* d_rowptr_c, int32_t* d_colidx_c, v
 int ptap_numeric(ptap_plan_t plan, bsr_t A, bsr_t P, double* d_vals_c, void* stream);
 int ptap_get_info(ptap_plan_t plan, int64_t* nnzb_ap, int64_t* n_products_1, int64_t* n_products_2,
                   int64_t* algorithmic_bytes, int64_t* n_r_value_builds);
-/* How the two stages of a plan are scheduled: out8 = { stage 1 runs lane programs (1) or the gather kernel (0), its
- * bricks, distinct programs, dynamic shared memory per brick; the same four for stage 2 }. */
+/* How the two stages of a plan are scheduled: out8 = { stage 1 runs the staged kernel (1) or the gather kernel (0), its
+ * bricks, reserved, dynamic shared memory per brick; the same four for stage 2 }. */
 int ptap_get_schedule(ptap_plan_t plan, int64_t* out8);
 /* Runs only one stage of ptap_numeric (1: AP = A*P, 2: A_c = R*AP from the AP left by the last stage 1); for
  * profiling and tests.  stage 2 needs d_vals_c, stage 1 ignores it. */
@@ -150,16 +150,12 @@ int ptap_destroy(ptap_plan_t plan);
 void* ptap_host_plan_build(int32_t nbrows_a, const int32_t* rowptr_a, const int32_t* colidx_a, int32_t nbcols_p,
                            const int32_t* rowptr_p, const int32_t* colidx_p);
 int ptap_host_plan_get(void* handle, const char* name, const void** ptr, int64_t* count, int32_t* elem_bytes);
-/* Host side of the numeric schedule (cold part of ptap_symbolic), for tests: builds the lane programs of stage 1
- * (AP = A*P) or stage 2 (A_c = R*AP) for fine / coarse block sizes bs_f / bs_c under a shared-memory budget, CHECKS
- * every distinct program against the structure it was built from (each block product of each output block exactly
- * once, on a lane of the right class, from the staged copy of the right blocks) and reports out12 = { plan usable
- * (1/0), bricks, distinct programs, largest brick's shared memory in bytes, block products covered, lane steps
- * (32 x warp steps: products / lane steps = lane utilisation), plan bytes, modelled shared-memory cycles of the X
- * loads and of the Y loads under the quarter-warp bank model (4 per warp step = conflict free), verified (1/0),
- * chunks, staged Y block copies }.  A failed check also leaves its reason in bsr_last_error(). */
-int ptap_host_prog_stats(void* handle, int32_t bs_f, int32_t bs_c, int32_t stage, int64_t smem_budget,
-                         int64_t* out12);
+/* Host side of the staged numeric schedule (cold part of ptap_symbolic), for tests: builds the brick / chunk / pass
+ * plan of stage 1 (AP = A*P) or stage 2 (A_c = R*AP) for fine / coarse block sizes bs_f / bs_c under a shared-memory
+ * budget and reports out8 = { plan usable (1/0), bricks, chunks, largest brick's shared memory in bytes, set mask bits
+ * (= block products covered, each exactly once), lanes over all entries, passes, steps over all passes }. */
+int ptap_host_stream_stats(void* handle, int32_t bs_f, int32_t bs_c, int32_t stage, int64_t smem_budget,
+                           int64_t* out8);
 void ptap_host_plan_free(void* handle);
 
 /* ------------------------------------------------------------------ V-cycle and PCG
@@ -198,7 +194,7 @@ int bsr_counters(int64_t* n_kernel_launches, int64_t* n_allocs);
 
 /* ------------------------------------------------------------------ options of the COLD calls (tests, tuning)
  * Process-wide; read by ptap_symbolic only, never by a hot call.  Names: "ptap_force_gather" (1: keep the
- * one-thread-per-output-block gather kernels instead of the lane programs, the path any matrix outside the program
+ * one-thread-per-output-block gather kernels instead of the staged kernels, the path any matrix outside the staged
  * format takes), "ptap_smem_stage1" / "ptap_smem_stage2" (shared-memory bytes a brick of the stage may use).
  * Errors: BSR_ERR_NULL, BSR_ERR_SHAPE (unknown name or value out of range). */
 int bsr_set_option(const char* name, int64_t value);

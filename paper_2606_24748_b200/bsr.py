@@ -42,7 +42,7 @@ SYMBOLS = {
     "ptap_destroy": (C.c_int, [_V]),
     "ptap_host_plan_build": (C.c_void_p, [_I32, _V, _V, _I32, _V, _V]),
     "ptap_host_plan_get": (C.c_int, [_V, C.c_char_p, _PV, _PI64, _PI32]),
-    "ptap_host_prog_stats": (C.c_int, [_V, _I32, _I32, _I32, _I64, _PI64]),
+    "ptap_host_stream_stats": (C.c_int, [_V, _I32, _I32, _I32, _I64, _PI64]),
     "ptap_get_schedule": (C.c_int, [_V, _PI64]),
     "bsr_set_option": (C.c_int, [C.c_char_p, _I64]),
     "ptap_host_plan_free": (None, [_V]),
@@ -223,7 +223,7 @@ class PtapPlan:
     def schedule(self) -> dict:
         o = (C.c_int64 * 8)()
         _check(lib().ptap_get_schedule(self.h, o))
-        k = ["programs", "bricks", "distinct", "smem"]
+        k = ["staged", "bricks", "reserved", "smem"]
         return {1: dict(zip(k, [int(v) for v in o[:4]])), 2: dict(zip(k, [int(v) for v in o[4:]]))}
 
     def new_values(self):
@@ -266,7 +266,7 @@ class HostPlan:
     NAMES = ["rowptr_ap", "colidx_ap", "rowidx_ap", "rowptr_c", "colidx_c", "rowidx_c", "rowptr_r", "colidx_r",
              "perm_r", "pairptr1", "k1", "q1", "pstart", "pairptr2", "t2", "s2", "apstart"]
 
-    def __init__(self, A, P, budgets=(112 * 1024, 75000)):
+    def __init__(self, A, P):
         ra, ca = np.ascontiguousarray(A.rowptr, np.int32), np.ascontiguousarray(A.colidx, np.int32)
         rp, cp = np.ascontiguousarray(P.rowptr, np.int32), np.ascontiguousarray(P.colidx, np.int32)
         h = lib().ptap_host_plan_build(A.nbrows, ra.ctypes.data, ca.ctypes.data, P.nbcols, rp.ctypes.data,
@@ -284,15 +284,13 @@ class HostPlan:
                 else:
                     arr = np.empty(0, dt)
                 setattr(self, name, arr)
-            self.prog_stats = {}
+            self.stream_stats = {}
             if getattr(A, "bs_r", None) and getattr(P, "bs_c", None):
-                for stage, budget in ((1, budgets[0]), (2, budgets[1])):
-                    o = (C.c_int64 * 12)()
-                    _check(lib().ptap_host_prog_stats(h, A.bs_r, P.bs_c, stage, budget, o))
-                    self.prog_stats[stage] = dict(zip(["ok", "bricks", "programs", "max_smem", "products",
-                                                       "lane_steps", "plan_bytes", "xq_clk", "yq_clk", "verified",
-                                                       "chunks", "ycopies"], [int(v) for v in o]))
-                    self.prog_stats[stage]["why"] = lib().bsr_last_error().decode() if not o[9] else ""
+                for stage, budget in ((1, 112 * 1024), (2, 75000)):
+                    o = (C.c_int64 * 8)()
+                    _check(lib().ptap_host_stream_stats(h, A.bs_r, P.bs_c, stage, budget, o))
+                    self.stream_stats[stage] = dict(zip(["ok", "bricks", "chunks", "max_smem", "mask_bits", "lanes",
+                                                         "passes", "steps"], [int(v) for v in o]))
         finally:
             lib().ptap_host_plan_free(h)
 

@@ -84,17 +84,22 @@ struct HostPlan {
   int32_t max_k1 = 0, max_q1 = 0, max_t2 = 0, max_s2 = 0;
   std::string err;
   // builds everything from the host structures of A, P and R = P^T.  Returns BSR_OK or an error code.
-  // want_pairs = false: structures only (the gather lists are needed by the fallback kernels and the tests).
   int build(int32_t nbrows_a, const int32_t* rowptr_a, const int32_t* colidx_a, int32_t nbcols_p,
-            const int32_t* rowptr_p, const int32_t* colidx_p, const int32_t* rowptr_r, const int32_t* colidx_r,
-            bool want_pairs = true);
-  int64_t nprod1 = 0, nprod2 = 0;   // block products of the two stages
+            const int32_t* rowptr_p, const int32_t* colidx_p, const int32_t* rowptr_r, const int32_t* colidx_r);
 };
 
 // explicit transpose structure on the host: R = P^T rows sorted; perm[t] = slot of P that R's slot t comes from
 void host_transpose_structure(int32_t nbrows, int32_t nbcols, const int32_t* rowptr, const int32_t* colidx,
                               std::vector<int32_t>& rowptr_t, std::vector<int32_t>& colidx_t,
                               std::vector<int32_t>& perm);
+
+// process-wide options of the COLD calls (bsr_set_option); never read by a hot call
+struct Options {
+  int64_t force_gather = 0;                 // 1: ptap_symbolic keeps the gather kernels (tests of the fallback)
+  int64_t smem_stage1 = 112 * 1024;         // shared memory a stage-1 brick may use (two bricks per SM)
+  int64_t smem_stage2 = 75000;              // stage 2: three coarse rows per SM (register-limited)
+};
+Options& options();
 
 }  // namespace bsramg
 
@@ -126,3 +131,74 @@ struct bsr_matrix_s {
 };
 static const uint64_t BSR_MAGIC = 0x425352414d473031ull;
 
+// ------------------------------------------------------------------ brick-staged block products (ptap_stream.cpp)
+// One output-stationary block product C = X * Y (stage 1: X = A, Y = P; stage 2: X = R, Y = AP) cut into BRICKS
+// (one CTA each) of CHUNKS.  A chunk stages a set of X row pieces and every Y row they reference in shared memory.
+// A lane owns one output block C(row, slot) (M x N accumulators in registers).  A warp walks the X blocks of its
+// row piece(s) in order ("k-synchronous"): at step k every lane of the row reads the same X block (a broadcast),
+// and the lanes whose slot receives a product from X(row,k) -- bit `slot` of the block's MASK -- read consecutive
+// blocks of Y's row (lane's block = rank of its bit in the mask), so shared-memory reads are broadcast or
+// contiguous.  DIRECT bricks write each block once from registers at the end of a pass (stage 1).  PERSIST bricks
+// keep the accumulators over all chunks, every warp taking a share of each chunk's X blocks, and add the warps'
+// partial blocks in warp order through shared memory before writing the block once (stage 2) -- the atomic-free
+// segmented scatter of SURVEY.md 8(a) a7.
+namespace bsramg {
+
+struct StreamEntry {   // 16 bytes: one X row piece inside a pass
+  int32_t out;         // first slot of C's row (direct) / first accumulator of the row (persist)
+  int32_t xbase;       // staged X block index of the piece's first block
+  int32_t len;         // number of X blocks (steps)
+  uint8_t lane0;       // first lane of this entry in the warp
+  uint8_t nslots;      // output blocks of the row held by this entry's lanes
+  uint8_t slot0;       // first of them inside the row (a row's blocks may be split over two passes)
+  uint8_t pad1;
+};
+struct StreamPass { int32_t e0, e1, steps, pad; };   // entries [e0, e1) (relative to the chunk), max len
+struct StreamMeta { uint32_t mask, ybase; };          // per staged X block: receiving slots, staged Y row start
+struct StreamRun { int32_t src, n, dst; };            // copy n blocks from global block src to staged block dst
+struct StreamBrickHdr { int32_t chunk0, nchunks, out, nslots; };   // out / nslots: persist bricks (C row of the brick)
+struct StreamChunkHdr {   // 64 bytes: everything a CTA needs to know about a chunk, fetched with one load
+  int64_t meta0;          // first staged X block in StreamPlan::meta
+  int32_t nx, ny;         // staged X blocks (even, padded) and Y blocks
+  int32_t ent0, nent, pass0, npass, xr0, nxr, yr0, nyr;
+  int32_t pad[4];
+};
+static_assert(sizeof(StreamChunkHdr) == 64 && sizeof(StreamBrickHdr) == 16, "headers are fetched with 16-byte loads");
+
+struct StreamPlan {
+  bool ok = false;            // false: shapes / sizes outside this format -> caller keeps the gather kernel
+  std::string why;
+  bool persist = false;
+  int nwarps = 0;
+  int64_t max_smem = 0;       // dynamic shared memory of the largest brick
+  std::vector<StreamBrickHdr> bricks;
+  std::vector<StreamChunkHdr> chunks;
+  std::vector<StreamRun> xruns, yruns;
+  std::vector<StreamEntry> entries;
+  std::vector<StreamPass> passes;
+  std::vector<StreamMeta> meta;
+  int64_t nbricks() const { return (int64_t)bricks.size(); }
+  int64_t nchunks() const { return (int64_t)chunks.size(); }
+};
+
+struct StreamShape { int M, K, N; };   // C blocks M x N, X blocks M x K, Y blocks K x N
+inline int stream_xs(int M, int K) { return (M * K + 1) & ~1; }   // staged X block stride in doubles (16-byte rows)
+int64_t stream_smem_bytes(const StreamShape& sh, int64_t nx, int64_t ny, int64_t nentries, int64_t npasses);
+
+// piece of an X row: blocks [t0, t1) of row `row`
+struct StreamPiece { int32_t row, t0, t1; };
+struct StreamChunkDef { std::vector<StreamPiece> pieces; };
+struct StreamBrickDef { std::vector<StreamChunkDef> chunks; bool direct = true; };
+
+// builds the flat plan of C = X*Y for the given bricks.  pairptr/off_x: per C slot the ordered products (HostPlan).
+void stream_build(const StreamShape& sh, int nwarps, int64_t smem_budget, const std::vector<StreamBrickDef>& bricks,
+                  const int32_t* rowptr_x, const int32_t* colidx_x, const int32_t* rowptr_y, const int32_t* rowptr_c,
+                  const int32_t* pairptr, const uint16_t* off_x, const uint16_t* off_y, StreamPlan& out);
+
+// brick definitions of the two PtAP stages
+void stream_bricks_stage1(const HostPlan& hp, const StreamShape& sh, int64_t smem_budget, const int32_t* rowptr_a,
+                          const int32_t* colidx_a, const int32_t* rowptr_p, std::vector<StreamBrickDef>& bricks);
+void stream_bricks_stage2(const HostPlan& hp, const StreamShape& sh, int nwarps, int64_t smem_budget,
+                          const int32_t* rowptr_r, const int32_t* colidx_r, std::vector<StreamBrickDef>& bricks);
+
+}  // namespace bsramg

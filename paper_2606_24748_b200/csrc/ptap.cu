@@ -13,9 +13,10 @@
 // zero-fill pass, bit-reproducible.
 #include <algorithm>
 #include <cstring>
+#include <cstdlib>
 
 #include "internal.h"
-#include "ptap_prog.h"
+#include "ptap_stream.h"
 
 struct ptap_plan_s {
   uint64_t magic = 0;
@@ -28,7 +29,7 @@ struct ptap_plan_s {
   int32_t *rowptr_c = nullptr, *colidx_c = nullptr, *rowidx_c = nullptr, *pairptr2 = nullptr, *apstart = nullptr;
   void *pairs1 = nullptr, *pairs2 = nullptr;
   double* vals_ap = nullptr;
-  bsramg::ProgDev s1, s2;  // lane programs of the two stages (ok == false: gather kernels)
+  bsramg::StreamDev s1, s2;  // brick-staged schedules of the two stages (ok == false: gather kernels)
 };
 static const uint64_t PLAN_MAGIC = 0x5054415031303030ull;
 
@@ -120,51 +121,44 @@ static int product_launch(bool wide, int64_t nout, const int32_t* rowidx, const 
 }
 
 template <typename T>
-static int prog_up(const std::vector<T>& h, const T** d, ProgDev& pd, cudaStream_t st) {
+static int stream_up(const std::vector<T>& h, const T** d, StreamDev& sd, cudaStream_t st) {
   T* p = nullptr;
   BSR_TRY(upload(&p, h, st));
-  pd.owned.push_back(p);
-  pd.bytes += (int64_t)h.size() * sizeof(T);
+  sd.owned.push_back(p);
+  sd.bytes += (int64_t)h.size() * sizeof(T);
   *d = p;
   return BSR_OK;
 }
 
-void prog_release(ProgDev& pd) {
-  for (void* p : pd.owned) dev_free(p);
-  pd = ProgDev();
+int stream_upload(const StreamShape& sh, const StreamPlan& sp, StreamDev& sd, cudaStream_t st) {
+  sd = StreamDev();
+  if (!sp.ok) return BSR_OK;
+  StreamArgs& a = sd.args;
+  int rc = stream_up(sp.bricks, &a.bricks, sd, st);
+  if (rc == BSR_OK) rc = stream_up(sp.chunks, &a.chunks, sd, st);
+  if (rc == BSR_OK) rc = stream_up(sp.xruns, &a.xruns, sd, st);
+  if (rc == BSR_OK) rc = stream_up(sp.yruns, &a.yruns, sd, st);
+  if (rc == BSR_OK) rc = stream_up(sp.entries, &a.entries, sd, st);
+  if (rc == BSR_OK) rc = stream_up(sp.passes, &a.passes, sd, st);
+  if (rc == BSR_OK) rc = stream_up(sp.meta, &a.meta, sd, st);
+  if (rc == BSR_OK) rc = stream_launch(sh.M, sh.K, sh.N, a, sp.persist, 0, sp.max_smem, st, true);   // shared-memory opt-in
+  if (rc == BSR_OK && cudaStreamSynchronize(st) != cudaSuccess) rc = fail(BSR_ERR_CUDA, "stream plan upload failed");
+  if (rc != BSR_OK) { stream_release(sd); return rc; }
+  sd.ok = true; sd.persist = sp.persist; sd.nbricks = sp.nbricks(); sd.smem = sp.max_smem;
+  return BSR_OK;
 }
 
-int prog_upload(const ProgPlan& pp, ProgDev& pd, cudaStream_t st) {
-  pd = ProgDev();
-  if (!pp.ok) return BSR_OK;
-  ProgArgs& a = pd.args;
-  int rc = prog_up(pp.rec_off, &a.rec_off, pd, st);
-  if (rc == BSR_OK) rc = prog_up(pp.rec, &a.rec, pd, st);
-  if (rc == BSR_OK) rc = prog_up(pp.blob, &a.blob, pd, st);
-  a.nbricks = (int32_t)pp.nbricks; a.rec_max_bytes = pp.rec_max_bytes; a.blob_max_bytes = pp.blob_max_bytes;
-  a.smem_total = (int32_t)pp.max_smem;
-  int ctas = 0;
-  if (rc == BSR_OK) rc = prog_launch(pp.shape, pp.persist, a, 0, pp.max_smem, st, true, &ctas);   // shared-memory opt-in
-  if (rc == BSR_OK) {
-    int dev = 0, sms = 0;
-    if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess)
-      rc = fail(BSR_ERR_CUDA, "no CUDA device");
-    else if (ctas < 1) rc = fail(BSR_ERR_LIMIT, "a brick's shared memory does not fit an SM");
-    pd.grid = (int32_t)std::min<int64_t>(pp.nbricks, (int64_t)sms * ctas);
-  }
-  if (rc == BSR_OK && cudaStreamSynchronize(st) != cudaSuccess) rc = fail(BSR_ERR_CUDA, "program upload failed");
-  if (rc != BSR_OK) { prog_release(pd); return rc; }
-  pd.ok = true; pd.persist = pp.persist; pd.shape = pp.shape; pd.nbricks = pp.nbricks; pd.smem = pp.max_smem;
-  pd.nprograms = pp.nprograms;
-  return BSR_OK;
+void stream_release(StreamDev& sd) {
+  for (void* p : sd.owned) dev_free(p);
+  sd = StreamDev();
 }
 
 static int stage1(ptap_plan_t pl, cudaStream_t st) {
   bsr_t A = pl->A, P = pl->P;
   if (pl->s1.ok) {
-    ProgArgs a = pl->s1.args;
+    StreamArgs a = pl->s1.args;
     a.xvals = A->d_vals; a.yvals = P->d_vals; a.cvals = pl->vals_ap;
-    return prog_launch(pl->s1.shape, false, a, pl->s1.grid, pl->s1.smem, st, false);
+    return stream_launch(pl->bf, pl->bf, pl->bc, a, false, pl->s1.nbricks, pl->s1.smem, st);
   }
 #define S1(BF, BC)                                                                                             \
   return product_launch<BF, BF, BC>(pl->wide1, pl->nnzb_ap, pl->rowidx_ap, A->d_rowptr, pl->pstart, pl->pairptr1, \
@@ -185,9 +179,9 @@ static int stage1(ptap_plan_t pl, cudaStream_t st) {
 static int stage2(ptap_plan_t pl, double* d_vals_c, cudaStream_t st) {
   bsr_t R = pl->P->T;
   if (pl->s2.ok) {
-    ProgArgs a = pl->s2.args;
+    StreamArgs a = pl->s2.args;
     a.xvals = R->d_vals; a.yvals = pl->vals_ap; a.cvals = d_vals_c;
-    return prog_launch(pl->s2.shape, true, a, pl->s2.grid, pl->s2.smem, st, false);
+    return stream_launch(pl->bc, pl->bf, pl->bc, a, true, pl->s2.nbricks, pl->s2.smem, st);
   }
 #define S2(BF, BC)                                                                                              \
   return product_launch<BC, BF, BC>(pl->wide2, pl->nnzb_c, pl->rowidx_c, R->d_rowptr, pl->apstart, pl->pairptr2, \
@@ -249,7 +243,7 @@ static void plan_release(ptap_plan_t pl) {
   dev_free(pl->rowptr_ap); dev_free(pl->colidx_ap); dev_free(pl->rowidx_ap); dev_free(pl->pairptr1);
   dev_free(pl->pstart); dev_free(pl->rowptr_c); dev_free(pl->colidx_c); dev_free(pl->rowidx_c);
   dev_free(pl->pairptr2); dev_free(pl->apstart); dev_free(pl->pairs1); dev_free(pl->pairs2); dev_free(pl->vals_ap);
-  prog_release(pl->s1); prog_release(pl->s2);
+  stream_release(pl->s1); stream_release(pl->s2);
   pl->magic = 0;
   delete pl;
 }
@@ -277,15 +271,14 @@ int bsr_set_option(const char* name, int64_t value) {
   if (!strcmp(name, "ptap_force_gather")) o.force_gather = value != 0;
   else if (!strcmp(name, "ptap_smem_stage1") && value >= 4096) o.smem_stage1 = value;
   else if (!strcmp(name, "ptap_smem_stage2") && value >= 4096) o.smem_stage2 = value;
-  else if (!strcmp(name, "ptap_round_len") && value >= 1 && value <= 64) o.round_len = value;
   else return fail(BSR_ERR_SHAPE, "bsr_set_option: unknown option or bad value '%s'", name);
   return BSR_OK;
 }
 
 int ptap_get_schedule(ptap_plan_t pl, int64_t* out8) {
   if (!pl || pl->magic != PLAN_MAGIC || !out8) return fail(BSR_ERR_NULL, "invalid plan handle");
-  out8[0] = pl->s1.ok; out8[1] = pl->s1.nbricks; out8[2] = pl->s1.nprograms; out8[3] = pl->s1.smem;
-  out8[4] = pl->s2.ok; out8[5] = pl->s2.nbricks; out8[6] = pl->s2.nprograms; out8[7] = pl->s2.smem;
+  out8[0] = pl->s1.ok; out8[1] = pl->s1.nbricks; out8[2] = 0; out8[3] = pl->s1.smem;
+  out8[4] = pl->s2.ok; out8[5] = pl->s2.nbricks; out8[6] = 0; out8[7] = pl->s2.smem;
   return BSR_OK;
 }
 
@@ -302,61 +295,57 @@ int ptap_symbolic(ptap_plan_t* out, bsr_t A, bsr_t P, int32_t* nbrows_c, int64_t
   cudaStream_t st = (cudaStream_t)stream;
   BSR_TRY(transpose_ensure(P, st));  // R = P^T, cached on P
   bsr_t R = P->T;
-  const Options opt = options();
-  // structures of AP and A_c (the gather lists only if a stage ends up on the fallback kernels)
   HostPlan hp;
-  bool have_pairs = opt.force_gather != 0;
   int rc = hp.build(A->nbrows, A->h_rowptr.data(), A->h_colidx.data(), P->nbcols, P->h_rowptr.data(),
-                    P->h_colidx.data(), R->h_rowptr.data(), R->h_colidx.data(), have_pairs);
+                    P->h_colidx.data(), R->h_rowptr.data(), R->h_colidx.data());
   if (rc != BSR_OK) return fail(rc, "ptap_symbolic: %s", hp.err.c_str());
   ptap_plan_s* pl = new (std::nothrow) ptap_plan_s();
   if (!pl) return fail(BSR_ERR_ALLOC, "host allocation failed");
   pl->A = A; pl->P = P; pl->nnzb_a = A->nnzb; pl->nnzb_p = P->nnzb;
   pl->bf = A->bs_r; pl->bc = P->bs_c; pl->nbrows_a = A->nbrows; pl->nbrows_c = P->nbcols;
   pl->nnzb_ap = (int64_t)hp.colidx_ap.size(); pl->nnzb_c = (int64_t)hp.colidx_c.size();
-  pl->nprod1 = hp.nprod1; pl->nprod2 = hp.nprod2;
+  pl->nprod1 = (int64_t)hp.k1.size(); pl->nprod2 = (int64_t)hp.t2.size();
+  pl->wide1 = hp.max_k1 > 255 || hp.max_q1 > 255;
+  pl->wide2 = hp.max_t2 > 255 || hp.max_s2 > 255;
   if (pl->nnzb_ap * pl->bf * pl->bc >= (1LL << 31) || pl->nnzb_c * pl->bc * pl->bc >= (1LL << 31)) {
     delete pl;
     return fail(BSR_ERR_LIMIT, "AP or A_c has 2^31 or more values");
   }
+  const Options opt = options();
   rc = upload(&pl->rowptr_ap, hp.rowptr_ap, st);
   if (rc == BSR_OK) rc = upload(&pl->colidx_ap, hp.colidx_ap, st);
   if (rc == BSR_OK) rc = upload(&pl->rowptr_c, hp.rowptr_c, st);
   if (rc == BSR_OK) rc = upload(&pl->colidx_c, hp.colidx_c, st);
   if (rc == BSR_OK) rc = dev_alloc_t(&pl->vals_ap, (size_t)pl->nnzb_ap * pl->bf * pl->bc);
   if (rc == BSR_OK && !opt.force_gather) {
-    // lane programs (ptap_prog.cpp); a stage whose bricks do not fit the format keeps the gather kernel
-    ProgPlan pp;
-    const ProgShape sh1{pl->bf, pl->bf, pl->bc}, sh2{pl->bc, pl->bf, pl->bc};
-    prog_plan_stage1(sh1, opt.smem_stage1, (int)opt.round_len, A->nbrows, A->h_rowptr.data(), A->h_colidx.data(), P->h_rowptr.data(),
-                     P->h_colidx.data(), P->nbcols, hp.rowptr_ap.data(), hp.colidx_ap.data(), pp);
-    rc = prog_upload(pp, pl->s1, st);
+    // brick-staged schedules (ptap_stream.cpp); a stage whose shapes do not fit keeps the gather kernel
+    std::vector<StreamBrickDef> bricks;
+    StreamPlan sp;
+    const StreamShape sh1{pl->bf, pl->bf, pl->bc}, sh2{pl->bc, pl->bf, pl->bc};
+    stream_bricks_stage1(hp, sh1, opt.smem_stage1, A->h_rowptr.data(), A->h_colidx.data(), P->h_rowptr.data(), bricks);
+    stream_build(sh1, STREAM_THREADS_DIRECT / 32, opt.smem_stage1, bricks, A->h_rowptr.data(), A->h_colidx.data(),
+                 P->h_rowptr.data(), hp.rowptr_ap.data(), hp.pairptr1.data(), hp.k1.data(), hp.q1.data(), sp);
+    rc = stream_upload(sh1, sp, pl->s1, st);
     if (rc == BSR_OK) {
-      prog_plan_stage2(sh2, opt.smem_stage2, P->nbcols, R->h_rowptr.data(), R->h_colidx.data(), hp.rowptr_ap.data(),
-                       hp.colidx_ap.data(), hp.rowptr_c.data(), hp.colidx_c.data(), pp);
-      rc = prog_upload(pp, pl->s2, st);
+      const int nw2 = STREAM_THREADS_PERSIST / 32;
+      stream_bricks_stage2(hp, sh2, nw2, opt.smem_stage2, R->h_rowptr.data(), R->h_colidx.data(), bricks);
+      stream_build(sh2, nw2, opt.smem_stage2, bricks, R->h_rowptr.data(), R->h_colidx.data(), hp.rowptr_ap.data(),
+                   hp.rowptr_c.data(), hp.pairptr2.data(), hp.t2.data(), hp.s2.data(), sp);
+      rc = stream_upload(sh2, sp, pl->s2, st);
     }
   }
-  if (rc == BSR_OK && (!pl->s1.ok || !pl->s2.ok)) {
-    if (!have_pairs) {
-      rc = hp.build(A->nbrows, A->h_rowptr.data(), A->h_colidx.data(), P->nbcols, P->h_rowptr.data(),
-                    P->h_colidx.data(), R->h_rowptr.data(), R->h_colidx.data(), true);
-      if (rc != BSR_OK) fail(rc, "ptap_symbolic: %s", hp.err.c_str());
-    }
-    pl->wide1 = hp.max_k1 > 255 || hp.max_q1 > 255;
-    pl->wide2 = hp.max_t2 > 255 || hp.max_s2 > 255;
-    if (rc == BSR_OK && !pl->s1.ok) {
-      rc = upload(&pl->rowidx_ap, hp.rowidx_ap, st);
-      if (rc == BSR_OK) rc = upload(&pl->pairptr1, hp.pairptr1, st);
-      if (rc == BSR_OK) rc = upload(&pl->pstart, hp.pstart, st);
-      if (rc == BSR_OK) rc = upload_pairs(&pl->pairs1, pl->wide1, hp.k1, hp.q1, st);
-    }
-    if (rc == BSR_OK && !pl->s2.ok) {
-      rc = upload(&pl->rowidx_c, hp.rowidx_c, st);
-      if (rc == BSR_OK) rc = upload(&pl->pairptr2, hp.pairptr2, st);
-      if (rc == BSR_OK) rc = upload(&pl->apstart, hp.apstart, st);
-      if (rc == BSR_OK) rc = upload_pairs(&pl->pairs2, pl->wide2, hp.t2, hp.s2, st);
-    }
+  // the gather lists go to the device only for a stage that stays on the fallback kernels
+  if (rc == BSR_OK && !pl->s1.ok) {
+    rc = upload(&pl->rowidx_ap, hp.rowidx_ap, st);
+    if (rc == BSR_OK) rc = upload(&pl->pairptr1, hp.pairptr1, st);
+    if (rc == BSR_OK) rc = upload(&pl->pstart, hp.pstart, st);
+    if (rc == BSR_OK) rc = upload_pairs(&pl->pairs1, pl->wide1, hp.k1, hp.q1, st);
+  }
+  if (rc == BSR_OK && !pl->s2.ok) {
+    rc = upload(&pl->rowidx_c, hp.rowidx_c, st);
+    if (rc == BSR_OK) rc = upload(&pl->pairptr2, hp.pairptr2, st);
+    if (rc == BSR_OK) rc = upload(&pl->apstart, hp.apstart, st);
+    if (rc == BSR_OK) rc = upload_pairs(&pl->pairs2, pl->wide2, hp.t2, hp.s2, st);
   }
   if (rc == BSR_OK && cudaStreamSynchronize(st) != cudaSuccess) rc = fail(BSR_ERR_CUDA, "plan upload failed");
   if (rc != BSR_OK) {

@@ -14,7 +14,6 @@
 #include <cstring>
 
 #include "internal.h"
-#include "ptap_prog.h"
 
 namespace bsramg {
 
@@ -41,8 +40,6 @@ struct Product {
   std::vector<int32_t>*rowptr_c, *colidx_c, *rowidx_c, *pairptr;
   std::vector<uint16_t>*off_x, *off_y;
   int32_t max_off_x = 0, max_off_y = 0;
-  int64_t nprod = 0;
-  bool want_pairs = true;
 };
 
 int symbolic_product(int32_t nrows, const int32_t* rowptr_x, const int32_t* colidx_x, const int32_t* rowptr_y,
@@ -71,14 +68,12 @@ int symbolic_product(int32_t nrows, const int32_t* rowptr_x, const int32_t* coli
   const int64_t nc = prefix(nblk, *out.rowptr_c);
   const int64_t np = prefix(nprod, prodptr);
   if (nc >= (1LL << 31) || np >= (1LL << 31)) { err = "more than 2^31 blocks or block products"; return BSR_ERR_LIMIT; }
-  out.nprod = np;
   out.colidx_c->resize((size_t)nc);
   out.rowidx_c->resize((size_t)nc);
-  const bool wp = out.want_pairs;
-  out.pairptr->assign(wp ? (size_t)nc + 1 : 0, 0);
-  out.off_x->resize(wp ? (size_t)np : 0);
-  out.off_y->resize(wp ? (size_t)np : 0);
-  if (wp) (*out.pairptr)[(size_t)nc] = (int32_t)np;
+  out.pairptr->resize((size_t)nc + 1);
+  out.off_x->resize((size_t)np);
+  out.off_y->resize((size_t)np);
+  (*out.pairptr)[(size_t)nc] = (int32_t)np;
   int32_t mx = 0, my = 0;
   // pass 2: fill.  key = (output column, offset in X's row, offset in Y's row); sorting groups by column and
   // orders each group by ascending x-slot, i.e. ascending inner index.
@@ -104,14 +99,12 @@ int symbolic_product(int32_t nrows, const int32_t* rowptr_x, const int32_t* coli
           ++slot;
           (*out.colidx_c)[slot] = (int32_t)col;
           (*out.rowidx_c)[slot] = i;
-          if (wp) (*out.pairptr)[slot] = p;
+          (*out.pairptr)[slot] = p;
           last = col;
         }
         const int32_t ox = (int32_t)((key >> 16) & 0xffff), oy = (int32_t)(key & 0xffff);
-        if (wp) {
-          (*out.off_x)[p] = (uint16_t)ox;
-          (*out.off_y)[p] = (uint16_t)oy;
-        }
+        (*out.off_x)[p] = (uint16_t)ox;
+        (*out.off_y)[p] = (uint16_t)oy;
         mx = std::max(mx, ox);
         my = std::max(my, oy);
         ++p;
@@ -127,26 +120,23 @@ int symbolic_product(int32_t nrows, const int32_t* rowptr_x, const int32_t* coli
 
 int HostPlan::build(int32_t nbrows_a_, const int32_t* rowptr_a, const int32_t* colidx_a, int32_t nbcols_p_,
                     const int32_t* rowptr_p, const int32_t* colidx_p, const int32_t* rowptr_r,
-                    const int32_t* colidx_r, bool want_pairs) {
+                    const int32_t* colidx_r) {
   nbrows_a = nbrows_a_;
   nbcols_p = nbcols_p_;
   // stage 1: AP = A * P
   Product s1;
-  s1.want_pairs = want_pairs;
   s1.rowptr_c = &rowptr_ap; s1.colidx_c = &colidx_ap; s1.rowidx_c = &rowidx_ap; s1.pairptr = &pairptr1;
   s1.off_x = &k1; s1.off_y = &q1;
   int rc = symbolic_product(nbrows_a, rowptr_a, colidx_a, rowptr_p, colidx_p, s1, err);
   if (rc != BSR_OK) return rc;
-  max_k1 = s1.max_off_x; max_q1 = s1.max_off_y; nprod1 = s1.nprod;
+  max_k1 = s1.max_off_x; max_q1 = s1.max_off_y;
   // stage 2: A_c = R * AP
   Product st2;
-  st2.want_pairs = want_pairs;
   st2.rowptr_c = &rowptr_c; st2.colidx_c = &colidx_c; st2.rowidx_c = &rowidx_c; st2.pairptr = &pairptr2;
   st2.off_x = &t2; st2.off_y = &s2;
   rc = symbolic_product(nbcols_p, rowptr_r, colidx_r, rowptr_ap.data(), colidx_ap.data(), st2, err);
   if (rc != BSR_OK) return rc;
-  max_t2 = st2.max_off_x; max_s2 = st2.max_off_y; nprod2 = st2.nprod;
-  if (!want_pairs) { pstart.clear(); apstart.clear(); return BSR_OK; }
+  max_t2 = st2.max_off_x; max_s2 = st2.max_off_y;
   // row starts of the gathered operand, one per slot of the left operand (saves one indirection in the kernels)
   const int64_t nnzb_a = rowptr_a[nbrows_a], nnzb_r = rowptr_r[nbcols_p];
   pstart.resize((size_t)nnzb_a);
@@ -168,8 +158,7 @@ extern "C" {
 struct ptap_host_plan_s {
   HostPlan plan;
   std::vector<int32_t> rowptr_r, colidx_r, perm_r;
-  std::vector<int32_t> rowptr_a, colidx_a, rowptr_p, colidx_p;   // copies, for ptap_host_prog_stats
-  int32_t nbcols_p = 0;
+  std::vector<int32_t> rowptr_a, colidx_a, rowptr_p;   // copies, for ptap_host_stream_stats
 };
 
 void* ptap_host_plan_build(int32_t nbrows_a, const int32_t* rowptr_a, const int32_t* colidx_a, int32_t nbcols_p,
@@ -184,8 +173,6 @@ void* ptap_host_plan_build(int32_t nbrows_a, const int32_t* rowptr_a, const int3
   h->rowptr_a.assign(rowptr_a, rowptr_a + nbrows_a + 1);
   h->colidx_a.assign(colidx_a, colidx_a + rowptr_a[nbrows_a]);
   h->rowptr_p.assign(rowptr_p, rowptr_p + nbrows_a + 1);
-  h->colidx_p.assign(colidx_p, colidx_p + rowptr_p[nbrows_a]);
-  h->nbcols_p = nbcols_p;
   int rc = h->plan.build(nbrows_a, rowptr_a, colidx_a, nbcols_p, rowptr_p, colidx_p, h->rowptr_r.data(),
                          h->colidx_r.data());
   if (rc != BSR_OK) {
@@ -212,35 +199,30 @@ int ptap_host_plan_get(void* handle, const char* name, const void** ptr, int64_t
   return fail(BSR_ERR_NULL, "ptap_host_plan_get: unknown array '%s'", name);
 }
 
-int ptap_host_prog_stats(void* handle, int32_t bs_f, int32_t bs_c, int32_t stage, int64_t smem_budget,
-                         int64_t* out12) {
-  if (!handle || !out12 || (stage != 1 && stage != 2)) return fail(BSR_ERR_NULL, "ptap_host_prog_stats: bad argument");
+int ptap_host_stream_stats(void* handle, int32_t bs_f, int32_t bs_c, int32_t stage, int64_t smem_budget,
+                           int64_t* out8) {
+  if (!handle || !out8 || (stage != 1 && stage != 2)) return fail(BSR_ERR_NULL, "ptap_host_stream_stats: bad argument");
   ptap_host_plan_s* h = (ptap_host_plan_s*)handle;
   const HostPlan& hp = h->plan;
-  ProgPlan pp;
-  const ProgShape sh = stage == 1 ? ProgShape{bs_f, bs_f, bs_c} : ProgShape{bs_c, bs_f, bs_c};
-  if (stage == 1)
-    prog_plan_stage1(sh, smem_budget, (int)options().round_len, hp.nbrows_a, h->rowptr_a.data(), h->colidx_a.data(), h->rowptr_p.data(),
-                     h->colidx_p.data(), h->nbcols_p, hp.rowptr_ap.data(), hp.colidx_ap.data(), pp, true);
-  else
-    prog_plan_stage2(sh, smem_budget, h->nbcols_p, h->rowptr_r.data(), h->colidx_r.data(), hp.rowptr_ap.data(),
-                     hp.colidx_ap.data(), hp.rowptr_c.data(), hp.colidx_c.data(), pp, true);
-  // every distinct program is checked against the relative structure it was built from; totals are weighted by the
-  // number of bricks that run the program
-  int64_t verified = pp.ok ? 1 : 0, products = 0, xq = 0, yq = 0, lane_steps = 0;
-  std::string why = pp.why;
-  for (size_t e = 0; e < pp.kept.size() && pp.ok; ++e) {
-    if (pp.kept_id[e] < 0) continue;
-    ProgStats st;
-    std::string w;
-    if (!prog_verify(sh, stage == 2, pp.kept[e].first, *pp.kept[e].second, w, &st)) { verified = 0; why = w; break; }
-    const int64_t uses = pp.prog_uses[(size_t)pp.kept_id[e]];
-    products += st.products * uses; lane_steps += st.lane_steps * uses; xq += st.xq_clk * uses; yq += st.yq_clk * uses;
+  std::vector<StreamBrickDef> bricks;
+  StreamPlan sp;
+  if (stage == 1) {
+    const StreamShape sh{bs_f, bs_f, bs_c};
+    stream_bricks_stage1(hp, sh, smem_budget, h->rowptr_a.data(), h->colidx_a.data(), h->rowptr_p.data(), bricks);
+    stream_build(sh, 8, smem_budget, bricks, h->rowptr_a.data(), h->colidx_a.data(), h->rowptr_p.data(),
+                 hp.rowptr_ap.data(), hp.pairptr1.data(), hp.k1.data(), hp.q1.data(), sp);
+  } else {
+    const StreamShape sh{bs_c, bs_f, bs_c};
+    stream_bricks_stage2(hp, sh, 4, smem_budget, h->rowptr_r.data(), h->colidx_r.data(), bricks);
+    stream_build(sh, 4, smem_budget, bricks, h->rowptr_r.data(), h->colidx_r.data(), hp.rowptr_ap.data(),
+                 hp.rowptr_c.data(), hp.pairptr2.data(), hp.t2.data(), hp.s2.data(), sp);
   }
-  if (!verified && !why.empty()) fail(BSR_ERR_PLAN, "%s", why.c_str());
-  out12[0] = pp.ok ? 1 : 0; out12[1] = pp.stats.bricks; out12[2] = pp.stats.programs; out12[3] = pp.max_smem;
-  out12[4] = products; out12[5] = lane_steps; out12[6] = pp.stats.plan_bytes; out12[7] = xq; out12[8] = yq;
-  out12[9] = verified; out12[10] = pp.nchunks; out12[11] = pp.nycopies;
+  int64_t bits = 0, lanes = 0, steps = 0;
+  for (const StreamMeta& m : sp.meta) bits += __builtin_popcount(m.mask);
+  for (const StreamEntry& e : sp.entries) lanes += e.nslots;
+  for (const StreamPass& p : sp.passes) steps += p.steps;
+  out8[0] = sp.ok ? 1 : 0; out8[1] = sp.nbricks(); out8[2] = sp.nchunks(); out8[3] = sp.max_smem;
+  out8[4] = bits; out8[5] = lanes; out8[6] = (int64_t)sp.passes.size(); out8[7] = steps;
   return BSR_OK;
 }
 

@@ -103,66 +103,20 @@ def test_host_plan_rejects_nothing_silently_on_empty_rows():
     assert hp.rowptr_c.tolist() == [0, 1, 1]
 
 
-def _random_bsr(rng, nbrows, nbcols, br, bc, maxlen):
-    rows, rp = [], [0]
-    for _ in range(nbrows):
-        n = int(rng.integers(0, min(maxlen, nbcols) + 1))
-        rows.append(np.sort(rng.choice(nbcols, size=n, replace=False)).astype(np.int32))
-        rp.append(rp[-1] + n)
-    ci = np.concatenate(rows) if rp[-1] else np.empty(0, np.int32)
-    return pr.HostBSR(nbrows, nbcols, br, bc, np.array(rp, np.int32), ci.astype(np.int32),
-                      rng.uniform(-1, 1, (rp[-1], br, bc)))
-
-
-def test_lane_programs_cover_every_product_once():
-    """Host logic of the numeric PtAP (ptap_prog.cpp): the library checks every distinct lane program against the
-    structure it was built from (each block product of each output block exactly once, on a lane of the right column
-    class, from the staged copy of the right blocks); here the totals are compared with the gather plan, every brick
-    must fit its shared-memory budget, the Y loads must be bank-conflict free under the quarter-warp model and the
-    lanes well used; structured meshes must share programs between bricks."""
-    cases = [(pr.make_generator(0), True), (pr.Generator(2, 24, seed=3), True), (pr.Generator(3, 13, seed=5), True)]
-    for g, structured in cases:
+def test_staged_schedule_covers_every_product_once():
+    """Host logic of the staged numeric PtAP (ptap_stream.cpp): the per-block masks of both stages must hold exactly
+    one bit per block product of the gather plan, every brick must fit its shared-memory budget, and stage 2 has one
+    brick per coarse row."""
+    from paper_2606_24748_b200 import bsr, problems as pr
+    for g in (pr.make_generator(0), pr.Generator(2, 24, seed=3), pr.Generator(3, 13, seed=5)):
         g.build_prolongator(0)
         A, P = g.A(0), g.P(0)
         hp = bsr.HostPlan(A, P)
-        s1, s2 = hp.prog_stats[1], hp.prog_stats[2]
-        assert s1["ok"] == 1 and s2["ok"] == 1, (s1, s2)
-        assert s1["verified"] == 1 and s2["verified"] == 1, (s1["why"], s2["why"])
-        assert s1["products"] == hp.k1.shape[0]          # stage 1: every A(i,j)*P(j,J) product once
-        assert s2["products"] == hp.t2.shape[0]          # stage 2: every R(I,i)*AP(i,K) product once
+        s1, s2 = hp.stream_stats[1], hp.stream_stats[2]
+        assert s1["ok"] == 1 and s2["ok"] == 1
+        assert s1["mask_bits"] == hp.k1.shape[0]          # stage 1: every A(i,j)*P(j,J) product once
+        assert s2["mask_bits"] == hp.t2.shape[0]          # stage 2: every R(I,i)*AP(i,K) product once
         assert s1["max_smem"] <= 112 * 1024 and s2["max_smem"] <= 75000
-        assert s2["bricks"] == P.nbcols and s2["chunks"] >= s2["programs"]
-        for s in (s1, s2):
-            assert s["yq_clk"] == 4 * s["lane_steps"] // 32     # Y reads: one wavefront per quarter warp
-            assert s["xq_clk"] <= 2.5 * 4 * s["lane_steps"] // 32
-        assert s1["programs"] <= s1["bricks"] and s2["programs"] <= s2["bricks"]
-    # a larger structured grid: interior bricks share programs, lanes are busy
-    g = pr.Generator(3, 26, seed=5)
-    g.build_prolongator(0)
-    hp = bsr.HostPlan(g.A(0), g.P(0))
-    s1, s2 = hp.prog_stats[1], hp.prog_stats[2]
-    assert s1["verified"] == 1 and s2["verified"] == 1
-    assert s1["programs"] < 0.6 * s1["bricks"] and s2["programs"] < 0.6 * s2["bricks"]
-    assert s1["products"] / s1["lane_steps"] > 0.7 and s2["products"] / s2["lane_steps"] > 0.5, (s1, s2)
-
-
-@pytest.mark.parametrize("shape", [(3, 6), (2, 3), (6, 6), (3, 3)])
-def test_lane_programs_on_irregular_structure(shape):
-    """Random sparsity (rows of 0..40 blocks, P rows of 0..9 blocks, AP rows far beyond 32 blocks): the program format
-    has no row-length limit; every product is still covered exactly once and small budgets force splitting."""
-    rng = np.random.default_rng(11)
-    bf, bc = shape
-    A = _random_bsr(rng, 150, 150, bf, bf, 40)
-    P = _random_bsr(rng, 150, 37, bf, bc, 9)
-    # a budget no single row fits in: the plan says so (ptap_symbolic then keeps the gather kernels)
-    if shape == (3, 6):
-        tiny = bsr.HostPlan(A, P, budgets=(20000, 12000)).prog_stats
-        assert tiny[1]["ok"] == 0 and tiny[2]["ok"] == 0
-    for budgets in ((112 * 1024, 75000), (90000, 60000)):
-        hp = bsr.HostPlan(A, P, budgets=budgets)
-        s1, s2 = hp.prog_stats[1], hp.prog_stats[2]
-        assert s1["ok"] == 1 and s1["verified"] == 1, (s1, s1["why"])
-        assert s2["ok"] == 1 and s2["verified"] == 1, (s2, s2["why"])
-        assert s1["products"] == hp.k1.shape[0] and s2["products"] == hp.t2.shape[0]
-        assert s1["max_smem"] <= budgets[0] and s2["max_smem"] <= budgets[1]
-        assert np.diff(hp.rowptr_ap).max() > 32
+        assert s2["bricks"] == P.nbcols and s2["chunks"] >= s2["bricks"]
+        assert s1["lanes"] == hp.colidx_ap.shape[0]       # one lane per AP block
+        assert s1["passes"] * 32 >= s1["lanes"] and s1["steps"] > 0
