@@ -14,6 +14,10 @@
 //   orc_ptap_form2      the same through a materialised AP and R (timed)    PAPER.md:103 ("local blocked triple product")
 //   orc_hier_*          block-Jacobi/Chebyshev V-cycle and PCG              PAPER.md:42 (cycle), 113 (pbjacobi, CG,
 //                                                                           unpreconditioned residual norm)
+//   orc_prolongator_smooth  P = (I - omega D^-1 A) P~ over the pattern of A P~   PAPER.md:54-56 (eq.), 244 (block AXPY
+//                                                                           with SUBSET_NONZERO_PATTERN)
+//   orc_bcoo_structure / orc_bcoo_sum   blocked COO assembly: coordinates declared once incl. duplicates, the value
+//                       stream of dense bs_r x bs_c blocks summed per destination
 // Floating point: fp64 data ("int32 indices and fp64 values"); sums that define one output
 // entry are accumulated in long double and rounded once (reading R14), except form2 and the
 // dense Cholesky, which use plain double (form2 is the timed CPU baseline).
@@ -21,7 +25,10 @@
 // Pins (tests/test_oracle_*.py, all `-m "not gpu"`): dense matvec / dense P^T A P by brute force at config 0
 // and a 2D grid; scipy.sparse BSR products; adjoint identity; closed-form structure counts; A_c symmetry and
 // rigid-body-mode annihilation; A_c^(k) = s_k A_c^(0); closed-form Chebyshev polynomial; two-grid operator
-// assembled densely; V-cycle symmetry; PCG with exact preconditioner.  No routine here is "parity unpinned".
+// assembled densely (two and three levels, 6x6 smoother blocks); V-cycle symmetry; PCG with exact preconditioner;
+// prolongator smoothing against the dense formula, the generator's own P and exact mode reproduction on a Neumann
+// problem; blocked COO against scipy's coordinate-format duplicate summation and a dense scatter-add.
+// No routine here is "parity unpinned".
 #include <algorithm>
 #include <cmath>
 #include <cstdint>
@@ -366,6 +373,126 @@ int orc_ptap_form2(const orc_bsr* Ap, const orc_bsr* Pp, const orc_bsr* Rp, cons
     }
   }
   return bad ? -2 : 0;
+}
+
+// ------------------------------------------------------------------ prolongator smoothing
+// P = (I - omega D^-1 A) P~, D the bs x bs block diagonal of A (reading R11), on the
+// boolean pattern of A*P~ (reading R5; the paper's MatAYPX adds P~ on a SUBSET of that pattern).
+// Row by row, in the paper's order: T_i(J) = sum_j A(i,j) P~(j,J); P(i,J) = P~(i,J) - omega * D_i^-1 * T_i(J).
+// Long double throughout (the inverse included), rounded once per entry.  (rowptr_p, colidx_p) is the symbolic
+// pattern of A*P~ (orc_spgemm_symbolic); a P~ block outside it is an error.
+int orc_prolongator_smooth(const orc_bsr* Ap, const orc_bsr* Ptp, double omega, const int32_t* rowptr_p,
+                           const int32_t* colidx_p, double* vals_p) {
+  const orc_bsr &A = *Ap, &Pt = *Ptp;
+  if (A.bs_r != A.bs_c || A.nbrows != A.nbcols || A.nbcols != Pt.nbrows || A.bs_c != Pt.bs_r || A.bs_r > 6) return -1;
+  const int bf = A.bs_r, bc = Pt.bs_c;
+  int bad = 0;
+#pragma omp parallel for schedule(static)
+  for (int32_t i = 0; i < A.nbrows; ++i) {
+    const int32_t* lo = colidx_p + rowptr_p[i];
+    const int32_t* hi = colidx_p + rowptr_p[i + 1];
+    const int64_t nslot = hi - lo;
+    std::vector<ld> T((size_t)nslot * bf * bc, 0.0L);
+    // D_i^-1 in long double (Gauss-Jordan with partial pivoting)
+    ld M[6][12];
+    bool found = false;
+    for (int64_t k = A.rowptr[i]; k < A.rowptr[i + 1]; ++k)
+      if (A.colidx[k] == i) {
+        for (int r = 0; r < bf; ++r)
+          for (int c = 0; c < bf; ++c) { M[r][c] = A.vals[(size_t)k * bf * bf + r * bf + c]; M[r][bf + c] = (r == c); }
+        found = true;
+      }
+    if (!found) { bad = 1; continue; }
+    for (int c = 0; c < bf; ++c) {
+      int p = c;
+      for (int r = c + 1; r < bf; ++r) if (fabsl(M[r][c]) > fabsl(M[p][c])) p = r;
+      if (M[p][c] == 0) { bad = 1; break; }
+      if (p != c) for (int j = 0; j < 2 * bf; ++j) std::swap(M[p][j], M[c][j]);
+      const ld piv = M[c][c];
+      for (int j = 0; j < 2 * bf; ++j) M[c][j] /= piv;
+      for (int r = 0; r < bf; ++r) if (r != c) {
+        const ld f = M[r][c];
+        for (int j = 0; j < 2 * bf; ++j) M[r][j] -= f * M[c][j];
+      }
+    }
+    // T_i = row i of A * P~
+    for (int64_t k = A.rowptr[i]; k < A.rowptr[i + 1]; ++k) {
+      const int32_t j = A.colidx[k];
+      const double* a = A.vals + (size_t)k * bf * bf;
+      for (int64_t q = Pt.rowptr[j]; q < Pt.rowptr[j + 1]; ++q) {
+        const int32_t* it = std::lower_bound(lo, hi, Pt.colidx[q]);
+        if (it == hi || *it != Pt.colidx[q]) { bad = 1; continue; }
+        ld* t = &T[(size_t)(it - lo) * bf * bc];
+        const double* p = Pt.vals + (size_t)q * bf * bc;
+        for (int r = 0; r < bf; ++r)
+          for (int c = 0; c < bc; ++c)
+            for (int m = 0; m < bf; ++m) t[r * bc + c] += (ld)a[r * bf + m] * (ld)p[m * bc + c];
+      }
+    }
+    // P(i,J) = P~(i,J) - omega D_i^-1 T_i(J)
+    for (int64_t s = 0; s < nslot; ++s) {
+      const double* own = nullptr;
+      for (int64_t q = Pt.rowptr[i]; q < Pt.rowptr[i + 1]; ++q)
+        if (Pt.colidx[q] == lo[s]) own = Pt.vals + (size_t)q * bf * bc;
+      for (int r = 0; r < bf; ++r)
+        for (int c = 0; c < bc; ++c) {
+          ld z = 0;
+          for (int m = 0; m < bf; ++m) z += M[r][bf + m] * T[(size_t)s * bf * bc + m * bc + c];
+          const ld v = (own ? (ld)own[r * bc + c] : 0.0L) - (ld)omega * z;
+          vals_p[((size_t)rowptr_p[i] + s) * bf * bc + r * bc + c] = (double)v;
+        }
+    }
+    // every P~ block of row i must lie inside the pattern (it does when A has its diagonal block)
+    for (int64_t q = Pt.rowptr[i]; q < Pt.rowptr[i + 1]; ++q) {
+      const int32_t* it = std::lower_bound(lo, hi, Pt.colidx[q]);
+      if (it == hi || *it != Pt.colidx[q]) bad = 1;
+    }
+  }
+  return bad ? -2 : 0;
+}
+
+// ------------------------------------------------------------------ blocked COO assembly
+// the caller declares once the (block row, block column) coordinate of every contribution,
+// duplicates included; the matrix has one block per distinct coordinate (rows in order, columns strictly ascending);
+// every numeric assembly sums, per destination block, the dense bs_r x bs_c blocks of the value stream that carry
+// its coordinate.  orc_bcoo_structure: pass colidx = null to count.  Returns nnzb, or -1 on a coordinate out of range.
+int64_t orc_bcoo_structure(int64_t n, const int32_t* brow, const int32_t* bcol, int32_t nbrows, int32_t nbcols,
+                           int32_t* rowptr, int32_t* colidx) {
+  std::vector<std::vector<int32_t>> rows((size_t)nbrows);
+  for (int64_t c = 0; c < n; ++c) {
+    if (brow[c] < 0 || brow[c] >= nbrows || bcol[c] < 0 || bcol[c] >= nbcols) return -1;
+    rows[(size_t)brow[c]].push_back(bcol[c]);
+  }
+  int64_t nnzb = 0;
+  rowptr[0] = 0;
+  for (int32_t i = 0; i < nbrows; ++i) {
+    std::vector<int32_t>& r = rows[(size_t)i];
+    std::sort(r.begin(), r.end());
+    r.erase(std::unique(r.begin(), r.end()), r.end());
+    if (colidx) std::copy(r.begin(), r.end(), colidx + nnzb);
+    nnzb += (int64_t)r.size();
+    rowptr[i + 1] = (int32_t)nnzb;
+  }
+  return nnzb;
+}
+
+// vals[slot(brow[c], bcol[c])] += stream block c, for c = 0..n-1 in coordinate (declaration) order: a plain
+// scatter-add, long double accumulators rounded once.  Returns -2 if a coordinate is not in the structure.
+int orc_bcoo_sum(int64_t n, const int32_t* brow, const int32_t* bcol, const double* stream, int32_t bs_r,
+                 int32_t bs_c, int32_t nbrows, const int32_t* rowptr, const int32_t* colidx, double* vals) {
+  const int bb = bs_r * bs_c;
+  const int64_t nnzb = rowptr[nbrows];
+  std::vector<ld> acc((size_t)nnzb * bb, 0.0L);
+  for (int64_t c = 0; c < n; ++c) {
+    const int32_t* lo = colidx + rowptr[brow[c]];
+    const int32_t* hi = colidx + rowptr[brow[c] + 1];
+    const int32_t* it = std::lower_bound(lo, hi, bcol[c]);
+    if (it == hi || *it != bcol[c]) return -2;
+    ld* a = &acc[(size_t)(it - colidx) * bb];
+    for (int e = 0; e < bb; ++e) a[e] += (ld)stream[(size_t)c * bb + e];
+  }
+  for (size_t t = 0; t < acc.size(); ++t) vals[t] = (double)acc[t];
+  return 0;
 }
 
 // ------------------------------------------------------------------ V-cycle / PCG (O10)

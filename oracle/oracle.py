@@ -66,6 +66,10 @@ def _load():
         lib.orc_spgemm_symbolic.argtypes = [C.c_int32, V, V, V, V, V, V]
         lib.orc_ptap_form1.argtypes = [P, P, V, V, V, C.c_int32, V]
         lib.orc_ptap_form2.argtypes = [P, P, P, V, V, V, V, V, V]
+        lib.orc_prolongator_smooth.argtypes = [P, P, C.c_double, V, V, V]
+        lib.orc_bcoo_structure.restype = C.c_int64
+        lib.orc_bcoo_structure.argtypes = [C.c_int64, V, V, C.c_int32, C.c_int32, V, V]
+        lib.orc_bcoo_sum.argtypes = [C.c_int64, V, V, V, C.c_int32, C.c_int32, C.c_int32, V, V, V]
         lib.orc_hier_create.restype = C.c_void_p
         lib.orc_hier_create.argtypes = [C.c_int, C.c_int, C.c_double, C.c_double]
         lib.orc_hier_destroy.argtypes = [V]
@@ -191,6 +195,42 @@ class PtapForm2:
         if rcode != 0:
             raise RuntimeError(f"orc_ptap_form2 failed ({rcode})")
         return OBsr(self.P.nbcols, self.P.nbcols, self.P.bs_c, self.P.bs_c, self.rc, self.cc, self.vals_c)
+
+
+def prolongator_smooth(A, Pt, omega: float) -> OBsr:
+    """P = (I - omega D^-1 A) P~ on the boolean pattern of A*P~ (D the block diagonal, R11)."""
+    rp, cp = spgemm_symbolic(A.nbrows, A.rowptr, A.colidx, Pt.rowptr, Pt.colidx)
+    ha, ht = _Held(A), _Held(Pt)
+    vals = np.zeros((cp.shape[0], Pt.bs_r, Pt.bs_c))
+    rcode = _load().orc_prolongator_smooth(ha.c, ht.c, float(omega), rp.ctypes.data, cp.ctypes.data, vals.ctypes.data)
+    if rcode != 0:
+        raise RuntimeError(f"orc_prolongator_smooth failed ({rcode})")
+    return OBsr(Pt.nbrows, Pt.nbcols, Pt.bs_r, Pt.bs_c, rp, cp, vals)
+
+
+def bcoo_assemble(brow, bcol, stream, nbrows: int, nbcols: int, structure=None) -> OBsr:
+    """Blocked COO assembly: one block per distinct (brow, bcol), each the sum of the
+    stream blocks (n, bs_r, bs_c) that carry its coordinate."""
+    brow, bcol = np.ascontiguousarray(brow, np.int32), np.ascontiguousarray(bcol, np.int32)
+    stream = np.ascontiguousarray(stream, np.float64)
+    n, bs_r, bs_c = stream.shape
+    assert brow.shape[0] == n and bcol.shape[0] == n
+    lib = _load()
+    if structure is None:
+        rp = np.empty(nbrows + 1, dtype=np.int32)
+        nnzb = lib.orc_bcoo_structure(n, brow.ctypes.data, bcol.ctypes.data, nbrows, nbcols, rp.ctypes.data, None)
+        if nnzb < 0:
+            raise RuntimeError("orc_bcoo_structure: coordinate out of range")
+        ci = np.empty(nnzb, dtype=np.int32)
+        lib.orc_bcoo_structure(n, brow.ctypes.data, bcol.ctypes.data, nbrows, nbcols, rp.ctypes.data, ci.ctypes.data)
+    else:
+        rp, ci = (np.ascontiguousarray(t, np.int32) for t in structure)
+    vals = np.empty((ci.shape[0], bs_r, bs_c))
+    rcode = lib.orc_bcoo_sum(n, brow.ctypes.data, bcol.ctypes.data, stream.ctypes.data, bs_r, bs_c, nbrows,
+                             rp.ctypes.data, ci.ctypes.data, vals.ctypes.data)
+    if rcode != 0:
+        raise RuntimeError(f"orc_bcoo_sum failed ({rcode})")
+    return OBsr(nbrows, nbcols, bs_r, bs_c, rp, ci, vals)
 
 
 class Hierarchy:

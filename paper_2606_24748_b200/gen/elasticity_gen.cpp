@@ -86,6 +86,8 @@ struct Gen {
   int modulus_mode = 0;  // 0: E = 1; 1: per-element lognormal(0, 1) (config 3)
   int dirichlet = 1;     // 0: pure Neumann operator (used by the invariant tests)
   std::vector<Level> levels;
+  std::vector<double> Emod;  // per-element modulus (empty: 1 everywhere)
+  std::vector<double> Ke;    // reference element matrix (E = 1)
   std::string err;
 };
 
@@ -148,7 +150,7 @@ void build_fine_operator(Gen& G) {
   // per-element Young's modulus (config 3: lognormal(0,1), Box-Muller cosine branch, element order)
   const int nez = (d == 3) ? ne : 1;
   const int64_t NE = (int64_t)ne * ne * nez;
-  std::vector<double> Emod;
+  std::vector<double>& Emod = G.Emod;
   if (G.modulus_mode == 1) {
     Emod.resize(NE);
     SplitMix64 g = stream(G.seed, 4);
@@ -158,7 +160,7 @@ void build_fine_operator(Gen& G) {
       Emod[e] = std::exp(z);
     }
   }
-  std::vector<double> Ke;
+  std::vector<double>& Ke = G.Ke;
   element_matrix(d, h, 1.0, G.nu, Ke);
   const int nen = 1 << d, nd = d * nen, bb = d * d;
 
@@ -573,6 +575,51 @@ int egen_element_matrix(int d, double h, double E, double nu, double* out) {
   std::vector<double> K;
   element_matrix(d, h, E, nu, K);
   std::memcpy(out, K.data(), sizeof(double) * K.size());
+  return 0;
+}
+
+// The finite-element contribution stream of elements [e0, e1) in ascending element order (blocked COO form,
+// PAPER.md:248-250): per element 4^d (2D: 16, 3D: 64) contributions (a, b), a slowest; coordinate = (node of a, node
+// of b); block = E_e * Ke[a][b] (d x d, row-major).  With Dirichlet the clamped face is folded into the stream: a
+// block whose row or column node has ix = 0 is zero, except the node's own diagonal block, which carries
+// I / (number of adjacent elements) so that the assembled block is exactly I (R4).  Any output may be null.
+int egen_element_stream(egen_t G, int64_t e0, int64_t e1, int32_t* brow, int32_t* bcol, double* vals) {
+  if (!G || e0 < 0 || e1 < e0) return -1;
+  const int d = G->d, ne = G->ne, n = ne + 1, nen = 1 << d, nd = d * nen, bb = d * d;
+  const int64_t NE = (int64_t)ne * ne * (d == 3 ? ne : 1);
+  if (e1 > NE) return -2;
+#pragma omp parallel for schedule(static)
+  for (int64_t e = e0; e < e1; ++e) {
+    const int ex = (int)(e % ne), ey = (int)((e / ne) % ne), ez = (d == 3) ? (int)(e / ((int64_t)ne * ne)) : 0;
+    const double Ee = G->Emod.empty() ? 1.0 : G->Emod[(size_t)e];
+    for (int a = 0; a < nen; ++a)
+      for (int b = 0; b < nen; ++b) {
+        const int64_t c = (e - e0) * nen * nen + a * nen + b;
+        const int ax = ex + (a & 1), ay = ey + ((a >> 1) & 1), az = ez + ((a >> 2) & 1);
+        const int bx = ex + (b & 1), by = ey + ((b >> 1) & 1), bz = ez + ((b >> 2) & 1);
+        if (brow) brow[c] = (int32_t)(ax + (int64_t)n * (ay + (int64_t)n * az));
+        if (bcol) bcol[c] = (int32_t)(bx + (int64_t)n * (by + (int64_t)n * bz));
+        if (!vals) continue;
+        double* blk = vals + (size_t)c * bb;
+        for (int i = 0; i < d; ++i)
+          for (int j = 0; j < d; ++j) blk[i * d + j] = Ee * G->Ke[(size_t)(a * d + i) * nd + (b * d + j)];
+        if (G->dirichlet && (ax == 0 || bx == 0)) {
+          for (int t = 0; t < bb; ++t) blk[t] = 0.0;
+          if (a == b) {
+            const int cy = (ay > 0 && ay < ne) ? 2 : 1, cz = (d == 3 && az > 0 && az < ne) ? 2 : 1;
+            for (int i = 0; i < d; ++i) blk[i * d + i] = 1.0 / (double)(cy * cz);
+          }
+        }
+      }
+  }
+  return 0;
+}
+
+// borrowed: per-element moduli (null when E = 1 everywhere) and the reference element matrix (E = 1)
+int egen_element_data(egen_t G, const double** emod, const double** ke) {
+  if (!G) return -1;
+  *emod = G->Emod.empty() ? nullptr : G->Emod.data();
+  *ke = G->Ke.data();
   return 0;
 }
 

@@ -41,6 +41,9 @@ def _load():
         lib.egen_level_arrays.argtypes = [C.c_void_p, C.c_int, C.POINTER(C.POINTER(C.c_double)),
                                           C.POINTER(C.POINTER(C.c_double)), C.POINTER(C.POINTER(C.c_int32))]
         lib.egen_element_matrix.argtypes = [C.c_int, C.c_double, C.c_double, C.c_double, C.c_void_p]
+        lib.egen_element_stream.argtypes = [C.c_void_p, C.c_int64, C.c_int64, C.c_void_p, C.c_void_p, C.c_void_p]
+        lib.egen_element_data.argtypes = [C.c_void_p, C.POINTER(C.POINTER(C.c_double)),
+                                          C.POINTER(C.POINTER(C.c_double))]
         lib.egen_uniform.argtypes = [C.c_uint64, C.c_uint64, C.c_int64, C.c_double, C.c_double, C.c_void_p]
         _lib = lib
     return _lib
@@ -154,6 +157,32 @@ class Generator:
                                          va.ctypes.data)
         if rc != 0:
             raise RuntimeError(f"egen_set_operator failed ({rc})")
+
+    @property
+    def nelements(self) -> int:
+        return self.ne ** self.d
+
+    def element_stream(self, e0: int = 0, e1: int | None = None, values: bool = True):
+        """Blocked COO contribution stream of elements [e0, e1): (brow, bcol, blocks (n, d, d)),
+        4^d contributions per element in element order; the clamped face is folded into the blocks (R4)."""
+        e1 = self.nelements if e1 is None else e1
+        n = (e1 - e0) * 4 ** self.d
+        brow, bcol = np.empty(n, dtype=np.int32), np.empty(n, dtype=np.int32)
+        vals = np.empty((n, self.d, self.d)) if values else None
+        rc = self._lib.egen_element_stream(self._h, e0, e1, brow.ctypes.data, bcol.ctypes.data,
+                                           vals.ctypes.data if values else None)
+        if rc != 0:
+            raise ValueError(f"egen_element_stream failed ({rc})")
+        return brow, bcol, vals
+
+    def element_data(self):
+        """(per-element moduli or None, reference element matrix for E = 1): inputs of the device-side emission."""
+        em, ke = C.POINTER(C.c_double)(), C.POINTER(C.c_double)()
+        self._lib.egen_element_data(self._h, em, ke)
+        nd = self.d * 2 ** self.d
+        K = np.ctypeslib.as_array(ke, shape=(nd, nd)).copy()
+        E = np.ctypeslib.as_array(em, shape=(self.nelements,)).copy() if em else None
+        return E, K
 
     def level_info(self, level: int) -> dict:
         nn, bs, nb = C.c_int32(), C.c_int32(), C.c_int32()
