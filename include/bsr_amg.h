@@ -39,6 +39,8 @@ extern "C" {
 typedef struct bsr_matrix_s* bsr_t;      /* opaque; created by bsr_create, released by bsr_destroy   */
 typedef struct ptap_plan_s* ptap_plan_t; /* opaque; created by ptap_symbolic, released by ptap_destroy */
 typedef struct vcycle_s* vcycle_t;       /* opaque; created by vcycle_create, released by vcycle_destroy */
+typedef struct psmooth_plan_s* psmooth_plan_t; /* opaque; prolongator_smooth_symbolic / prolongator_smooth_destroy */
+typedef struct bcoo_plan_s* bcoo_plan_t;       /* opaque; bcoo_plan_create / bcoo_destroy */
 
 enum {
   BSR_OK = 0,
@@ -186,6 +188,62 @@ int pcg_solve(vcycle_t vc, const double* d_b, double* d_x, int32_t iters, double
 /* End-to-end convenience with HOST vectors (copies, runs vcycle_apply, copies back, synchronises). */
 int vcycle_apply_host(vcycle_t vc, const double* h_b, double* h_x, void* stream);
 int vcycle_destroy(vcycle_t vc);
+
+/* ------------------------------------------------------------------ prolongator smoothing
+ * P = (I - omega D^-1 A) P~: "one step of a damped-Jacobi prolongator smoother", D the bs x bs block
+ * diagonal of A, in blocks on the device; the block AXPY that adds P~ on a subset of the pattern (the paper's MatAYPX
+ * with SUBSET_NONZERO_PATTERN) and the D^-1 left-multiply are fused into the store of the product A*P~,
+ * so the step is ONE pass over A.
+ * prolongator_smooth_symbolic (COLD): from the STRUCTURES of A (square, bs x bs, every row holding its diagonal block)
+ *   and P~ (bs x bs_coarse; shapes 2x3, 3x3, 3x6, 6x6) computes the structure of P = boolean pattern of A*P~ (columns
+ *   strictly ascending, blocks kept even if numerically zero) and the product schedule.  Outputs *nnzb_p.
+ *   Errors: BSR_ERR_NULL, BSR_ERR_SHAPE, BSR_ERR_BLOCK, BSR_ERR_STRUCTURE (a P~ block outside the pattern: A lacks a
+ *   diagonal block), BSR_ERR_ALLOC, BSR_ERR_LIMIT, BSR_ERR_CUDA.
+ * prolongator_smooth_structure: copies P's structure into caller-allocated device arrays d_rowptr_p[nbrows+1],
+ *   d_colidx_p[nnzb_p].
+ * prolongator_smooth_numeric (HOT: enqueues two kernels, no allocation, no synchronisation): d_vals_p[nnzb_p*bs*bsc]
+ *   (16-byte aligned) = values of P for the CURRENT values of A and P~ and the given omega.  A singular or missing
+ *   diagonal block is reported by prolongator_smooth_status (COLD: synchronises) as BSR_ERR_NUMERIC.
+ * prolongator_smooth_get_info: block products A(i,j)*P~(j,J), algorithmic bytes bytes(A)+bytes(P~)+bytes(P), and
+ *   whether the staged kernel (1) or the gather fallback (0) runs. */
+int prolongator_smooth_symbolic(psmooth_plan_t* out, bsr_t A, bsr_t P_tent, int64_t* nnzb_p, void* stream);
+int prolongator_smooth_structure(psmooth_plan_t plan, int32_t* d_rowptr_p, int32_t* d_colidx_p, void* stream);
+int prolongator_smooth_numeric(psmooth_plan_t plan, bsr_t A, bsr_t P_tent, double omega, double* d_vals_p,
+                               void* stream);
+int prolongator_smooth_status(psmooth_plan_t plan, void* stream);
+int prolongator_smooth_get_info(psmooth_plan_t plan, int64_t* n_products, int64_t* algorithmic_bytes, int32_t* staged);
+int prolongator_smooth_destroy(psmooth_plan_t plan);
+
+/* ------------------------------------------------------------------ blocked COO assembly
+ * "Each declared coordinate addresses a block, the value stream is a sequence of dense blocks (square or rectangular),
+ * and the scatter writes and sums contiguous bs_r*bs_c runs".
+ * bcoo_plan_create (COLD, synchronises): the caller declares ONCE the block coordinates (d_brow[c], d_bcol[c]),
+ *   c = 0..n-1, of every contribution, duplicates included (device arrays, read here and not kept).  The plan holds
+ *   the structure of the assembled matrix (one block per distinct coordinate; rows with no contribution are empty;
+ *   columns strictly ascending) and the duplicate-summation map in gather form.  Outputs *nnzb.
+ *   Errors: BSR_ERR_NULL, BSR_ERR_SHAPE, BSR_ERR_BLOCK, BSR_ERR_STRUCTURE (coordinate out of range), BSR_ERR_LIMIT
+ *   (n >= 2^31 or nnzb*bs_r*bs_c >= 2^31), BSR_ERR_ALLOC, BSR_ERR_CUDA.
+ * bcoo_structure: copies the structure into caller-allocated device arrays d_rowptr[nbrows+1], d_colidx[nnzb].
+ * bcoo_set_values (HOT, one kernel): d_vals[nnzb*bs_r*bs_c] <- for every block the sum, in declaration order, of the
+ *   stream blocks d_stream[c*bs_r*bs_c ...] (row-major) that carry its coordinate.  No atomics; d_vals is overwritten.
+ * bcoo_get_info: contributions, blocks, algorithmic bytes 8*bs_r*bs_c*(n + nnzb) + 4*n + 4*(nnzb+1). */
+int bcoo_plan_create(bcoo_plan_t* out, int64_t n, const int32_t* d_brow, const int32_t* d_bcol, int32_t nbrows,
+                     int32_t nbcols, int32_t bs_r, int32_t bs_c, int64_t* nnzb, void* stream);
+int bcoo_structure(bcoo_plan_t plan, int32_t* d_rowptr, int32_t* d_colidx, void* stream);
+int bcoo_set_values(bcoo_plan_t plan, const double* d_stream, double* d_vals, void* stream);
+int bcoo_get_info(bcoo_plan_t plan, int64_t* n_contrib, int64_t* nnzb, int64_t* algorithmic_bytes);
+int bcoo_destroy(bcoo_plan_t plan);
+/* Finite-element driver of the primitive ("finite-element assembly the natural next application"): Q1
+ * elasticity on the uniform grid of ne elements per side (d = 2 or 3), elements [e0, e1) in ascending order, 4^d
+ * contributions (a, b) per element, a slowest; local node a sits at offset bit k of a in direction k.
+ * fem_q1_element_coords: d_brow / d_bcol [(e1-e0)*4^d] = global node of a / of b.
+ * fem_q1_element_blocks: d_stream[(e1-e0)*4^d*d*d] = E_e * Ke[a][b] blocks (d_Ke: the (d*2^d)^2 reference element
+ *   matrix for E = 1, row-major; d_E: one modulus per element of the WHOLE grid, or null for E = 1).  dirichlet != 0
+ *   folds the clamped face ix = 0 into the stream (a block whose row or column node is clamped is zero, the node's own
+ *   diagonal block carries I / #adjacent elements: the assembled block is exactly I, reading R4). */
+int fem_q1_element_coords(int32_t d, int32_t ne, int64_t e0, int64_t e1, int32_t* d_brow, int32_t* d_bcol, void* stream);
+int fem_q1_element_blocks(int32_t d, int32_t ne, int64_t e0, int64_t e1, const double* d_Ke, const double* d_E,
+                          int32_t dirichlet, double* d_stream, void* stream);
 
 /* ------------------------------------------------------------------ counters (metrics)
  * Process-wide counts since load: kernels launched by this library, device allocations made by this library.

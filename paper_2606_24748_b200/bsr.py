@@ -55,6 +55,19 @@ SYMBOLS = {
     "vcycle_apply_host": (C.c_int, [_V, _V, _V, _V]),
     "vcycle_destroy": (C.c_int, [_V]),
     "bsr_counters": (C.c_int, [_PI64, _PI64]),
+    "prolongator_smooth_symbolic": (C.c_int, [_PV, _V, _V, _PI64, _V]),
+    "prolongator_smooth_structure": (C.c_int, [_V, _V, _V, _V]),
+    "prolongator_smooth_numeric": (C.c_int, [_V, _V, _V, _D, _V, _V]),
+    "prolongator_smooth_status": (C.c_int, [_V, _V]),
+    "prolongator_smooth_get_info": (C.c_int, [_V, _PI64, _PI64, _PI32]),
+    "prolongator_smooth_destroy": (C.c_int, [_V]),
+    "bcoo_plan_create": (C.c_int, [_PV, _I64, _V, _V, _I32, _I32, _I32, _I32, _PI64, _V]),
+    "bcoo_structure": (C.c_int, [_V, _V, _V, _V]),
+    "bcoo_set_values": (C.c_int, [_V, _V, _V, _V]),
+    "bcoo_get_info": (C.c_int, [_V, _PI64, _PI64, _PI64]),
+    "bcoo_destroy": (C.c_int, [_V]),
+    "fem_q1_element_coords": (C.c_int, [_I32, _I32, _I64, _I64, _V, _V, _V]),
+    "fem_q1_element_blocks": (C.c_int, [_I32, _I32, _I64, _I64, _V, _V, _I32, _V, _V]),
 }
 
 
@@ -259,6 +272,122 @@ class PtapPlan:
         va = torch.empty(n * bf * bc, dtype=torch.float64, device=dev)
         _check(lib().ptap_get_ap(self.h, _dev(rp), _dev(ci), _dev(va), _stream()))
         return rp.cpu().numpy(), ci.cpu().numpy(), va.cpu().numpy().reshape(n, bf, bc)
+
+
+class ProlongatorSmoother:
+    """P = (I - omega D^-1 A) P~ on the device (prolongator_smooth_*)."""
+
+    def __init__(self, A: Bsr, P_tent: Bsr):
+        import torch
+        self.A, self.Pt = A, P_tent
+        h, nnz = C.c_void_p(), C.c_int64()
+        _check(lib().prolongator_smooth_symbolic(C.byref(h), A.h, P_tent.h, C.byref(nnz), _stream()))
+        self.h, self.nnzb_p = h, nnz.value
+        dev = A.vals.device
+        self.rowptr_p = torch.empty(A.nbrows + 1, dtype=torch.int32, device=dev)
+        self.colidx_p = torch.empty(self.nnzb_p, dtype=torch.int32, device=dev)
+        _check(lib().prolongator_smooth_structure(self.h, _dev(self.rowptr_p), _dev(self.colidx_p), _stream()))
+
+    def close(self):
+        if getattr(self, "h", None):
+            lib().prolongator_smooth_destroy(self.h)
+            self.h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def info(self) -> dict:
+        a, b, c = C.c_int64(), C.c_int64(), C.c_int32()
+        _check(lib().prolongator_smooth_get_info(self.h, C.byref(a), C.byref(b), C.byref(c)))
+        return dict(n_products=a.value, algorithmic_bytes=b.value, staged=bool(c.value))
+
+    def new_values(self):
+        import torch
+        return torch.empty(self.nnzb_p * self.Pt.bs_r * self.Pt.bs_c, dtype=torch.float64, device=self.A.vals.device)
+
+    def numeric(self, omega: float, vals_p=None, check: bool = False):
+        """vals_p = values of the smoothed prolongator for the current A, P~ (prolongator_smooth_numeric)."""
+        if vals_p is None:
+            vals_p = self.new_values()
+        _check(lib().prolongator_smooth_numeric(self.h, self.A.h, self.Pt.h, float(omega), _dev(vals_p), _stream()))
+        if check:
+            _check(lib().prolongator_smooth_status(self.h, _stream()))
+        return vals_p
+
+    def matrix(self, vals_p) -> Bsr:
+        """Wrap P (structure of the plan, given values) as a Bsr."""
+        return Bsr(self.A.nbrows, self.Pt.nbcols, self.Pt.bs_r, self.Pt.bs_c, self.rowptr_p, self.colidx_p, vals_p)
+
+
+class BcooPlan:
+    """Blocked COO assembly plan (bcoo_plan_create): coordinates declared once."""
+
+    def __init__(self, brow, bcol, nbrows: int, nbcols: int, bs_r: int, bs_c: int):
+        import torch
+        assert brow.dtype == torch.int32 and bcol.dtype == torch.int32 and brow.numel() == bcol.numel()
+        self.nbrows, self.nbcols, self.bs_r, self.bs_c, self.n = nbrows, nbcols, bs_r, bs_c, int(brow.numel())
+        h, nnz = C.c_void_p(), C.c_int64()
+        _check(lib().bcoo_plan_create(C.byref(h), self.n, _dev(brow), _dev(bcol), nbrows, nbcols, bs_r, bs_c,
+                                      C.byref(nnz), _stream()))
+        self.h, self.nnzb = h, nnz.value
+        self.rowptr = torch.empty(nbrows + 1, dtype=torch.int32, device=brow.device)
+        self.colidx = torch.empty(self.nnzb, dtype=torch.int32, device=brow.device)
+        _check(lib().bcoo_structure(self.h, _dev(self.rowptr), _dev(self.colidx), _stream()))
+
+    def close(self):
+        if getattr(self, "h", None):
+            lib().bcoo_destroy(self.h)
+            self.h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def info(self) -> dict:
+        v = [C.c_int64() for _ in range(3)]
+        _check(lib().bcoo_get_info(self.h, *[C.byref(t) for t in v]))
+        return dict(n_contrib=v[0].value, nnzb=v[1].value, algorithmic_bytes=v[2].value)
+
+    def new_values(self):
+        import torch
+        return torch.empty(self.nnzb * self.bs_r * self.bs_c, dtype=torch.float64, device=self.rowptr.device)
+
+    def set_values(self, stream, vals=None):
+        """vals = the assembled block values for this stream of contribution blocks (bcoo_set_values)."""
+        assert stream.numel() == self.n * self.bs_r * self.bs_c
+        if vals is None:
+            vals = self.new_values()
+        _check(lib().bcoo_set_values(self.h, _dev(stream), _dev(vals), _stream()))
+        return vals
+
+    def matrix(self, vals) -> Bsr:
+        return Bsr(self.nbrows, self.nbcols, self.bs_r, self.bs_c, self.rowptr, self.colidx, vals)
+
+
+def fem_q1_coords(d: int, ne: int, e0: int, e1: int, device="cuda"):
+    """(brow, bcol) of the Q1 element contributions of elements [e0, e1) (fem_q1_element_coords)."""
+    import torch
+    n = (e1 - e0) * 4 ** d
+    brow = torch.empty(n, dtype=torch.int32, device=device)
+    bcol = torch.empty(n, dtype=torch.int32, device=device)
+    _check(lib().fem_q1_element_coords(d, ne, e0, e1, _dev(brow), _dev(bcol), _stream()))
+    return brow, bcol
+
+
+def fem_q1_blocks(d: int, ne: int, e0: int, e1: int, Ke, E, dirichlet: bool, out=None):
+    """The stream of E_e * Ke[a][b] blocks of elements [e0, e1) (fem_q1_element_blocks); Ke, E device tensors."""
+    import torch
+    n = (e1 - e0) * 4 ** d * d * d
+    if out is None:
+        out = torch.empty(n, dtype=torch.float64, device=Ke.device)
+    assert out.numel() == n
+    _check(lib().fem_q1_element_blocks(d, ne, e0, e1, _dev(Ke), _dev(E), 1 if dirichlet else 0, _dev(out), _stream()))
+    return out
 
 
 class HostPlan:

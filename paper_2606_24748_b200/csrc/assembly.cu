@@ -1,0 +1,263 @@
+// assembly.cu -- blocked COO assembly of a BSR matrix and its finite-element driver.
+//
+// "the caller supplies, once, the (i,j) coordinates of every contribution ... builds a cached ...
+// scatter plan, and thereafter each numeric assembly is a single MatSetValuesCOO that scatters a flat value array and
+// sums duplicates, entirely on the device.  We generalize this to blocks ... each coordinate addresses a dense
+// bs_r x bs_c block ... The block size need not be square".  PAPER.md:248-250: "the value stream is a sequence of
+// dense blocks (square or rectangular), and the scatter writes and sums contiguous bs_r*bs_c runs"; finite-element
+// assembly, "where per-element dense matrices generate exactly such a stream of duplicated ... contributions", is
+// named as the next application.
+//
+// bcoo_plan_create (COLD) builds the sorted-unique map once: the matrix structure (one block per distinct coordinate,
+// columns strictly ascending) and, per destination block, the ordered list of stream positions that carry its
+// coordinate -- the duplicate-summation map in GATHER form.  bcoo_set_values (HOT) is one kernel: every destination
+// value is the sum of its contributions in declaration order, read as contiguous bs_r*bs_c runs of the stream and
+// written once.  No atomics, bit-reproducible.  The fem_q1_* calls are the driver for Q1 elasticity: 4^d block
+// contributions per element, scaled by the element's modulus on the device.
+#include <algorithm>
+#include <numeric>
+
+#include "internal.h"
+
+struct bcoo_plan_s {
+  uint64_t magic = 0;
+  int64_t n = 0, nnzb = 0;
+  int32_t nbrows = 0, nbcols = 0, bs_r = 0, bs_c = 0;
+  int32_t *rowptr = nullptr, *colidx = nullptr, *segptr = nullptr, *perm = nullptr;
+};
+static const uint64_t BCOO_MAGIC = 0x42434f4f504c414eull;
+
+namespace bsramg {
+
+// one thread per destination value: consecutive threads read consecutive doubles of the same contribution block
+template <int BB>
+__global__ void __launch_bounds__(256)
+bcoo_sum_kernel(int64_t nvals, const int32_t* __restrict__ segptr, const int32_t* __restrict__ perm,
+                const double* __restrict__ stream, double* __restrict__ vals) {
+  const int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= nvals) return;
+  const int64_t slot = t / BB;
+  const int e = (int)(t - slot * BB);
+  const int32_t p0 = __ldg(segptr + slot), p1 = __ldg(segptr + slot + 1);
+  double s = 0.0;
+  int32_t p = p0;
+  for (; p + 1 < p1; p += 2) {   // two independent loads in flight, added in declaration order
+    const double v0 = __ldg(stream + (int64_t)__ldg(perm + p) * BB + e);
+    const double v1 = __ldg(stream + (int64_t)__ldg(perm + p + 1) * BB + e);
+    s += v0;
+    s += v1;
+  }
+  if (p < p1) s += __ldg(stream + (int64_t)__ldg(perm + p) * BB + e);
+  vals[t] = s;
+}
+
+// ---- Q1 elasticity driver: element e = ex + ne*(ey + ne*ez), local node a has offset bit k of a in direction k
+__device__ __forceinline__ void q1_nodes(int d, int ne, int64_t e, int a, int b, int& ia, int& ib, int (&ca)[3], int (&cb)[3]) {
+  const int n = ne + 1;
+  const int ex = (int)(e % ne), ey = (int)((e / ne) % ne), ez = (d == 3) ? (int)(e / ((int64_t)ne * ne)) : 0;
+  ca[0] = ex + (a & 1); ca[1] = ey + ((a >> 1) & 1); ca[2] = ez + ((a >> 2) & 1);
+  cb[0] = ex + (b & 1); cb[1] = ey + ((b >> 1) & 1); cb[2] = ez + ((b >> 2) & 1);
+  ia = ca[0] + n * (ca[1] + n * ca[2]);
+  ib = cb[0] + n * (cb[1] + n * cb[2]);
+}
+
+__global__ void __launch_bounds__(256)
+q1_coords_kernel(int d, int ne, int64_t e0, int64_t ncontrib, int32_t* __restrict__ brow, int32_t* __restrict__ bcol) {
+  const int64_t c = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (c >= ncontrib) return;
+  const int nen = 1 << d, nn = nen * nen;
+  const int64_t e = e0 + c / nn;
+  const int ab = (int)(c % nn), a = ab / nen, b = ab % nen;
+  int ia, ib, ca[3], cb[3];
+  q1_nodes(d, ne, e, a, b, ia, ib, ca, cb);
+  brow[c] = ia;
+  bcol[c] = ib;
+}
+
+// stream value (c, i, j) = E_e * Ke[a*d+i][b*d+j]; with `dirichlet` the face ix = 0 is clamped in the stream itself
+// (reading R4): a block whose row or column node is clamped is zero, except the node's own diagonal block,
+// which carries I / (number of elements adjacent to the node) so that the assembled block is exactly I
+__global__ void __launch_bounds__(256)
+q1_blocks_kernel(int d, int ne, int64_t e0, int64_t nvals, const double* __restrict__ Ke, const double* __restrict__ E,
+                 int dirichlet, double* __restrict__ stream) {
+  const int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= nvals) return;
+  const int nen = 1 << d, nn = nen * nen, bb = d * d, nd = d * nen;
+  const int64_t c = t / bb;
+  const int ij = (int)(t - c * bb), i = ij / d, j = ij - i * d;
+  const int64_t e = e0 + c / nn;
+  const int ab = (int)(c % nn), a = ab / nen, b = ab % nen;
+  double v = (E ? __ldg(E + e) : 1.0) * __ldg(Ke + (a * d + i) * nd + (b * d + j));
+  if (dirichlet) {
+    int ia, ib, ca[3], cb[3];
+    q1_nodes(d, ne, e, a, b, ia, ib, ca, cb);
+    if (ca[0] == 0 || cb[0] == 0) {
+      v = 0.0;
+      if (a == b && i == j) {
+        const int cy = (ca[1] > 0 && ca[1] < ne) ? 2 : 1;
+        const int cz = (d == 3 && ca[2] > 0 && ca[2] < ne) ? 2 : 1;
+        v = 1.0 / (double)(cy * cz);
+      }
+    }
+  }
+  stream[t] = v;
+}
+
+static void bcoo_release(bcoo_plan_s* pl) {
+  if (!pl) return;
+  dev_free(pl->rowptr); dev_free(pl->colidx); dev_free(pl->segptr); dev_free(pl->perm);
+  pl->magic = 0;
+  delete pl;
+}
+
+}  // namespace bsramg
+
+using namespace bsramg;
+
+extern "C" {
+
+int bcoo_plan_create(bcoo_plan_t* out, int64_t n, const int32_t* d_brow, const int32_t* d_bcol, int32_t nbrows,
+                     int32_t nbcols, int32_t bs_r, int32_t bs_c, int64_t* nnzb_out, void* stream) {
+  if (!out) return fail(BSR_ERR_NULL, "bcoo_plan_create: out is null");
+  *out = nullptr;
+  if (n < 0 || nbrows < 0 || nbcols < 0) return fail(BSR_ERR_SHAPE, "negative size");
+  if (n > 0 && (!d_brow || !d_bcol)) return fail(BSR_ERR_NULL, "null coordinate array");
+  if (!shape_supported(bs_r, bs_c)) return fail(BSR_ERR_BLOCK, "unsupported block shape %dx%d", bs_r, bs_c);
+  if (n >= (1LL << 31)) return fail(BSR_ERR_LIMIT, "2^31 or more contributions");
+  cudaStream_t st = (cudaStream_t)stream;
+  std::vector<int32_t> br((size_t)n), bc((size_t)n);
+  if (n) {
+    CUDA_TRY(cudaMemcpyAsync(br.data(), d_brow, (size_t)n * 4, cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(cudaMemcpyAsync(bc.data(), d_bcol, (size_t)n * 4, cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(cudaStreamSynchronize(st));
+  }
+  // counting sort of the contributions by block row (stable: declaration order inside a row)
+  std::vector<int64_t> rstart((size_t)nbrows + 1, 0);
+  int bad = 0;
+  for (int64_t c = 0; c < n; ++c) {
+    if (br[(size_t)c] < 0 || br[(size_t)c] >= nbrows || bc[(size_t)c] < 0 || bc[(size_t)c] >= nbcols) { bad = 1; break; }
+    rstart[(size_t)br[(size_t)c] + 1]++;
+  }
+  if (bad) return fail(BSR_ERR_STRUCTURE, "block coordinate out of range");
+  for (int32_t i = 0; i < nbrows; ++i) rstart[(size_t)i + 1] += rstart[(size_t)i];
+  std::vector<int32_t> byrow((size_t)n);
+  {
+    std::vector<int64_t> fill(rstart.begin(), rstart.end() - 1);
+    for (int64_t c = 0; c < n; ++c) byrow[(size_t)fill[(size_t)br[(size_t)c]]++] = (int32_t)c;
+  }
+  // inside each row: order by (column, declaration index); distinct columns become the row's blocks
+  std::vector<int32_t> nblk((size_t)nbrows, 0);
+#pragma omp parallel for schedule(dynamic, 1024)
+  for (int32_t i = 0; i < nbrows; ++i) {
+    int32_t* lo = byrow.data() + rstart[(size_t)i];
+    int32_t* hi = byrow.data() + rstart[(size_t)i + 1];
+    std::sort(lo, hi, [&](int32_t u, int32_t v) { return bc[(size_t)u] != bc[(size_t)v] ? bc[(size_t)u] < bc[(size_t)v] : u < v; });
+    int32_t cnt = 0;
+    for (int32_t* p = lo; p < hi; ++p)
+      if (p == lo || bc[(size_t)*p] != bc[(size_t)p[-1]]) ++cnt;
+    nblk[(size_t)i] = cnt;
+  }
+  std::vector<int32_t> rowptr((size_t)nbrows + 1, 0);
+  int64_t nnzb = 0;
+  for (int32_t i = 0; i < nbrows; ++i) { nnzb += nblk[(size_t)i]; rowptr[(size_t)i + 1] = (int32_t)nnzb; }
+  if (nnzb * bs_r * bs_c >= (1LL << 31)) return fail(BSR_ERR_LIMIT, "the assembled matrix has 2^31 or more values");
+  std::vector<int32_t> colidx((size_t)nnzb), segptr((size_t)nnzb + 1);
+  segptr[(size_t)nnzb] = (int32_t)n;
+#pragma omp parallel for schedule(dynamic, 1024)
+  for (int32_t i = 0; i < nbrows; ++i) {
+    int32_t s = rowptr[(size_t)i];
+    for (int64_t p = rstart[(size_t)i]; p < rstart[(size_t)i + 1]; ++p)
+      if (p == rstart[(size_t)i] || bc[(size_t)byrow[(size_t)p]] != bc[(size_t)byrow[(size_t)p - 1]]) {
+        colidx[(size_t)s] = bc[(size_t)byrow[(size_t)p]];
+        segptr[(size_t)s] = (int32_t)p;
+        ++s;
+      }
+  }
+  bcoo_plan_s* pl = new (std::nothrow) bcoo_plan_s();
+  if (!pl) return fail(BSR_ERR_ALLOC, "host allocation failed");
+  pl->n = n; pl->nnzb = nnzb; pl->nbrows = nbrows; pl->nbcols = nbcols; pl->bs_r = bs_r; pl->bs_c = bs_c;
+  int rc = upload(&pl->rowptr, rowptr, st);
+  if (rc == BSR_OK) rc = upload(&pl->colidx, colidx, st);
+  if (rc == BSR_OK) rc = upload(&pl->segptr, segptr, st);
+  if (rc == BSR_OK) rc = upload(&pl->perm, byrow, st);
+  if (rc == BSR_OK && cudaStreamSynchronize(st) != cudaSuccess) rc = fail(BSR_ERR_CUDA, "plan upload failed");
+  if (rc != BSR_OK) { bcoo_release(pl); return rc; }
+  pl->magic = BCOO_MAGIC;
+  if (nnzb_out) *nnzb_out = nnzb;
+  *out = pl;
+  return BSR_OK;
+}
+
+int bcoo_structure(bcoo_plan_t pl, int32_t* d_rowptr, int32_t* d_colidx, void* stream) {
+  if (!pl || pl->magic != BCOO_MAGIC) return fail(BSR_ERR_NULL, "invalid plan handle");
+  if (!d_rowptr || (pl->nnzb && !d_colidx)) return fail(BSR_ERR_NULL, "null output array");
+  cudaStream_t st = (cudaStream_t)stream;
+  CUDA_TRY(cudaMemcpyAsync(d_rowptr, pl->rowptr, ((size_t)pl->nbrows + 1) * 4, cudaMemcpyDeviceToDevice, st));
+  if (pl->nnzb) CUDA_TRY(cudaMemcpyAsync(d_colidx, pl->colidx, (size_t)pl->nnzb * 4, cudaMemcpyDeviceToDevice, st));
+  return BSR_OK;
+}
+
+int bcoo_set_values(bcoo_plan_t pl, const double* d_stream, double* d_vals, void* stream) {
+  if (!pl || pl->magic != BCOO_MAGIC) return fail(BSR_ERR_NULL, "invalid plan handle");
+  if (pl->nnzb == 0) return BSR_OK;
+  if (!d_stream || !d_vals) return fail(BSR_ERR_NULL, "null array");
+  cudaStream_t st = (cudaStream_t)stream;
+  const int bb = pl->bs_r * pl->bs_c;
+  const int64_t nvals = pl->nnzb * bb;
+  const unsigned grid = (unsigned)((nvals + 255) / 256);
+  switch (bb) {
+    case 4: LAUNCH(bcoo_sum_kernel<4>, grid, 256, 0, st, nvals, pl->segptr, pl->perm, d_stream, d_vals); break;
+    case 6: LAUNCH(bcoo_sum_kernel<6>, grid, 256, 0, st, nvals, pl->segptr, pl->perm, d_stream, d_vals); break;
+    case 9: LAUNCH(bcoo_sum_kernel<9>, grid, 256, 0, st, nvals, pl->segptr, pl->perm, d_stream, d_vals); break;
+    case 18: LAUNCH(bcoo_sum_kernel<18>, grid, 256, 0, st, nvals, pl->segptr, pl->perm, d_stream, d_vals); break;
+    case 36: LAUNCH(bcoo_sum_kernel<36>, grid, 256, 0, st, nvals, pl->segptr, pl->perm, d_stream, d_vals); break;
+    default: return fail(BSR_ERR_BLOCK, "unsupported block shape");
+  }
+  return BSR_OK;
+}
+
+int bcoo_get_info(bcoo_plan_t pl, int64_t* n_contrib, int64_t* nnzb, int64_t* algorithmic_bytes) {
+  if (!pl || pl->magic != BCOO_MAGIC) return fail(BSR_ERR_NULL, "invalid plan handle");
+  if (n_contrib) *n_contrib = pl->n;
+  if (nnzb) *nnzb = pl->nnzb;
+  // the value stream read once, the destination values written once, one stream position per contribution and one
+  // segment pointer per destination block
+  if (algorithmic_bytes)
+    *algorithmic_bytes = 8LL * pl->bs_r * pl->bs_c * (pl->n + pl->nnzb) + 4LL * pl->n + 4LL * (pl->nnzb + 1);
+  return BSR_OK;
+}
+
+int bcoo_destroy(bcoo_plan_t pl) {
+  if (!pl) return BSR_OK;
+  if (pl->magic != BCOO_MAGIC) return fail(BSR_ERR_NULL, "invalid plan handle");
+  bcoo_release(pl);
+  return BSR_OK;
+}
+
+int fem_q1_element_coords(int32_t d, int32_t ne, int64_t e0, int64_t e1, int32_t* d_brow, int32_t* d_bcol, void* stream) {
+  if ((d != 2 && d != 3) || ne < 1 || e0 < 0 || e1 < e0) return fail(BSR_ERR_SHAPE, "fem_q1_element_coords: bad argument");
+  const int64_t nel = (d == 3) ? (int64_t)ne * ne * ne : (int64_t)ne * ne;
+  if (e1 > nel) return fail(BSR_ERR_SHAPE, "element range outside the grid");
+  const int64_t nc = (e1 - e0) << (2 * d);
+  if (nc == 0) return BSR_OK;
+  if (!d_brow || !d_bcol) return fail(BSR_ERR_NULL, "null coordinate array");
+  if (nc >= (1LL << 31)) return fail(BSR_ERR_LIMIT, "2^31 or more contributions");
+  LAUNCH(q1_coords_kernel, (unsigned)((nc + 255) / 256), 256, 0, (cudaStream_t)stream, d, ne, e0, nc, d_brow, d_bcol);
+  return BSR_OK;
+}
+
+int fem_q1_element_blocks(int32_t d, int32_t ne, int64_t e0, int64_t e1, const double* d_Ke, const double* d_E,
+                          int32_t dirichlet, double* d_stream, void* stream) {
+  if ((d != 2 && d != 3) || ne < 1 || e0 < 0 || e1 < e0) return fail(BSR_ERR_SHAPE, "fem_q1_element_blocks: bad argument");
+  const int64_t nel = (d == 3) ? (int64_t)ne * ne * ne : (int64_t)ne * ne;
+  if (e1 > nel) return fail(BSR_ERR_SHAPE, "element range outside the grid");
+  const int64_t nv = ((e1 - e0) << (2 * d)) * d * d;
+  if (nv == 0) return BSR_OK;
+  if (!d_Ke || !d_stream) return fail(BSR_ERR_NULL, "null array");
+  const int64_t nblocks = (nv + 255) / 256;
+  if (nblocks >= (1LL << 31)) return fail(BSR_ERR_LIMIT, "stream too long for one launch");
+  LAUNCH(q1_blocks_kernel, (unsigned)nblocks, 256, 0, (cudaStream_t)stream, d, ne, e0, nv, d_Ke, d_E, dirichlet, d_stream);
+  return BSR_OK;
+}
+
+}  // extern "C"

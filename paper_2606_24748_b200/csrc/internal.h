@@ -63,6 +63,9 @@ enum Epilogue { EPI_ASSIGN = 0, /* y = A x */ EPI_RESID = 1, /* y = b - A x */ E
 
 // internal SpMV with epilogue; b only for EPI_RESID
 int spmv_launch(bsr_t A, const double* d_x, double* d_y, const double* d_b, Epilogue epi, cudaStream_t st);
+// dinv[i] = inverse of A's bs x bs diagonal block of row i (point-block Jacobi data); *status |= 1 on a
+// missing or singular block
+int block_diag_inverse(bsr_t A, double* dinv, int* status, cudaStream_t st);
 // makes sure the cached transpose exists and its values are current; hot when nothing changed
 int transpose_ensure(bsr_t A, cudaStream_t st);
 
@@ -83,6 +86,9 @@ struct HostPlan {
   std::vector<int32_t> apstart;  // per R slot t: rowptr_ap[colidx_r[t]]
   int32_t max_k1 = 0, max_q1 = 0, max_t2 = 0, max_s2 = 0;
   std::string err;
+  // stage 1 only (structure and gather lists of A*P): what prolongator smoothing needs (smooth.cu)
+  int build_stage1(int32_t nbrows_a, const int32_t* rowptr_a, const int32_t* colidx_a, int32_t nbcols_p,
+                   const int32_t* rowptr_p, const int32_t* colidx_p);
   // builds everything from the host structures of A, P and R = P^T.  Returns BSR_OK or an error code.
   int build(int32_t nbrows_a, const int32_t* rowptr_a, const int32_t* colidx_a, int32_t nbcols_p,
             const int32_t* rowptr_p, const int32_t* colidx_p, const int32_t* rowptr_r, const int32_t* colidx_r);

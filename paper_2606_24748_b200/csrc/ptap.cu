@@ -130,7 +130,7 @@ static int stream_up(const std::vector<T>& h, const T** d, StreamDev& sd, cudaSt
   return BSR_OK;
 }
 
-int stream_upload(const StreamShape& sh, const StreamPlan& sp, StreamDev& sd, cudaStream_t st) {
+int stream_upload(const StreamShape& sh, const StreamPlan& sp, StreamDev& sd, cudaStream_t st, bool smooth) {
   sd = StreamDev();
   if (!sp.ok) return BSR_OK;
   StreamArgs& a = sd.args;
@@ -141,7 +141,9 @@ int stream_upload(const StreamShape& sh, const StreamPlan& sp, StreamDev& sd, cu
   if (rc == BSR_OK) rc = stream_up(sp.entries, &a.entries, sd, st);
   if (rc == BSR_OK) rc = stream_up(sp.passes, &a.passes, sd, st);
   if (rc == BSR_OK) rc = stream_up(sp.meta, &a.meta, sd, st);
-  if (rc == BSR_OK) rc = stream_launch(sh.M, sh.K, sh.N, a, sp.persist, 0, sp.max_smem, st, true);   // shared-memory opt-in
+  if (rc == BSR_OK)   // shared-memory opt-in of the kernel that will run this plan
+    rc = smooth ? stream_launch_smooth(sh.M, sh.N, a, 0, sp.max_smem, st, true)
+                : stream_launch(sh.M, sh.K, sh.N, a, sp.persist, 0, sp.max_smem, st, true);
   if (rc == BSR_OK && cudaStreamSynchronize(st) != cudaSuccess) rc = fail(BSR_ERR_CUDA, "stream plan upload failed");
   if (rc != BSR_OK) { stream_release(sd); return rc; }
   sd.ok = true; sd.persist = sp.persist; sd.nbricks = sp.nbricks(); sd.smem = sp.max_smem;

@@ -118,9 +118,8 @@ int symbolic_product(int32_t nrows, const int32_t* rowptr_x, const int32_t* coli
 
 }  // namespace
 
-int HostPlan::build(int32_t nbrows_a_, const int32_t* rowptr_a, const int32_t* colidx_a, int32_t nbcols_p_,
-                    const int32_t* rowptr_p, const int32_t* colidx_p, const int32_t* rowptr_r,
-                    const int32_t* colidx_r) {
+int HostPlan::build_stage1(int32_t nbrows_a_, const int32_t* rowptr_a, const int32_t* colidx_a, int32_t nbcols_p_,
+                           const int32_t* rowptr_p, const int32_t* colidx_p) {
   nbrows_a = nbrows_a_;
   nbcols_p = nbcols_p_;
   // stage 1: AP = A * P
@@ -130,6 +129,18 @@ int HostPlan::build(int32_t nbrows_a_, const int32_t* rowptr_a, const int32_t* c
   int rc = symbolic_product(nbrows_a, rowptr_a, colidx_a, rowptr_p, colidx_p, s1, err);
   if (rc != BSR_OK) return rc;
   max_k1 = s1.max_off_x; max_q1 = s1.max_off_y;
+  const int64_t nnzb_a = rowptr_a[nbrows_a];
+  pstart.resize((size_t)nnzb_a);
+#pragma omp parallel for schedule(static)
+  for (int64_t k = 0; k < nnzb_a; ++k) pstart[(size_t)k] = rowptr_p[colidx_a[k]];
+  return BSR_OK;
+}
+
+int HostPlan::build(int32_t nbrows_a_, const int32_t* rowptr_a, const int32_t* colidx_a, int32_t nbcols_p_,
+                    const int32_t* rowptr_p, const int32_t* colidx_p, const int32_t* rowptr_r,
+                    const int32_t* colidx_r) {
+  int rc = build_stage1(nbrows_a_, rowptr_a, colidx_a, nbcols_p_, rowptr_p, colidx_p);
+  if (rc != BSR_OK) return rc;
   // stage 2: A_c = R * AP
   Product st2;
   st2.rowptr_c = &rowptr_c; st2.colidx_c = &colidx_c; st2.rowidx_c = &rowidx_c; st2.pairptr = &pairptr2;
@@ -138,11 +149,8 @@ int HostPlan::build(int32_t nbrows_a_, const int32_t* rowptr_a, const int32_t* c
   if (rc != BSR_OK) return rc;
   max_t2 = st2.max_off_x; max_s2 = st2.max_off_y;
   // row starts of the gathered operand, one per slot of the left operand (saves one indirection in the kernels)
-  const int64_t nnzb_a = rowptr_a[nbrows_a], nnzb_r = rowptr_r[nbcols_p];
-  pstart.resize((size_t)nnzb_a);
+  const int64_t nnzb_r = rowptr_r[nbcols_p];
   apstart.resize((size_t)nnzb_r);
-#pragma omp parallel for schedule(static)
-  for (int64_t k = 0; k < nnzb_a; ++k) pstart[(size_t)k] = rowptr_p[colidx_a[k]];
 #pragma omp parallel for schedule(static)
   for (int64_t t = 0; t < nnzb_r; ++t) apstart[(size_t)t] = rowptr_ap[(size_t)colidx_r[t]];
   return BSR_OK;

@@ -77,9 +77,10 @@ __device__ __forceinline__ void lds_block(const double* __restrict__ p, double (
   }
 }
 
-template <int M, int K, int N, int NT, bool PERSIST>
+template <int M, int K, int N, int NT, bool PERSIST, int EPI = 0>
 __global__ void __launch_bounds__(NT, PERSIST ? 3 : STREAM_MINB1)
 stream_product_kernel(const StreamArgs a) {
+  static_assert(EPI == 0 || (!PERSIST && M == K), "the smoothing epilogue belongs to the direct A*P~ product");
   constexpr int MK = M * K, KN = K * N, MN = M * N, XS = (MK + 1) & ~1, NW = NT / 32;
   extern __shared__ __align__(16) unsigned char smem[];
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -209,6 +210,26 @@ stream_product_kernel(const StreamArgs a) {
         }
       }
       if (!PERSIST && slot >= 0) {
+        if (EPI == 1) {
+          // P(i,J) = P~(i,J) - omega * D_i^-1 * (A P~)(i,J)   (the block AXPY on the subset
+          // pattern of PAPER.md:244 fused into the store of the product)
+          const int64_t o = (int64_t)out + slot;
+          const int32_t row = __ldg(a.out_row + o), own = __ldg(a.own_slot + o);
+          const double* di = a.dinv + (int64_t)row * M * M;
+          double z[MN];
+#pragma unroll
+          for (int r = 0; r < M; ++r)
+#pragma unroll
+            for (int c = 0; c < N; ++c) {
+              double t = 0.0;
+#pragma unroll
+              for (int m = 0; m < M; ++m) t = fma(__ldg(di + r * M + m), acc[m * N + c], t);
+              z[r * N + c] = t;
+            }
+#pragma unroll
+          for (int e = 0; e < MN; ++e)
+            acc[e] = fma(-a.omega, z[e], own >= 0 ? __ldg(a.own_vals + (int64_t)own * MN + e) : 0.0);
+        }
         double* dst = a.cvals + (int64_t)(out + slot) * MN;
         if (MN % 2 == 0) {
 #pragma unroll
@@ -263,6 +284,29 @@ static int stream_launch_mkn(const StreamArgs& a, bool persist, int64_t nbricks,
     LAUNCH(kern, (unsigned)nbricks, STREAM_THREADS_DIRECT, (size_t)smem, st, a);
   }
   return BSR_OK;
+}
+
+template <int M, int N>
+static int stream_launch_smooth_mn(const StreamArgs& a, int64_t nbricks, int64_t smem, cudaStream_t st, bool prepare) {
+  auto kern = stream_product_kernel<M, M, N, STREAM_THREADS_DIRECT, false, 1>;
+  if (prepare) {
+    CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    return BSR_OK;
+  }
+  if (nbricks == 0) return BSR_OK;
+  LAUNCH(kern, (unsigned)nbricks, STREAM_THREADS_DIRECT, (size_t)smem, st, a);
+  return BSR_OK;
+}
+
+int stream_launch_smooth(int M, int N, const StreamArgs& a, int64_t nbricks, int64_t smem, cudaStream_t st,
+                         bool prepare) {
+  switch (M * 10 + N) {
+    case 23: return stream_launch_smooth_mn<2, 3>(a, nbricks, smem, st, prepare);
+    case 33: return stream_launch_smooth_mn<3, 3>(a, nbricks, smem, st, prepare);
+    case 36: return stream_launch_smooth_mn<3, 6>(a, nbricks, smem, st, prepare);
+    case 66: return stream_launch_smooth_mn<6, 6>(a, nbricks, smem, st, prepare);
+  }
+  return fail(BSR_ERR_BLOCK, "no staged smoothing kernel for <%d,%d,%d>", M, M, N);
 }
 
 int stream_launch(int M, int K, int N, const StreamArgs& a, bool persist, int64_t nbricks, int64_t smem, cudaStream_t st,

@@ -19,6 +19,12 @@ struct StreamArgs {  // all device pointers
   const StreamMeta* meta;
   const double *xvals, *yvals;
   double* cvals;
+  // store epilogue of prolongator smoothing (smooth.cu; direct bricks only): C(row,J) = own(row,J) - omega * D_row^-1 * acc
+  const double* dinv = nullptr;       // M x M per X row
+  const double* own_vals = nullptr;   // blocks of the tentative prolongator
+  const int32_t* out_row = nullptr;   // per output slot: its row
+  const int32_t* own_slot = nullptr;  // per output slot: the tentative block with the same coordinate, or -1
+  double omega = 0.0;
 };
 
 // device copy of a StreamPlan
@@ -29,10 +35,13 @@ struct StreamDev {
   std::vector<void*> owned;
 };
 
-int stream_upload(const StreamShape& sh, const StreamPlan& sp, StreamDev& sd, cudaStream_t st);
+int stream_upload(const StreamShape& sh, const StreamPlan& sp, StreamDev& sd, cudaStream_t st, bool smooth = false);
 void stream_release(StreamDev& sd);
 // prepare = true: cold call that sets the kernel's dynamic shared memory attribute on the current device
 int stream_launch(int M, int K, int N, const StreamArgs& a, bool persist, int64_t nbricks, int64_t smem, cudaStream_t st,
                   bool prepare = false);
+// the direct kernel with the smoothing epilogue (shapes <2,2,3>, <3,3,3>, <3,3,6>, <6,6,6>)
+int stream_launch_smooth(int M, int N, const StreamArgs& a, int64_t nbricks, int64_t smem, cudaStream_t st,
+                         bool prepare = false);
 
 }  // namespace bsramg

@@ -1,0 +1,243 @@
+// smooth.cu -- device prolongator smoothing P = (I - omega D^-1 A) P~ in blocks.
+//
+// "The tentative prolongator is improved by one step of a damped-Jacobi prolongator smoother,
+// P = (I - omega D^-1 A) P~" (D the bs x bs block diagonal, reading R11).  PAPER.md:244: the cold setup is
+// "dominated by symbolic coarsening and prolongator smoothing"; the smoother's MatAYPX with SUBSET_NONZERO_PATTERN
+// "runs natively in blocks: the diagonal block is added directly ... adds block-for-block on device".
+//
+// Here the whole update is one pass over A: the pattern of P is the boolean pattern of A*P~ (cold, host,
+// HostPlan::build_stage1 -- the same symbolic product ptap_symbolic uses for AP), the numeric phase is the staged
+// <bf,bf,bc> product kernel of ptap_stream.cu with the update fused into its store:
+//     P(i,J) = P~(i,J) [if stored] - omega * D_i^-1 * sum_j A(i,j) P~(j,J)
+// so A*P~ is never written to memory and the block AXPY costs no extra pass.  D^-1 comes from the same block
+// inversion kernel the V-cycle's point-block Jacobi uses.  A matrix outside the staged format runs a one-thread-per-
+// output-block gather kernel with the same epilogue.  No atomics; fixed summation order.
+#include <algorithm>
+
+#include "internal.h"
+#include "ptap_stream.h"
+
+struct psmooth_plan_s {
+  uint64_t magic = 0;
+  bsr_t A = nullptr, Pt = nullptr;
+  int64_t nnzb_a = 0, nnzb_pt = 0, nnzb_p = 0, nprod = 0;
+  int32_t bf = 0, bc = 0, nbrows = 0, nbcols = 0;
+  int32_t *rowptr_p = nullptr, *colidx_p = nullptr, *out_row = nullptr, *own_slot = nullptr;
+  int32_t *pairptr = nullptr, *pstart = nullptr;   // gather fallback only
+  void* pairs = nullptr;
+  double* dinv = nullptr;
+  int* status = nullptr;
+  bsramg::StreamDev s1;
+};
+static const uint64_t PSM_MAGIC = 0x50534d4f4f544831ull;
+
+namespace bsramg {
+
+// gather fallback: one thread per output block, products in the plan's order, same epilogue as the staged kernel
+template <int M, int N>
+__global__ void __launch_bounds__(128)
+smooth_gather_kernel(int32_t nout, const int32_t* __restrict__ out_row, const int32_t* __restrict__ own_slot,
+                     const int32_t* __restrict__ rowptr_a, const int32_t* __restrict__ pstart,
+                     const int32_t* __restrict__ pairptr, const uint32_t* __restrict__ pairs,
+                     const double* __restrict__ avals, const double* __restrict__ tvals,
+                     const double* __restrict__ dinv, double omega, double* __restrict__ pvals) {
+  const int32_t u = blockIdx.x * blockDim.x + threadIdx.x;
+  if (u >= nout) return;
+  const int32_t row = __ldg(out_row + u);
+  const int32_t x0 = __ldg(rowptr_a + row);
+  double acc[M * N];
+#pragma unroll
+  for (int e = 0; e < M * N; ++e) acc[e] = 0.0;
+  for (int32_t p = __ldg(pairptr + u); p < __ldg(pairptr + u + 1); ++p) {
+    const uint32_t code = __ldg(pairs + p);
+    const int32_t xs = x0 + (int32_t)(code & 0xffffu);
+    const int32_t ys = __ldg(pstart + xs) + (int32_t)(code >> 16);
+    const double* xb = avals + (int64_t)xs * M * M;
+    const double* yb = tvals + (int64_t)ys * M * N;
+#pragma unroll
+    for (int r = 0; r < M; ++r)
+#pragma unroll
+      for (int m = 0; m < M; ++m) {
+        const double xv = __ldg(xb + r * M + m);
+#pragma unroll
+        for (int c = 0; c < N; ++c) acc[r * N + c] = fma(xv, __ldg(yb + m * N + c), acc[r * N + c]);
+      }
+  }
+  const double* di = dinv + (int64_t)row * M * M;
+  const int32_t own = __ldg(own_slot + u);
+  double* dst = pvals + (int64_t)u * M * N;
+#pragma unroll
+  for (int r = 0; r < M; ++r)
+#pragma unroll
+    for (int c = 0; c < N; ++c) {
+      double t = 0.0;
+#pragma unroll
+      for (int m = 0; m < M; ++m) t = fma(__ldg(di + r * M + m), acc[m * N + c], t);
+      dst[r * N + c] = fma(-omega, t, own >= 0 ? __ldg(tvals + (int64_t)own * M * N + r * N + c) : 0.0);
+    }
+}
+
+template <int M, int N>
+static int smooth_gather_launch(psmooth_plan_s* pl, double omega, double* d_vals_p, cudaStream_t st) {
+  if (pl->nnzb_p == 0) return BSR_OK;
+  const unsigned grid = (unsigned)((pl->nnzb_p + 127) / 128);
+  LAUNCH((smooth_gather_kernel<M, N>), grid, 128, 0, st, (int32_t)pl->nnzb_p, pl->out_row, pl->own_slot,
+         pl->A->d_rowptr, pl->pstart, pl->pairptr, (const uint32_t*)pl->pairs, pl->A->d_vals, pl->Pt->d_vals, pl->dinv,
+         omega, d_vals_p);
+  return BSR_OK;
+}
+
+static void psmooth_release(psmooth_plan_s* pl) {
+  if (!pl) return;
+  dev_free(pl->rowptr_p); dev_free(pl->colidx_p); dev_free(pl->out_row); dev_free(pl->own_slot);
+  dev_free(pl->pairptr); dev_free(pl->pstart); dev_free(pl->pairs); dev_free(pl->dinv); dev_free(pl->status);
+  stream_release(pl->s1);
+  pl->magic = 0;
+  delete pl;
+}
+
+static bool smooth_shape(int bf, int bc) {
+  return (bf == 2 && bc == 3) || (bf == 3 && bc == 3) || (bf == 3 && bc == 6) || (bf == 6 && bc == 6);
+}
+
+}  // namespace bsramg
+
+using namespace bsramg;
+
+extern "C" {
+
+int prolongator_smooth_symbolic(psmooth_plan_t* out, bsr_t A, bsr_t Pt, int64_t* nnzb_p, void* stream) {
+  if (!out) return fail(BSR_ERR_NULL, "prolongator_smooth_symbolic: out is null");
+  *out = nullptr;
+  if (!A || !Pt || A->magic != BSR_MAGIC || Pt->magic != BSR_MAGIC) return fail(BSR_ERR_NULL, "invalid matrix handle");
+  if (A->nbrows != A->nbcols || A->bs_r != A->bs_c) return fail(BSR_ERR_SHAPE, "A must be square with square blocks");
+  if (A->nbcols != Pt->nbrows || A->bs_c != Pt->bs_r)
+    return fail(BSR_ERR_SHAPE, "A (%d block cols, bs %d) does not match P~ (%d block rows, bs_r %d)", A->nbcols,
+                A->bs_c, Pt->nbrows, Pt->bs_r);
+  if (!smooth_shape(A->bs_r, Pt->bs_c)) return fail(BSR_ERR_BLOCK, "unsupported block shapes in prolongator smoothing");
+  cudaStream_t st = (cudaStream_t)stream;
+  HostPlan hp;
+  int rc = hp.build_stage1(A->nbrows, A->h_rowptr.data(), A->h_colidx.data(), Pt->nbcols, Pt->h_rowptr.data(),
+                           Pt->h_colidx.data());
+  if (rc != BSR_OK) return fail(rc, "prolongator_smooth_symbolic: %s", hp.err.c_str());
+  const int64_t np = (int64_t)hp.colidx_ap.size();
+  if (np * A->bs_r * Pt->bs_c >= (1LL << 31)) return fail(BSR_ERR_LIMIT, "P has 2^31 or more values");
+  // own_slot: the tentative block with the same coordinate (the SUBSET pattern of the block AXPY)
+  std::vector<int32_t> own((size_t)np, -1);
+  int bad = 0;
+#pragma omp parallel for schedule(static) reduction(| : bad)
+  for (int32_t i = 0; i < A->nbrows; ++i) {
+    const int32_t* lo = hp.colidx_ap.data() + hp.rowptr_ap[i];
+    const int32_t* hi = hp.colidx_ap.data() + hp.rowptr_ap[i + 1];
+    for (int32_t q = Pt->h_rowptr[i]; q < Pt->h_rowptr[i + 1]; ++q) {
+      const int32_t* it = std::lower_bound(lo, hi, Pt->h_colidx[q]);
+      if (it == hi || *it != Pt->h_colidx[q]) bad |= 1;   // A has no diagonal block in row i
+      else own[(size_t)(it - hp.colidx_ap.data())] = q;
+    }
+  }
+  if (bad) return fail(BSR_ERR_STRUCTURE, "a block of P~ lies outside the pattern of A*P~ (A lacks a diagonal block)");
+  psmooth_plan_s* pl = new (std::nothrow) psmooth_plan_s();
+  if (!pl) return fail(BSR_ERR_ALLOC, "host allocation failed");
+  pl->A = A; pl->Pt = Pt; pl->nnzb_a = A->nnzb; pl->nnzb_pt = Pt->nnzb; pl->nnzb_p = np;
+  pl->nprod = (int64_t)hp.k1.size();
+  pl->bf = A->bs_r; pl->bc = Pt->bs_c; pl->nbrows = A->nbrows; pl->nbcols = Pt->nbcols;
+  rc = upload(&pl->rowptr_p, hp.rowptr_ap, st);
+  if (rc == BSR_OK) rc = upload(&pl->colidx_p, hp.colidx_ap, st);
+  if (rc == BSR_OK) rc = upload(&pl->out_row, hp.rowidx_ap, st);
+  if (rc == BSR_OK) rc = upload(&pl->own_slot, own, st);
+  if (rc == BSR_OK) rc = dev_alloc_t(&pl->dinv, (size_t)A->nbrows * A->bs_r * A->bs_r);
+  if (rc == BSR_OK) rc = dev_alloc_t(&pl->status, 1);
+  if (rc == BSR_OK && cudaMemsetAsync(pl->status, 0, sizeof(int), st) != cudaSuccess) rc = fail(BSR_ERR_CUDA, "memset failed");
+  const Options opt = options();
+  if (rc == BSR_OK && !opt.force_gather) {
+    std::vector<StreamBrickDef> bricks;
+    StreamPlan sp;
+    const StreamShape sh{pl->bf, pl->bf, pl->bc};
+    stream_bricks_stage1(hp, sh, opt.smem_stage1, A->h_rowptr.data(), A->h_colidx.data(), Pt->h_rowptr.data(), bricks);
+    stream_build(sh, STREAM_THREADS_DIRECT / 32, opt.smem_stage1, bricks, A->h_rowptr.data(), A->h_colidx.data(),
+                 Pt->h_rowptr.data(), hp.rowptr_ap.data(), hp.pairptr1.data(), hp.k1.data(), hp.q1.data(), sp);
+    rc = stream_upload(sh, sp, pl->s1, st, /*smooth=*/true);
+  }
+  if (rc == BSR_OK && !pl->s1.ok) {
+    std::vector<uint32_t> packed(hp.k1.size());
+#pragma omp parallel for schedule(static)
+    for (int64_t p = 0; p < (int64_t)packed.size(); ++p) packed[(size_t)p] = hp.k1[(size_t)p] | ((uint32_t)hp.q1[(size_t)p] << 16);
+    uint32_t* dp = nullptr;
+    rc = upload(&pl->pairptr, hp.pairptr1, st);
+    if (rc == BSR_OK) rc = upload(&pl->pstart, hp.pstart, st);
+    if (rc == BSR_OK) rc = upload(&dp, packed, st);
+    pl->pairs = dp;
+    if (rc == BSR_OK && cudaStreamSynchronize(st) != cudaSuccess) rc = fail(BSR_ERR_CUDA, "plan upload failed");
+  }
+  if (rc == BSR_OK && cudaStreamSynchronize(st) != cudaSuccess) rc = fail(BSR_ERR_CUDA, "plan upload failed");
+  if (rc != BSR_OK) { psmooth_release(pl); return rc; }
+  pl->magic = PSM_MAGIC;
+  if (nnzb_p) *nnzb_p = np;
+  *out = pl;
+  return BSR_OK;
+}
+
+int prolongator_smooth_structure(psmooth_plan_t pl, int32_t* d_rowptr_p, int32_t* d_colidx_p, void* stream) {
+  if (!pl || pl->magic != PSM_MAGIC) return fail(BSR_ERR_NULL, "invalid plan handle");
+  if (!d_rowptr_p || (pl->nnzb_p && !d_colidx_p)) return fail(BSR_ERR_NULL, "null output array");
+  cudaStream_t st = (cudaStream_t)stream;
+  CUDA_TRY(cudaMemcpyAsync(d_rowptr_p, pl->rowptr_p, ((size_t)pl->nbrows + 1) * 4, cudaMemcpyDeviceToDevice, st));
+  if (pl->nnzb_p)
+    CUDA_TRY(cudaMemcpyAsync(d_colidx_p, pl->colidx_p, (size_t)pl->nnzb_p * 4, cudaMemcpyDeviceToDevice, st));
+  return BSR_OK;
+}
+
+int prolongator_smooth_numeric(psmooth_plan_t pl, bsr_t A, bsr_t Pt, double omega, double* d_vals_p, void* stream) {
+  if (!pl || pl->magic != PSM_MAGIC) return fail(BSR_ERR_NULL, "invalid plan handle");
+  if (!A || !Pt || A->magic != BSR_MAGIC || Pt->magic != BSR_MAGIC) return fail(BSR_ERR_NULL, "invalid matrix handle");
+  if (A != pl->A || Pt != pl->Pt || A->nnzb != pl->nnzb_a || Pt->nnzb != pl->nnzb_pt)
+    return fail(BSR_ERR_PLAN, "plan was built from different matrices");
+  if (!d_vals_p && pl->nnzb_p) return fail(BSR_ERR_NULL, "d_vals_p is null");
+  if ((uintptr_t)d_vals_p & 15) return fail(BSR_ERR_ALIGN, "d_vals_p must be 16-byte aligned");
+  cudaStream_t st = (cudaStream_t)stream;
+  BSR_TRY(block_diag_inverse(A, pl->dinv, pl->status, st));
+  if (pl->s1.ok) {
+    StreamArgs a = pl->s1.args;
+    a.xvals = A->d_vals; a.yvals = Pt->d_vals; a.cvals = d_vals_p;
+    a.dinv = pl->dinv; a.own_vals = Pt->d_vals; a.out_row = pl->out_row; a.own_slot = pl->own_slot; a.omega = omega;
+    return stream_launch_smooth(pl->bf, pl->bc, a, pl->s1.nbricks, pl->s1.smem, st);
+  }
+  switch (pl->bf * 10 + pl->bc) {
+    case 23: return smooth_gather_launch<2, 3>(pl, omega, d_vals_p, st);
+    case 33: return smooth_gather_launch<3, 3>(pl, omega, d_vals_p, st);
+    case 36: return smooth_gather_launch<3, 6>(pl, omega, d_vals_p, st);
+    case 66: return smooth_gather_launch<6, 6>(pl, omega, d_vals_p, st);
+  }
+  return fail(BSR_ERR_BLOCK, "unsupported block shapes in prolongator smoothing");
+}
+
+int prolongator_smooth_status(psmooth_plan_t pl, void* stream) {
+  if (!pl || pl->magic != PSM_MAGIC) return fail(BSR_ERR_NULL, "invalid plan handle");
+  cudaStream_t st = (cudaStream_t)stream;
+  int h = 0;
+  CUDA_TRY(cudaMemcpyAsync(&h, pl->status, sizeof(int), cudaMemcpyDeviceToHost, st));
+  CUDA_TRY(cudaStreamSynchronize(st));
+  if (h) return fail(BSR_ERR_NUMERIC, "singular or missing diagonal block in prolongator smoothing");
+  return BSR_OK;
+}
+
+int prolongator_smooth_get_info(psmooth_plan_t pl, int64_t* n_products, int64_t* algorithmic_bytes, int32_t* staged) {
+  if (!pl || pl->magic != PSM_MAGIC) return fail(BSR_ERR_NULL, "invalid plan handle");
+  if (n_products) *n_products = pl->nprod;
+  if (algorithmic_bytes) {
+    auto bytes = [](int64_t nnzb, int br, int bc, int64_t nbrows) { return nnzb * (8LL * br * bc + 4) + 4LL * (nbrows + 1); };
+    *algorithmic_bytes = bytes(pl->nnzb_a, pl->bf, pl->bf, pl->nbrows) + bytes(pl->nnzb_pt, pl->bf, pl->bc, pl->nbrows) +
+                         bytes(pl->nnzb_p, pl->bf, pl->bc, pl->nbrows);
+  }
+  if (staged) *staged = pl->s1.ok ? 1 : 0;
+  return BSR_OK;
+}
+
+int prolongator_smooth_destroy(psmooth_plan_t pl) {
+  if (!pl) return BSR_OK;
+  if (pl->magic != PSM_MAGIC) return fail(BSR_ERR_NULL, "invalid plan handle");
+  psmooth_release(pl);
+  return BSR_OK;
+}
+
+}  // extern "C"

@@ -113,18 +113,19 @@ cheb_update_kernel(int64_t n, const double* __restrict__ dinv, const double* __r
   x[e] = x_zero ? dn : x[e] + dn;
 }
 
-static int launch_dinv(Level& lv, int* status, cudaStream_t st) {
-  bsr_t A = lv.A;
+int block_diag_inverse(bsr_t A, double* dinv, int* status, cudaStream_t st) {
   const unsigned grid = (unsigned)((A->nbrows + 127) / 128);
   if (!grid) return BSR_OK;
-  switch (lv.bs) {
-    case 2: LAUNCH(dinv_kernel<2>, grid, 128, 0, st, A->nbrows, A->d_rowptr, A->d_colidx, A->d_vals, lv.Dinv, status); break;
-    case 3: LAUNCH(dinv_kernel<3>, grid, 128, 0, st, A->nbrows, A->d_rowptr, A->d_colidx, A->d_vals, lv.Dinv, status); break;
-    case 6: LAUNCH(dinv_kernel<6>, grid, 128, 0, st, A->nbrows, A->d_rowptr, A->d_colidx, A->d_vals, lv.Dinv, status); break;
-    default: return fail(BSR_ERR_BLOCK, "unsupported block size %d", lv.bs);
+  switch (A->bs_r) {
+    case 2: LAUNCH(dinv_kernel<2>, grid, 128, 0, st, A->nbrows, A->d_rowptr, A->d_colidx, A->d_vals, dinv, status); break;
+    case 3: LAUNCH(dinv_kernel<3>, grid, 128, 0, st, A->nbrows, A->d_rowptr, A->d_colidx, A->d_vals, dinv, status); break;
+    case 6: LAUNCH(dinv_kernel<6>, grid, 128, 0, st, A->nbrows, A->d_rowptr, A->d_colidx, A->d_vals, dinv, status); break;
+    default: return fail(BSR_ERR_BLOCK, "unsupported block size %d", A->bs_r);
   }
   return BSR_OK;
 }
+
+static int launch_dinv(Level& lv, int* status, cudaStream_t st) { return block_diag_inverse(lv.A, lv.Dinv, status, st); }
 
 static int launch_cheb(Level& lv, double* x, int first, double theta, double cd, double cz, int x_zero,
                        cudaStream_t st) {
