@@ -44,6 +44,22 @@ def measured_peak():
         return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md)"
 
 
+def read_traffic() -> dict:
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of each kernel, from the committed ncu --set full
+    capture: profiles/ncu_traffic.csv is written by `python -m paper_2606_24748_b200.ncu_summary` (profiles/ncu_traffic.md
+    names the commands)."""
+    out = {}
+    tp = os.path.join(ROOT, "profiles", "ncu_traffic.csv")
+    try:
+        for ln in open(tp).read().splitlines()[1:]:
+            f = [t.strip() for t in ln.split(",")]
+            if len(f) >= 2 and f[1]:
+                out[f[0]] = int(float(f[1]))
+    except Exception:
+        pass
+    return out
+
+
 def bsr_bytes(M) -> int:
     return M.nnzb * (8 * M.bs_r * M.bs_c + 4) + 4 * (M.nbrows + 1)
 
@@ -236,8 +252,14 @@ def run_ours(args) -> dict | None:
     nbytes_k = {"ptap_stage1_AP": bsr_bytes(A) + bsr_bytes(P) + bAP, "ptap_stage2_RAP": bsr_bytes(Rshape) + bAP + bAc}
     total_bytes = sum(nbytes.values())
     names = ["spmv_A", "spmv_P", "spmv_Pt", "ptap_stage1_AP", "ptap_stage2_RAP"]
+    # the operator changes between repetitions ("for PtAP change A's values between repetitions"):
+    # two device value buffers, A_0 and 1.25 A_0, rebound alternately (bsr_rebind_values bumps the state counter)
+    a_bufs = [GA.vals, GA.vals * 1.25]
+    step_no = [0]
 
     def step(ev=None):
+        GA.rebind_values(a_bufs[step_no[0] & 1])
+        step_no[0] += 1
         if ev: ev[0].record()
         GA.spmv(x, y)
         if ev: ev[1].record()
@@ -272,8 +294,9 @@ def run_ours(args) -> dict | None:
     l1, a1 = bsr.counters()
     clocks = sampler.stop()
     ms_total = t_start.elapsed_time(t_end)
-    per = {n: float(np.mean([evs[k][i].elapsed_time(evs[k][i + 1]) for k in range(args.steps)]))
-           for i, n in enumerate(names)}
+    samples = {n: [evs[k][i].elapsed_time(evs[k][i + 1]) for k in range(args.steps)] for i, n in enumerate(names)}
+    per = {n: float(np.median(v)) for n, v in samples.items()}          # median over the timed steps
+    per_min = {n: float(np.min(v)) for n, v in samples.items()}
     ms_total = max_over_ranks(ms_total, world, dev)
     ms_step = ms_total / args.steps
     value = job_value(total_bytes, world, ms_step * 1e-3)
@@ -313,34 +336,37 @@ def run_ours(args) -> dict | None:
     ops = {}
     for n in ["spmv_A", "spmv_P", "spmv_Pt"]:
         gbs = nbytes[n] / (per[n] * 1e-3) / 1e9
-        ops[n] = {"ms": per[n], "GB/s": gbs, "algorithmic_GB": nbytes[n] / 1e9, "frac_of_measured_hbm": gbs / peak,
-                  "frac_of_nominal_8TBs": gbs / NOMINAL_HBM_GBS}
+        ops[n] = {"ms": per[n], "ms_min": per_min[n], "GB/s": gbs, "algorithmic_GB": nbytes[n] / 1e9,
+                  "frac_of_measured_hbm": gbs / peak, "frac_of_nominal_8TBs": gbs / NOMINAL_HBM_GBS}
     ptap_ms = per["ptap_stage1_AP"] + per["ptap_stage2_RAP"]
     gbs = nbytes["ptap"] / (ptap_ms * 1e-3) / 1e9
     ops["ptap_numeric"] = {"ms": ptap_ms, "GB/s": gbs, "algorithmic_GB": nbytes["ptap"] / 1e9,
                            "frac_of_measured_hbm": gbs / peak, "frac_of_nominal_8TBs": gbs / NOMINAL_HBM_GBS,
                            "stage1_ms": per["ptap_stage1_AP"], "stage2_ms": per["ptap_stage2_RAP"],
+                           "ms_min": per_min["ptap_stage1_AP"] + per_min["ptap_stage2_RAP"],
+                           "a_values": "alternate between A_0 and 1.25 A_0 every step (bsr_rebind_values)",
                            "GFLOP": 2.0 * (info["n_products_1"] * A.bs_r * A.bs_r * P.bs_c +
                                            info["n_products_2"] * P.bs_c * A.bs_r * P.bs_c) / 1e9}
     ops["ptap_numeric"]["fp64_TFLOPs"] = ops["ptap_numeric"]["GFLOP"] / ptap_ms
     kb = dict(nbytes); kb.update(nbytes_k)
     dom = max(names, key=lambda n: per[n])
     ach = kb[dom] / (per[dom] * 1e-3) / 1e9
-    traffic = None
-    tp = os.path.join(ROOT, "profiles", "ncu_traffic.csv")  # copied by hand from the ncu --set full capture
-    if os.path.exists(tp):
-        try:
-            for ln in open(tp).read().splitlines()[1:]:
-                k, v = ln.split(",")
-                if k.strip() == dom:
-                    traffic = int(v)
-        except Exception:
-            traffic = None
+    traffic_all = read_traffic()   # profiles/ncu_traffic.csv, written by paper_2606_24748_b200/ncu_summary.py
+    traffic = traffic_all.get(dom)
+    # the ALU roof beside the HBM roof: fp64 FMA peak measured on this device by the library
+    fp64_peak = bsr.fp64_peak_tflops()
+    flops_k = {"ptap_stage1_AP": 2.0 * info["n_products_1"] * A.bs_r * A.bs_r * P.bs_c,
+               "ptap_stage2_RAP": 2.0 * info["n_products_2"] * P.bs_c * A.bs_r * P.bs_c}
+    alu = {n: {"achieved_tflops": f / (per[n] * 1e-3) / 1e12, "peak": fp64_peak,
+               "frac": f / (per[n] * 1e-3) / 1e12 / fp64_peak} for n, f in flops_k.items()}
     roofline = {"bound": "hbm", "kernel": dom, "achieved": ach, "peak": peak, "peak_source": peak_src, "unit": "GB/s",
                 "frac": ach / peak, "traffic": traffic, "algorithmic_bytes_per_launch": kb[dom],
                 "ms_per_launch": per[dom], "share_of_step": per[dom] / sum(per.values()),
-                "all_kernels": {n: {"ms": per[n], "GB/s": kb[n] / (per[n] * 1e-3) / 1e9,
-                                    "frac": kb[n] / (per[n] * 1e-3) / 1e9 / peak} for n in names}}
+                "alu": dict(alu.get(dom, {}), unit="TFLOP/s", peak_source="bsr_measure_fp64_peak (this run)",
+                            all_kernels=alu),
+                "all_kernels": {n: {"ms": per[n], "ms_min": per_min[n], "GB/s": kb[n] / (per[n] * 1e-3) / 1e9,
+                                    "frac": kb[n] / (per[n] * 1e-3) / 1e9 / peak, "traffic": traffic_all.get(n)}
+                                for n in names}}
     out = {"metric": METRIC, "value": value, "unit": "GB/s", "n_gpus": world, "steps": args.steps,
            "warmup": max(args.warmup, 3), "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak",
            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
@@ -351,19 +377,87 @@ def run_ours(args) -> dict | None:
            "e2e": {"value": e2e_val, "unit": "GB/s", "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                    "ms_per_step": e2e_s / e2e_steps * 1e3, "steps": e2e_steps},
            "gpu_launches": int(l1 - l0), "allocs_in_timed_region": int(a1 - a0)}
+    if not args.no_next_rows:
+        out["next_rows"] = run_next_rows(gen, A, GA, peak)
     if not args.no_vcycle:
         # release the config-3 device arrays first (config 4 is a second, smaller problem)
-        del plan, GA, GP, x, xc, y, yc, vals_c
+        del plan, GA, GP, x, xc, y, yc, vals_c, a_bufs
         torch.cuda.empty_cache()
         out["vcycle"] = run_vcycle(peak)
     if not args.no_cpu_baseline:
+        from oracle import oracle as orc
         op = OraclePass(A, P, seed)
         t = op.run()
-        out["cpu_baseline"] = {"value": op.total_bytes / t["total"] / 1e9, "unit": "GB/s", "cores": omp_threads(),
+        ncores = orc.set_threads(0)
+        out["cpu_baseline"] = {"value": op.total_bytes / t["total"] / 1e9, "unit": "GB/s", "cores": ncores,
                                "kind": "oracle", "sample": "one full pass of the same workload (all four operations)",
                                "seconds": {k: round(v, 4) for k, v in t.items()}}
+        orc.set_threads(1)                                          # once with 1 thread as well
+        t1 = op.run()
+        orc.set_threads(0)
+        out["cpu_baseline"]["one_thread"] = {"value": op.total_bytes / t1["total"] / 1e9, "unit": "GB/s", "cores": 1,
+                                             "seconds": {k: round(v, 4) for k, v in t1.items()}}
     if world > 1:
         dist.destroy_process_group()
+    return out
+
+
+def run_next_rows(gen, A, GA, peak: float, reps: int = 10) -> dict:
+    """SURVEY.md 8(f) rows f1 and f2 at the same config-3 grid: device prolongator smoothing (one pass over A) and
+    the blocked COO assembly of A from 134 M finite-element block contributions; median ms of `reps`, GB/s over the
+    algorithmic bytes the library reports, fraction of the measured HBM peak."""
+    import torch
+    from paper_2606_24748_b200 import bsr
+
+    def timed(fn):
+        for _ in range(3):
+            fn()
+        evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(reps)]
+        torch.cuda.synchronize()
+        for e0, e1 in evs:
+            e0.record(); fn(); e1.record()
+        torch.cuda.synchronize()
+        t = [e0.elapsed_time(e1) for e0, e1 in evs]
+        return float(np.median(t)), float(np.min(t))
+
+    def row(ms, ms_min, nbytes, **kw):
+        gbs = nbytes / (ms * 1e-3) / 1e9
+        return dict(ms=ms, ms_min=ms_min, algorithmic_GB=nbytes / 1e9, **{"GB/s": gbs}, frac_of_measured_hbm=gbs / peak,
+                    frac_of_nominal_8TBs=gbs / NOMINAL_HBM_GBS, **kw)
+
+    out = {}
+    Pt = gen.P_tent(0)
+    GT = bsr.Bsr.from_host(Pt, GA.vals.device)
+    t0 = time.perf_counter()
+    sm = bsr.ProlongatorSmoother(GA, GT)
+    cold = time.perf_counter() - t0
+    vals_p = sm.new_values()
+    omega = gen.level_info(0)["omega"]
+    ms, mn = timed(lambda: sm.numeric(omega, vals_p))
+    inf = sm.info()
+    out["prolongator_smooth"] = row(ms, mn, inf["algorithmic_bytes"], symbolic_s=cold, staged=inf["staged"],
+                                    n_products=inf["n_products"], launches_per_call=2)
+    del sm, GT, vals_p
+    d, ne = gen.d, gen.ne
+    E, Ke = gen.element_data()
+    dev = GA.vals.device
+    dKe = torch.from_numpy(Ke.reshape(-1)).to(dev)
+    dE = torch.from_numpy(E).to(dev) if E is not None else None
+    nel = gen.nelements
+    brow, bcol = bsr.fem_q1_coords(d, ne, 0, nel, dev)
+    n = (ne + 1) ** d
+    t0 = time.perf_counter()
+    plan = bsr.BcooPlan(brow, bcol, n, n, d, d)
+    cold = time.perf_counter() - t0
+    del brow, bcol
+    stream = bsr.fem_q1_blocks(d, ne, 0, nel, dKe, dE, True)
+    vals = plan.new_values()
+    ms, mn = timed(lambda: plan.set_values(stream, vals))
+    inf = plan.info()
+    out["bcoo_set_values"] = row(ms, mn, inf["algorithmic_bytes"], plan_s=cold, n_contrib=inf["n_contrib"],
+                                 nnzb=inf["nnzb"])
+    ms, mn = timed(lambda: bsr.fem_q1_blocks(d, ne, 0, nel, dKe, dE, True, stream))
+    out["fem_q1_element_blocks"] = row(ms, mn, 8 * stream.numel())
     return out
 
 
@@ -429,7 +523,7 @@ def run_vcycle(peak: float, cfg: int = 4, reps: int = 10) -> dict:
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--config", type=int, default=3, help="BASELINE.json config (3 = the 128^3 headline grid)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
@@ -437,6 +531,8 @@ def main():
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-vcycle", action="store_true", help="skip the config-4 V-cycle timing")
+    ap.add_argument("--no-next-rows", action="store_true", help="skip the f1 / f2 timings (prolongator smoothing, "
+                    "blocked COO assembly)")
     args = ap.parse_args()
     if args.impl == "reference":
         if int(os.environ.get("RANK", "0")) != 0:

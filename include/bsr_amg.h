@@ -73,6 +73,10 @@ int bsr_create(bsr_t* out, int32_t nbrows, int32_t nbcols, int32_t bs_r, int32_t
 /* The caller rewrote d_vals in place: bumps the matrix's state counter (the analogue of PETSc's object state that
  * gates the P-side cache).  Host-only, no device work. */
 int bsr_values_changed(bsr_t A);
+/* The caller's values now live in another device array of the same size (double buffering of operator updates):
+ * borrows d_vals (16-byte aligned) instead of the old array and bumps the state counter.  Host-only.
+ * Errors: BSR_ERR_NULL, BSR_ERR_ALIGN, BSR_ERR_PLAN (a library-owned matrix). */
+int bsr_rebind_values(bsr_t A, double* d_vals);
 /* Releases the descriptor and every library-owned cache attached to it (cached transpose).  Null is accepted. */
 int bsr_destroy(bsr_t A);
 /* Queries (host-only).  Any out pointer may be null. */
@@ -249,6 +253,9 @@ int fem_q1_element_blocks(int32_t d, int32_t ne, int64_t e0, int64_t e1, const d
  * Process-wide counts since load: kernels launched by this library, device allocations made by this library.
  * Hot calls must not move n_allocs. */
 int bsr_counters(int64_t* n_kernel_launches, int64_t* n_allocs);
+/* Measured fp64 FMA peak of the current device in TFLOP/s (register-resident FMA chains, CUDA events, best of 5):
+ * the ALU roof reported beside the HBM roof of the PtAP kernels.  COLD: allocates, synchronises. */
+int bsr_measure_fp64_peak(double* tflops, void* stream);
 
 /* ------------------------------------------------------------------ options of the COLD calls (tests, tuning)
  * Process-wide; read by ptap_symbolic only, never by a hot call.  Names: "ptap_force_gather" (1: keep the

@@ -35,6 +35,10 @@
 #include <cstring>
 #include <vector>
 
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
 extern "C" {
 typedef struct {
   int32_t nbrows, nbcols, bs_r, bs_c;
@@ -193,6 +197,19 @@ void vcycle(const Hier& H, int l, const double* b, double* x) {
 
 // =================================================================== C ABI
 extern "C" {
+
+// threads the row-parallel routines use from now on (0: the OpenMP default); returns the count in effect.  Only the
+// timing legs of bench.py call this (1 thread / all cores); it changes no arithmetic.
+int orc_set_threads(int n) {
+#ifdef _OPENMP
+  static const int dflt = omp_get_max_threads();
+  omp_set_num_threads(n > 0 ? n : dflt);
+  return omp_get_max_threads();
+#else
+  (void)n;
+  return 1;
+#endif
+}
 
 int orc_spmv(const orc_bsr* A, const double* x, double* y) { spmv(*A, x, y); return 0; }
 int orc_spmv_t(const orc_bsr* A, const double* x, double* y) { spmv_t(*A, x, y); return 0; }

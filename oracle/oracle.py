@@ -58,6 +58,7 @@ def _load():
         lib = C.CDLL(build())
         P = C.POINTER(_Bsr)
         V = C.c_void_p
+        lib.orc_set_threads.argtypes = [C.c_int]
         lib.orc_spmv.argtypes = [P, V, V]
         lib.orc_spmv_t.argtypes = [P, V, V]
         lib.orc_spmv_fast.argtypes = [P, V, V]
@@ -95,6 +96,11 @@ class _Held:
 
 def _vec(x) -> np.ndarray:
     return np.ascontiguousarray(x, dtype=np.float64)
+
+
+def set_threads(n: int = 0) -> int:
+    """OpenMP threads of the row-parallel routines from now on (0: default); returns the count in effect."""
+    return int(_load().orc_set_threads(int(n)))
 
 
 def spmv(A, x) -> np.ndarray:

@@ -25,6 +25,7 @@ SYMBOLS = {
     "bsr_last_error": (C.c_char_p, []),
     "bsr_create": (C.c_int, [_PV, _I32, _I32, _I32, _I32, _I64, _V, _V, _V, _V]),
     "bsr_values_changed": (C.c_int, [_V]),
+    "bsr_rebind_values": (C.c_int, [_V, _V]),
     "bsr_destroy": (C.c_int, [_V]),
     "bsr_get_info": (C.c_int, [_V, _PI32, _PI32, _PI32, _PI32, _PI64, _PI64]),
     "bsr_spmv": (C.c_int, [_V, _V, _V, _V]),
@@ -55,6 +56,7 @@ SYMBOLS = {
     "vcycle_apply_host": (C.c_int, [_V, _V, _V, _V]),
     "vcycle_destroy": (C.c_int, [_V]),
     "bsr_counters": (C.c_int, [_PI64, _PI64]),
+    "bsr_measure_fp64_peak": (C.c_int, [C.POINTER(_D), _V]),
     "prolongator_smooth_symbolic": (C.c_int, [_PV, _V, _V, _PI64, _V]),
     "prolongator_smooth_structure": (C.c_int, [_V, _V, _V, _V]),
     "prolongator_smooth_numeric": (C.c_int, [_V, _V, _V, _D, _V, _V]),
@@ -119,6 +121,13 @@ def counters():
     return a.value, b.value
 
 
+def fp64_peak_tflops() -> float:
+    """Measured fp64 FMA peak of the current device (bsr_measure_fp64_peak)."""
+    t = C.c_double()
+    _check(lib().bsr_measure_fp64_peak(C.byref(t), _stream()))
+    return t.value
+
+
 class Bsr:
     """A block-CSR matrix on the device (bsr_create).  Keeps the torch tensors it borrows alive."""
 
@@ -155,6 +164,12 @@ class Bsr:
 
     def values_changed(self):
         _check(lib().bsr_values_changed(self.h))
+
+    def rebind_values(self, vals):
+        """The values now live in another device tensor of the same size (bsr_rebind_values); bumps the state."""
+        assert vals.numel() == self.vals.numel() and vals.dtype == self.vals.dtype and vals.is_cuda
+        _check(lib().bsr_rebind_values(self.h, _dev(vals)))
+        self.vals = vals
 
     def set_values(self, host_vals):
         """Rewrite the values in place from a host array and bump the state counter."""

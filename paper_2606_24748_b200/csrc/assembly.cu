@@ -202,6 +202,7 @@ int bcoo_set_values(bcoo_plan_t pl, const double* d_stream, double* d_vals, void
   if (pl->nnzb == 0) return BSR_OK;
   if (!d_stream || !d_vals) return fail(BSR_ERR_NULL, "null array");
   cudaStream_t st = (cudaStream_t)stream;
+  NvtxRange nv("bcoo_set_values");
   const int bb = pl->bs_r * pl->bs_c;
   const int64_t nvals = pl->nnzb * bb;
   const unsigned grid = (unsigned)((nvals + 255) / 256);

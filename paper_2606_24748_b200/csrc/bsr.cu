@@ -570,6 +570,16 @@ int bsr_values_changed(bsr_t A) {
   return BSR_OK;
 }
 
+int bsr_rebind_values(bsr_t A, double* d_vals) {
+  if (!valid(A)) return fail(BSR_ERR_NULL, "invalid matrix handle");
+  if (!d_vals && A->nnzb > 0) return fail(BSR_ERR_NULL, "bsr_rebind_values: null array");
+  if ((uintptr_t)d_vals & 15) return fail(BSR_ERR_ALIGN, "d_vals not 16-byte aligned");
+  if (A->owns_arrays) return fail(BSR_ERR_PLAN, "library-owned matrix");
+  A->d_vals = d_vals;
+  A->state++;
+  return BSR_OK;
+}
+
 int bsr_destroy(bsr_t A) {
   if (!A) return BSR_OK;
   if (A->magic != BSR_MAGIC) return fail(BSR_ERR_NULL, "invalid matrix handle");
@@ -607,6 +617,7 @@ int bsr_spmv(bsr_t A, const double* d_x, double* d_y, void* stream) {
   if (!valid(A)) return fail(BSR_ERR_NULL, "invalid matrix handle");
   if (A->nbrows == 0) return BSR_OK;  // nothing to write; null vectors are fine for an empty matrix
   if ((!d_x && A->nbcols > 0) || !d_y) return fail(BSR_ERR_NULL, "null vector");
+  NvtxRange nv("bsr_spmv");
   return spmv_launch(A, d_x, d_y, nullptr, EPI_ASSIGN, (cudaStream_t)stream);
 }
 
@@ -621,6 +632,7 @@ int bsr_spmv_t(bsr_t A, const double* d_x, double* d_y, void* stream) {
   if (!valid(A)) return fail(BSR_ERR_NULL, "invalid matrix handle");
   if (A->nbcols == 0) return BSR_OK;
   if ((!d_x && A->nbrows > 0) || !d_y) return fail(BSR_ERR_NULL, "null vector");
+  NvtxRange nv("bsr_spmv_t");
   BSR_TRY(transpose_ensure(A, (cudaStream_t)stream));
   return spmv_launch(A->T, d_x, d_y, nullptr, EPI_ASSIGN, (cudaStream_t)stream);
 }

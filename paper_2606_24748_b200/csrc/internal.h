@@ -8,6 +8,7 @@
 #include <vector>
 
 #include <cuda_runtime.h>
+#include <nvtx3/nvToolsExt.h>
 
 #include "bsr_amg.h"
 
@@ -38,6 +39,14 @@ extern std::atomic<int64_t> g_allocs;
     cudaError_t e__ = cudaGetLastError();                                                \
     if (e__ != cudaSuccess) return ::bsramg::fail(BSR_ERR_CUDA, "launch %s: %s", #kernel, cudaGetErrorString(e__)); \
   } while (0)
+
+// NVTX range around a hot entry point (tracing); a no-op unless a profiler is attached
+struct NvtxRange {
+  explicit NvtxRange(const char* name) { nvtxRangePushA(name); }
+  ~NvtxRange() { nvtxRangePop(); }
+  NvtxRange(const NvtxRange&) = delete;
+  NvtxRange& operator=(const NvtxRange&) = delete;
+};
 
 int dev_alloc(void** p, size_t bytes);  // cudaMalloc + counter (cold paths only)
 void dev_free(void* p);

@@ -374,6 +374,7 @@ int ptap_structure(ptap_plan_t pl, int32_t* d_rowptr_c, int32_t* d_colidx_c, voi
 int ptap_numeric_stage(ptap_plan_t pl, int32_t stage, bsr_t A, bsr_t P, double* d_vals_c, void* stream) {
   BSR_TRY(plan_check(pl, A, P));
   cudaStream_t st = (cudaStream_t)stream;
+  NvtxRange nv(stage == 1 ? "ptap_numeric_stage1" : "ptap_numeric_stage2");
   if (stage == 1) return stage1(pl, st);
   if (stage == 2) {
     if (!d_vals_c && pl->nnzb_c) return fail(BSR_ERR_NULL, "d_vals_c is null");
@@ -389,6 +390,7 @@ int ptap_numeric(ptap_plan_t pl, bsr_t A, bsr_t P, double* d_vals_c, void* strea
   if (!d_vals_c && pl->nnzb_c) return fail(BSR_ERR_NULL, "d_vals_c is null");
   if ((uintptr_t)d_vals_c & 15) return fail(BSR_ERR_ALIGN, "d_vals_c must be 16-byte aligned");
   cudaStream_t st = (cudaStream_t)stream;
+  NvtxRange nv("ptap_numeric");
   BSR_TRY(transpose_ensure(P, st));  // state gate: re-transposes R's values only if P changed
   BSR_TRY(stage1(pl, st));
   return stage2(pl, d_vals_c, st);

@@ -195,6 +195,7 @@ int prolongator_smooth_numeric(psmooth_plan_t pl, bsr_t A, bsr_t Pt, double omeg
   if (!d_vals_p && pl->nnzb_p) return fail(BSR_ERR_NULL, "d_vals_p is null");
   if ((uintptr_t)d_vals_p & 15) return fail(BSR_ERR_ALIGN, "d_vals_p must be 16-byte aligned");
   cudaStream_t st = (cudaStream_t)stream;
+  NvtxRange nv("prolongator_smooth_numeric");
   BSR_TRY(block_diag_inverse(A, pl->dinv, pl->status, st));
   if (pl->s1.ok) {
     StreamArgs a = pl->s1.args;

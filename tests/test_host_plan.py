@@ -19,7 +19,7 @@ ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 def test_library_exports_every_declared_symbol():
     hdr = open(os.path.join(ROOT, "include", "bsr_amg.h")).read()
     hdr = re.sub(r"/\*.*?\*/", "", hdr, flags=re.S)
-    declared = set(re.findall(r"\b((?:bsr|ptap|vcycle|pcg)_[a-z_0-9]+)\s*\(", hdr))
+    declared = set(re.findall(r"\b((?:bsr|ptap|vcycle|pcg|prolongator_smooth|bcoo|fem_q1)_[a-z_0-9]+)\s*\(", hdr))
     assert {"bsr_create", "bsr_spmv", "bsr_spmv_t", "ptap_symbolic", "ptap_numeric", "vcycle_apply"} <= declared
     L = bsr.lib()
     for name in declared:
