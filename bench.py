@@ -384,6 +384,10 @@ def run_ours(args) -> dict | None:
         del plan, GA, GP, x, xc, y, yc, vals_c, a_bufs
         torch.cuda.empty_cache()
         out["vcycle"] = run_vcycle(peak)
+    if not args.no_second_workload:
+        import gc
+        gc.collect(); torch.cuda.empty_cache()
+        out["second_workload"] = run_second_workload(peak)
     if not args.no_cpu_baseline:
         from oracle import oracle as orc
         op = OraclePass(A, P, seed)
@@ -461,6 +465,52 @@ def run_next_rows(gen, A, GA, peak: float, reps: int = 10) -> dict:
     return out
 
 
+def run_second_workload(peak: float, reps: int = 10) -> dict:
+    """the same hot path on the denser (config 5: Q2 elements, ~185 nonzeros per row) and the
+    irregular (config 6: greedy aggregates) operator of the 65^3 node grid -- PAPER.md:206-217 finds that the block
+    advantage shrinks as rows get denser; rows beyond the staged PtAP format run the gather kernels (`staged`)."""
+    import torch
+    from paper_2606_24748_b200 import bsr, problems as pr
+
+    def timed(fn):
+        for _ in range(3):
+            fn()
+        evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(reps)]
+        torch.cuda.synchronize()
+        for e0, e1 in evs:
+            e0.record(); fn(); e1.record()
+        torch.cuda.synchronize()
+        return float(np.median([e0.elapsed_time(e1) for e0, e1 in evs]))
+
+    out = {}
+    for cfg in (5, 6):
+        gen, A, P = make_problem(cfg)
+        seed = pr.CONFIGS[cfg]["seed"]
+        GA, GP = bsr.Bsr.from_host(A), bsr.Bsr.from_host(P)
+        plan = bsr.PtapPlan(GA, GP)
+        GP.transpose_prepare()
+        x = torch.from_numpy(pr.uniform(seed, pr.PURPOSE_FINE, A.nbrows * A.bs_r)).cuda()
+        xc = torch.from_numpy(pr.uniform(seed, pr.PURPOSE_COARSE, P.nbcols * P.bs_c)).cuda()
+        y, yc, vals_c = torch.empty_like(x), torch.empty_like(xc), plan.new_values()
+        R = pr.HostBSR(P.nbcols, P.nbrows, P.bs_c, P.bs_r, None, P.colidx, None)
+        ops = {}
+        for name, fn, nb in (("spmv_A", lambda: GA.spmv(x, y), spmv_bytes(A)), ("spmv_P", lambda: GP.spmv(xc, y), spmv_bytes(P)),
+                             ("spmv_Pt", lambda: GP.spmv_t(x, yc), spmv_bytes(R)),
+                             ("ptap_numeric", lambda: plan.numeric(vals_c), plan.info()["algorithmic_bytes"])):
+            ms = timed(fn)
+            gbs = nb / (ms * 1e-3) / 1e9
+            ops[name] = {"ms": ms, "algorithmic_GB": nb / 1e9, "GB/s": gbs, "frac_of_measured_hbm": gbs / peak}
+        sched = plan.schedule()
+        ops["ptap_numeric"]["staged"] = [bool(sched[1]["staged"]), bool(sched[2]["staged"])]
+        out[f"cfg{cfg}"] = {"workload": workload_name(cfg, A, P), "nnz_per_row": A.nnzb * A.bs_c / A.nbrows,
+                            "max_blocks_per_row": {"A": int(np.diff(A.rowptr).max()), "P": int(np.diff(P.rowptr).max()),
+                                                   "A_c": int(np.diff(plan.rowptr_c.cpu().numpy()).max())},
+                            "l2": "A is %.2f GB (exceeds L2)" % (bsr_bytes(A) / 1e9), "ops": ops}
+        del plan, GA, GP, x, xc, y, yc, vals_c
+        torch.cuda.empty_cache()
+    return out
+
+
 def run_vcycle(peak: float, cfg: int = 4, reps: int = 10) -> dict:
     """BASELINE.json's third number: V-cycle ms at config 4 (96^3, three levels, V(2,2) degree-2 Chebyshev / block
     Jacobi, dense coarsest solve), plus the full hierarchy recompute and one PCG iteration.  The hierarchy is built
@@ -531,6 +581,7 @@ def main():
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-vcycle", action="store_true", help="skip the config-4 V-cycle timing")
+    ap.add_argument("--no-second-workload", action="store_true", help="skip the f4 timings (configs 5 and 6)")
     ap.add_argument("--no-next-rows", action="store_true", help="skip the f1 / f2 timings (prolongator smoothing, "
                     "blocked COO assembly)")
     args = ap.parse_args()

@@ -18,6 +18,11 @@
 //                20 power iterations on D^-1 A (R10, R11).
 //   O9 level 2   coarse near-null space B_j(C) = R_j * M(c_j - C) (R9, R20).
 // Random numbers: SplitMix64, one stream per (seed, purpose) (R12).
+// Second workload: order = 2 builds the Q2 (triquadratic, 27-node hex /
+// 9-node quad, 3-point Gauss) operator on the (2 ne + 1)^d node grid -- ~185 scalar nonzeros per row against Q1's ~78,
+// the paper's Q2 harness has 169-180 -- and agg_mode = 1 replaces the node boxes by a seeded greedy disjoint covering
+// of the operator's graph (root + neighbours, leftovers join an adjacent aggregate), which gives
+// irregular aggregate sizes and coarse rows longer than the 27 of the box stencil.
 //
 // C ABI at the bottom (egen_*); all arrays are host memory owned by the handle.
 #include <algorithm>
@@ -85,6 +90,8 @@ struct Gen {
   uint64_t seed = 0;
   int modulus_mode = 0;  // 0: E = 1; 1: per-element lognormal(0, 1) (config 3)
   int dirichlet = 1;     // 0: pure Neumann operator (used by the invariant tests)
+  int order = 1;         // 1: Q1 elements, 2: Q2 elements (f4)
+  int agg_mode = 0;      // 0: 3^d node boxes (R6), 1: seeded greedy disjoint covering of the graph (f4)
   std::vector<Level> levels;
   std::vector<double> Emod;  // per-element modulus (empty: 1 everywhere)
   std::vector<double> Ke;    // reference element matrix (E = 1)
@@ -93,59 +100,83 @@ struct Gen {
 
 // ---------------------------------------------------------------- O2: element matrix
 // K[(a*d+i)][(b*d+j)] = int  lam d_i N_a d_j N_b + mu d_j N_a d_i N_b + mu delta_ij grad N_a . grad N_b
-// Local node a has reference coordinates (+-1 per direction), bit k of a selects direction k (x fastest).
-void element_matrix(int d, double h, double E, double nu, std::vector<double>& K) {
-  const int nen = 1 << d, nd = d * nen;
+// Tensor-product Lagrange element of order p (1: Q1, 2: Q2) on a cube of side h: local node a has index a_k in
+// {0..p} in direction k, a = a_0 + (p+1) (a_1 + (p+1) a_2) (x fastest); p+1 Gauss points per direction.
+void element_matrix(int d, int p, double h, double E, double nu, std::vector<double>& K) {
+  const int n1 = p + 1;
+  int nen = 1;
+  for (int k = 0; k < d; ++k) nen *= n1;
+  const int nd = d * nen;
   K.assign((size_t)nd * nd, 0.0);
   const double lam = E * nu / ((1 + nu) * (1 - 2 * nu)), mu = E / (2 * (1 + nu));
-  const double g = 1.0 / std::sqrt(3.0);
+  double gp[3], gw[3];
+  if (p == 1) { gp[0] = -1.0 / std::sqrt(3.0); gp[1] = -gp[0]; gw[0] = gw[1] = 1.0; }
+  else { gp[0] = -std::sqrt(0.6); gp[1] = 0.0; gp[2] = std::sqrt(0.6); gw[0] = gw[2] = 5.0 / 9.0; gw[1] = 8.0 / 9.0; }
+  auto shape = [&](int a, double xi, double& N, double& dN) {   // 1D Lagrange on nodes -1, (0,) 1
+    if (p == 1) { const double s = a ? 1.0 : -1.0; N = (1 + s * xi) / 2; dN = s / 2; }
+    else if (a == 0) { N = xi * (xi - 1) / 2; dN = xi - 0.5; }
+    else if (a == 1) { N = 1 - xi * xi; dN = -2 * xi; }
+    else { N = xi * (xi + 1) / 2; dN = xi + 0.5; }
+  };
   const double detJ = std::pow(h / 2, d);
-  for (int q = 0; q < nen; ++q) {  // 2^d Gauss points, weight 1
-    double xi[3] = {0, 0, 0};
-    for (int k = 0; k < d; ++k) xi[k] = ((q >> k) & 1) ? g : -g;
-    double dN[8][3];
-    for (int a = 0; a < nen; ++a)
+  int nq = 1;
+  for (int k = 0; k < d; ++k) nq *= n1;
+  std::vector<double> dN((size_t)nen * 3);
+  for (int q = 0; q < nq; ++q) {
+    double xi[3] = {0, 0, 0}, w = 1;
+    for (int k = 0, t = q; k < d; ++k, t /= n1) { xi[k] = gp[t % n1]; w *= gw[t % n1]; }
+    for (int a = 0; a < nen; ++a) {
+      int ak[3] = {0, 0, 0};
+      for (int k = 0, t = a; k < d; ++k, t /= n1) ak[k] = t % n1;
       for (int k = 0; k < d; ++k) {
         double v = 1;
         for (int m = 0; m < d; ++m) {
-          double s = ((a >> m) & 1) ? 1.0 : -1.0;
-          v *= (m == k) ? s / 2 : (1 + s * xi[m]) / 2;
+          double N, D;
+          shape(ak[m], xi[m], N, D);
+          v *= (m == k) ? D : N;
         }
-        dN[a][k] = v * (2 / h);
+        dN[(size_t)a * 3 + k] = v * (2 / h);
       }
+    }
     for (int a = 0; a < nen; ++a)
       for (int b = 0; b < nen; ++b) {
         double gg = 0;
-        for (int k = 0; k < d; ++k) gg += dN[a][k] * dN[b][k];
+        for (int k = 0; k < d; ++k) gg += dN[(size_t)a * 3 + k] * dN[(size_t)b * 3 + k];
         for (int i = 0; i < d; ++i)
           for (int j = 0; j < d; ++j) {
-            double v = lam * dN[a][i] * dN[b][j] + mu * dN[a][j] * dN[b][i] + (i == j ? mu * gg : 0.0);
-            K[(size_t)(a * d + i) * nd + (b * d + j)] += v * detJ;
+            double v = lam * dN[(size_t)a * 3 + i] * dN[(size_t)b * 3 + j] + mu * dN[(size_t)a * 3 + j] * dN[(size_t)b * 3 + i] +
+                       (i == j ? mu * gg : 0.0);
+            K[(size_t)(a * d + i) * nd + (b * d + j)] += v * detJ * w;
           }
       }
   }
 }
 
 // ---------------------------------------------------------------- O1, O3, O4: fine operator
-inline int clip_lo(int i) { return i > 0 ? -1 : 0; }
-inline int clip_hi(int i, int n) { return i < n - 1 ? 1 : 0; }
+// Node i (one direction) of an order-p grid couples to the nodes of the elements that contain it: an element-corner
+// node (i % p == 0) to [i-p, i+p], an interior node to its own element [i - i%p, i - i%p + p]; clipped to the grid.
+inline int nb_lo(int i, int p) { return std::max(0, i - ((i % p == 0) ? p : i % p)); }
+inline int nb_hi(int i, int p, int n) { return std::min(n - 1, i + ((i % p == 0) ? p : p - i % p)); }
+// elements containing node i: [el_lo, el_hi]
+inline int el_lo(int i, int p) { return std::max(0, (i % p == 0) ? i / p - 1 : i / p); }
+inline int el_hi(int i, int p, int ne) { return std::min(ne - 1, i / p); }
 
 void build_fine_operator(Gen& G) {
   Level& L = G.levels[0];
-  const int d = G.d, n = G.ne + 1, ne = G.ne;
+  const int d = G.d, p = G.order, ne = G.ne, n = p * ne + 1, n1 = p + 1;
   L.d = d; L.bs = d; L.nb = (d == 3) ? 6 : 3;
   L.nx[0] = n; L.nx[1] = n; L.nx[2] = (d == 3) ? n : 1;
   const int nz = L.nx[2];
   const int64_t N = L.nnodes();
-  const double h = 1.0 / ne;
+  const double h = 1.0 / ne, hn = h / p;
   L.coords.resize((size_t)N * d);
   for (int iz = 0; iz < nz; ++iz)
     for (int iy = 0; iy < n; ++iy)
       for (int ix = 0; ix < n; ++ix) {
         int64_t id = ix + (int64_t)n * (iy + (int64_t)n * iz);
-        L.coords[id * d + 0] = ix * h;
-        L.coords[id * d + 1] = iy * h;
-        if (d == 3) L.coords[id * d + 2] = iz * h;
+        L.coords[id * d + 0] = ix * hn;
+        L.coords[id * d + 1] = iy * hn;
+        if (d == 3) L.coords[id * d + 2] = iz * hn;
       }
   // per-element Young's modulus (config 3: lognormal(0,1), Box-Muller cosine branch, element order)
   const int nez = (d == 3) ? ne : 1;
@@ -161,8 +192,10 @@ void build_fine_operator(Gen& G) {
     }
   }
   std::vector<double>& Ke = G.Ke;
-  element_matrix(d, h, 1.0, G.nu, Ke);
-  const int nen = 1 << d, nd = d * nen, bb = d * d;
+  element_matrix(d, p, h, 1.0, G.nu, Ke);
+  int nen = 1;
+  for (int k = 0; k < d; ++k) nen *= n1;
+  const int nd = d * nen, bb = d * d;
 
   Bsr& A = L.A;
   A.nbrows = A.nbcols = (int32_t)N; A.bs_r = A.bs_c = d;
@@ -171,8 +204,8 @@ void build_fine_operator(Gen& G) {
     for (int iy = 0; iy < n; ++iy)
       for (int ix = 0; ix < n; ++ix) {
         int64_t id = ix + (int64_t)n * (iy + (int64_t)n * iz);
-        int cx = clip_hi(ix, n) - clip_lo(ix) + 1, cy = clip_hi(iy, n) - clip_lo(iy) + 1;
-        int cz = (d == 3) ? clip_hi(iz, nz) - clip_lo(iz) + 1 : 1;
+        int cx = nb_hi(ix, p, n) - nb_lo(ix, p) + 1, cy = nb_hi(iy, p, n) - nb_lo(iy, p) + 1;
+        int cz = (d == 3) ? nb_hi(iz, p, nz) - nb_lo(iz, p) + 1 : 1;
         A.rowptr[id + 1] = cx * cy * cz;
       }
   for (int64_t i = 0; i < N; ++i) A.rowptr[i + 1] += A.rowptr[i];
@@ -185,28 +218,26 @@ void build_fine_operator(Gen& G) {
     for (int iy = 0; iy < n; ++iy)
       for (int ix = 0; ix < n; ++ix) {
         const int64_t id = ix + (int64_t)n * (iy + (int64_t)n * iz);
-        const int lx = clip_lo(ix), ly = clip_lo(iy), lz = (d == 3) ? clip_lo(iz) : 0;
-        const int cx = clip_hi(ix, n) - lx + 1, cy = clip_hi(iy, n) - ly + 1;
-        const int cz = (d == 3) ? clip_hi(iz, nz) - lz + 1 : 1;
+        const int x0 = nb_lo(ix, p), y0 = nb_lo(iy, p), z0 = (d == 3) ? nb_lo(iz, p) : 0;
+        const int cx = nb_hi(ix, p, n) - x0 + 1, cy = nb_hi(iy, p, n) - y0 + 1;
+        const int cz = (d == 3) ? nb_hi(iz, p, nz) - z0 + 1 : 1;
         const int64_t base = A.rowptr[id];
         for (int sz = 0; sz < cz; ++sz)
           for (int sy = 0; sy < cy; ++sy)
             for (int sx = 0; sx < cx; ++sx)
               A.colidx[base + (sz * cy + sy) * cx + sx] =
-                  (int32_t)((ix + lx + sx) + (int64_t)n * ((iy + ly + sy) + (int64_t)n * (iz + lz + sz)));
+                  (int32_t)((x0 + sx) + (int64_t)n * ((y0 + sy) + (int64_t)n * (z0 + sz)));
         // gather form of the element loop: adjacent elements in ascending element id
-        for (int oz = (d == 3 ? -1 : 0); oz <= 0; ++oz)
-          for (int oy = -1; oy <= 0; ++oy)
-            for (int ox = -1; ox <= 0; ++ox) {
-              const int ex = ix + ox, ey = iy + oy, ez = iz + oz;
-              if (ex < 0 || ex >= ne || ey < 0 || ey >= ne) continue;
-              if (d == 3 && (ez < 0 || ez >= ne)) continue;
+        const int ez0 = (d == 3) ? el_lo(iz, p) : 0, ez1 = (d == 3) ? el_hi(iz, p, ne) : 0;
+        for (int ez = ez0; ez <= ez1; ++ez)
+          for (int ey = el_lo(iy, p); ey <= el_hi(iy, p, ne); ++ey)
+            for (int ex = el_lo(ix, p); ex <= el_hi(ix, p, ne); ++ex) {
               const int64_t e = ex + (int64_t)ne * (ey + (int64_t)ne * (d == 3 ? ez : 0));
               const double Ee = Emod.empty() ? 1.0 : Emod[e];
-              const int a = (-ox) | ((-oy) << 1) | ((d == 3 ? -oz : 0) << 2);
+              const int a = (ix - p * ex) + n1 * ((iy - p * ey) + n1 * (d == 3 ? iz - p * ez : 0));
               for (int b = 0; b < nen; ++b) {
-                const int dx = ox + (b & 1), dy = oy + ((b >> 1) & 1), dz = (d == 3) ? oz + ((b >> 2) & 1) : 0;
-                const int64_t slot = base + ((dz - lz) * cy + (dy - ly)) * cx + (dx - lx);
+                const int bx = p * ex + b % n1, by = p * ey + (b / n1) % n1, bz = (d == 3) ? p * ez + b / (n1 * n1) : 0;
+                const int64_t slot = base + ((bz - z0) * cy + (by - y0)) * cx + (bx - x0);
                 double* blk = &A.vals[(size_t)slot * bb];
                 for (int i = 0; i < d; ++i)
                   for (int j = 0; j < d; ++j) blk[i * d + j] += Ee * Ke[(size_t)(a * d + i) * nd + (b * d + j)];
@@ -331,20 +362,56 @@ bool build_P(Gen& G, int l) {
   const int d = L.d, bs = L.bs, nb = L.nb;
   const int64_t N = L.nnodes();
   int na[3] = {1, 1, 1};
-  for (int k = 0; k < d; ++k) na[k] = std::max(1, L.nx[k] / 3);
-  const int64_t NA = (int64_t)na[0] * na[1] * na[2];
-  L.agg.resize(N);
-  std::vector<std::vector<int32_t>> members(NA);
-  for (int iz = 0; iz < L.nx[2]; ++iz)
-    for (int iy = 0; iy < L.nx[1]; ++iy)
-      for (int ix = 0; ix < L.nx[0]; ++ix) {
-        const int64_t id = ix + (int64_t)L.nx[0] * (iy + (int64_t)L.nx[1] * iz);
-        const int ax = std::min(ix / 3, na[0] - 1), ay = std::min(iy / 3, na[1] - 1);
-        const int az = (d == 3) ? std::min(iz / 3, na[2] - 1) : 0;
-        const int64_t J = ax + (int64_t)na[0] * (ay + (int64_t)na[1] * az);
-        L.agg[id] = (int32_t)J;
-        members[J].push_back((int32_t)id);  // ascending node id
+  int64_t NA = 0;
+  L.agg.assign(N, -1);
+  if (G.agg_mode == 0) {
+    for (int k = 0; k < d; ++k) na[k] = std::max(1, L.nx[k] / 3);
+    NA = (int64_t)na[0] * na[1] * na[2];
+    for (int iz = 0; iz < L.nx[2]; ++iz)
+      for (int iy = 0; iy < L.nx[1]; ++iy)
+        for (int ix = 0; ix < L.nx[0]; ++ix) {
+          const int64_t id = ix + (int64_t)L.nx[0] * (iy + (int64_t)L.nx[1] * iz);
+          const int ax = std::min(ix / 3, na[0] - 1), ay = std::min(iy / 3, na[1] - 1);
+          const int az = (d == 3) ? std::min(iz / 3, na[2] - 1) : 0;
+          L.agg[id] = (int32_t)(ax + (int64_t)na[0] * (ay + (int64_t)na[1] * az));
+        }
+  } else {
+    // greedy disjoint covering of the operator's graph, every stored block an edge (threshold 0):
+    // pass 1 visits the nodes in a seeded random order and makes root + neighbours an aggregate when all of them
+    // are still free; later passes attach every free node to the aggregate of its first aggregated neighbour, one
+    // ring per pass (deterministic: decisions of a pass use the state before the pass)
+    const Bsr& G0 = L.A;
+    std::vector<int32_t> order(N);
+    for (int64_t i = 0; i < N; ++i) order[i] = (int32_t)i;
+    SplitMix64 g = stream(G.seed, 6 + 16 * (uint64_t)l);
+    for (int64_t i = N - 1; i > 0; --i) std::swap(order[i], order[(int64_t)(g.next() % (uint64_t)(i + 1))]);
+    for (int64_t t = 0; t < N; ++t) {
+      const int32_t r = order[t];
+      bool free_all = true;
+      for (int64_t k = G0.rowptr[r]; k < G0.rowptr[r + 1] && free_all; ++k) free_all = L.agg[G0.colidx[k]] < 0;
+      if (!free_all || L.agg[r] >= 0) continue;
+      for (int64_t k = G0.rowptr[r]; k < G0.rowptr[r + 1]; ++k) L.agg[G0.colidx[k]] = (int32_t)NA;
+      L.agg[r] = (int32_t)NA;
+      ++NA;
+    }
+    if (NA == 0) { G.err = "empty graph"; return false; }
+    for (bool left = true; left;) {
+      left = false;
+      std::vector<int32_t> next(L.agg);
+      bool progress = false;
+      for (int64_t i = 0; i < N; ++i) {
+        if (L.agg[i] >= 0) continue;
+        for (int64_t k = G0.rowptr[i]; k < G0.rowptr[i + 1]; ++k)
+          if (L.agg[G0.colidx[k]] >= 0) { next[i] = L.agg[G0.colidx[k]]; progress = true; break; }
+        if (next[i] < 0) left = true;
       }
+      L.agg.swap(next);
+      if (left && !progress) { G.err = "disconnected graph in aggregation"; return false; }
+    }
+    na[0] = (int)NA;
+  }
+  std::vector<std::vector<int32_t>> members(NA);
+  for (int64_t id = 0; id < N; ++id) members[L.agg[id]].push_back((int32_t)id);  // ascending node id
   // next level skeleton
   Level& Lc = G.levels[l + 1];
   Level& Lf = L;
@@ -501,13 +568,18 @@ typedef struct Gen* egen_t;
 
 // d = 2 or 3; ne elements per side; modulus_mode 0 (E = 1) or 1 (per-element lognormal(0,1), stream 4);
 // dirichlet 1 (face ix = 0 clamped, R4) or 0 (Neumann operator for the invariant tests).
-egen_t egen_create(int d, int ne, double nu, uint64_t seed, int modulus_mode, int dirichlet) {
-  if ((d != 2 && d != 3) || ne < 1) return nullptr;
+// order 1 (Q1) or 2 (Q2 elements, (2 ne + 1)^d nodes); agg_mode 0 (3^d node boxes) or 1 (seeded greedy covering).
+egen_t egen_create2(int d, int ne, double nu, uint64_t seed, int modulus_mode, int dirichlet, int order, int agg_mode) {
+  if ((d != 2 && d != 3) || ne < 1 || (order != 1 && order != 2) || (agg_mode != 0 && agg_mode != 1)) return nullptr;
   Gen* G = new Gen();
   G->d = d; G->ne = ne; G->nu = nu; G->seed = seed; G->modulus_mode = modulus_mode; G->dirichlet = dirichlet;
+  G->order = order; G->agg_mode = agg_mode;
   G->levels.resize(1);
   build_fine_operator(*G);
   return G;
+}
+egen_t egen_create(int d, int ne, double nu, uint64_t seed, int modulus_mode, int dirichlet) {
+  return egen_create2(d, ne, nu, seed, modulus_mode, dirichlet, 1, 0);
 }
 void egen_destroy(egen_t G) { delete G; }
 const char* egen_error(egen_t G) { return G ? G->err.c_str() : "null handle"; }
@@ -569,23 +641,33 @@ int egen_level_arrays(egen_t G, int level, const double** coords, const double**
   return 0;
 }
 
-// reference element matrix (for pin I1): out has (d*2^d)^2 entries
+// reference element matrix (for pin I1): out has (d*(order+1)^d)^2 entries
+int egen_element_matrix2(int d, int order, double h, double E, double nu, double* out) {
+  if ((d != 2 && d != 3) || (order != 1 && order != 2)) return -1;
+  std::vector<double> K;
+  element_matrix(d, order, h, E, nu, K);
+  std::memcpy(out, K.data(), sizeof(double) * K.size());
+  return 0;
+}
 int egen_element_matrix(int d, double h, double E, double nu, double* out) {
   if (d != 2 && d != 3) return -1;
   std::vector<double> K;
-  element_matrix(d, h, E, nu, K);
+  element_matrix(d, 1, h, E, nu, K);
   std::memcpy(out, K.data(), sizeof(double) * K.size());
   return 0;
 }
 
 // The finite-element contribution stream of elements [e0, e1) in ascending element order (blocked COO form,
-// PAPER.md:248-250): per element 4^d (2D: 16, 3D: 64) contributions (a, b), a slowest; coordinate = (node of a, node
+// PAPER.md:248-250): per element (order+1)^(2d) (Q1: 16 / 64) contributions (a, b), a slowest; coordinate = (node of a, node
 // of b); block = E_e * Ke[a][b] (d x d, row-major).  With Dirichlet the clamped face is folded into the stream: a
 // block whose row or column node has ix = 0 is zero, except the node's own diagonal block, which carries
 // I / (number of adjacent elements) so that the assembled block is exactly I (R4).  Any output may be null.
 int egen_element_stream(egen_t G, int64_t e0, int64_t e1, int32_t* brow, int32_t* bcol, double* vals) {
   if (!G || e0 < 0 || e1 < e0) return -1;
-  const int d = G->d, ne = G->ne, n = ne + 1, nen = 1 << d, nd = d * nen, bb = d * d;
+  const int d = G->d, ne = G->ne, p = G->order, n1 = p + 1, n = p * ne + 1, bb = d * d;
+  int nen = 1;
+  for (int k = 0; k < d; ++k) nen *= n1;
+  const int nd = d * nen;
   const int64_t NE = (int64_t)ne * ne * (d == 3 ? ne : 1);
   if (e1 > NE) return -2;
 #pragma omp parallel for schedule(static)
@@ -595,8 +677,8 @@ int egen_element_stream(egen_t G, int64_t e0, int64_t e1, int32_t* brow, int32_t
     for (int a = 0; a < nen; ++a)
       for (int b = 0; b < nen; ++b) {
         const int64_t c = (e - e0) * nen * nen + a * nen + b;
-        const int ax = ex + (a & 1), ay = ey + ((a >> 1) & 1), az = ez + ((a >> 2) & 1);
-        const int bx = ex + (b & 1), by = ey + ((b >> 1) & 1), bz = ez + ((b >> 2) & 1);
+        const int ax = p * ex + a % n1, ay = p * ey + (a / n1) % n1, az = (d == 3) ? p * ez + a / (n1 * n1) : 0;
+        const int bx = p * ex + b % n1, by = p * ey + (b / n1) % n1, bz = (d == 3) ? p * ez + b / (n1 * n1) : 0;
         if (brow) brow[c] = (int32_t)(ax + (int64_t)n * (ay + (int64_t)n * az));
         if (bcol) bcol[c] = (int32_t)(bx + (int64_t)n * (by + (int64_t)n * bz));
         if (!vals) continue;
@@ -605,8 +687,8 @@ int egen_element_stream(egen_t G, int64_t e0, int64_t e1, int32_t* brow, int32_t
           for (int j = 0; j < d; ++j) blk[i * d + j] = Ee * G->Ke[(size_t)(a * d + i) * nd + (b * d + j)];
         if (G->dirichlet && (ax == 0 || bx == 0)) {
           for (int t = 0; t < bb; ++t) blk[t] = 0.0;
-          if (a == b) {
-            const int cy = (ay > 0 && ay < ne) ? 2 : 1, cz = (d == 3 && az > 0 && az < ne) ? 2 : 1;
+          if (a == b) {   // number of elements that contain the node: 1 or 2 per transverse direction
+            const int cy = el_hi(ay, p, ne) - el_lo(ay, p) + 1, cz = (d == 3) ? el_hi(az, p, ne) - el_lo(az, p) + 1 : 1;
             for (int i = 0; i < d; ++i) blk[i * d + i] = 1.0 / (double)(cy * cz);
           }
         }

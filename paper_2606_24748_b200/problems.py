@@ -23,8 +23,8 @@ def _load():
     if _lib is None:
         path = _build.build_gen()
         lib = C.CDLL(path)
-        lib.egen_create.restype = C.c_void_p
-        lib.egen_create.argtypes = [C.c_int, C.c_int, C.c_double, C.c_uint64, C.c_int, C.c_int]
+        lib.egen_create2.restype = C.c_void_p
+        lib.egen_create2.argtypes = [C.c_int, C.c_int, C.c_double, C.c_uint64, C.c_int, C.c_int, C.c_int, C.c_int]
         lib.egen_destroy.argtypes = [C.c_void_p]
         lib.egen_error.restype = C.c_char_p
         lib.egen_error.argtypes = [C.c_void_p]
@@ -40,7 +40,7 @@ def _load():
                                         C.POINTER(C.c_double)]
         lib.egen_level_arrays.argtypes = [C.c_void_p, C.c_int, C.POINTER(C.POINTER(C.c_double)),
                                           C.POINTER(C.POINTER(C.c_double)), C.POINTER(C.POINTER(C.c_int32))]
-        lib.egen_element_matrix.argtypes = [C.c_int, C.c_double, C.c_double, C.c_double, C.c_void_p]
+        lib.egen_element_matrix2.argtypes = [C.c_int, C.c_int, C.c_double, C.c_double, C.c_double, C.c_void_p]
         lib.egen_element_stream.argtypes = [C.c_void_p, C.c_int64, C.c_int64, C.c_void_p, C.c_void_p, C.c_void_p]
         lib.egen_element_data.argtypes = [C.c_void_p, C.POINTER(C.POINTER(C.c_double)),
                                           C.POINTER(C.POINTER(C.c_double))]
@@ -85,6 +85,11 @@ CONFIGS = {
     3: dict(d=3, ne=128, seed=3, modulus_mode=1, nlevels=2,
             name="cfg3: 3D 128^3 Q1 hex elasticity, lognormal E, bs 3->6"),
     4: dict(d=3, ne=96, seed=4, modulus_mode=0, nlevels=3, name="cfg4: 3D 96^3 Q1 hex elasticity, 3 levels"),
+    # second workload: the same 65^3 node grid as config 2
+    5: dict(d=3, ne=32, seed=5, modulus_mode=0, nlevels=2, order=2,
+            name="cfg5: 3D 32^3 Q2 hex elasticity (65^3 nodes, ~185 nnz/row), bs 3->6, box aggregates"),
+    6: dict(d=3, ne=64, seed=6, modulus_mode=0, nlevels=2, agg_mode=1,
+            name="cfg6: 3D 64^3 Q1 hex elasticity, greedy (MIS-like) aggregates, bs 3->6"),
 }
 
 # random streams (reading R12)
@@ -97,11 +102,11 @@ def uniform(seed: int, purpose: int, n: int, a: float = -1.0, b: float = 1.0) ->
     return out
 
 
-def element_matrix(d: int, h: float, E: float = 1.0, nu: float = 0.3) -> np.ndarray:
-    nd = d * 2 ** d
+def element_matrix(d: int, h: float, E: float = 1.0, nu: float = 0.3, order: int = 1) -> np.ndarray:
+    nd = d * (order + 1) ** d
     out = np.empty((nd, nd), dtype=np.float64)
-    if _load().egen_element_matrix(d, h, E, nu, out.ctypes.data) != 0:
-        raise ValueError("bad dimension")
+    if _load().egen_element_matrix2(d, order, h, E, nu, out.ctypes.data) != 0:
+        raise ValueError("bad dimension or order")
     return out
 
 
@@ -110,10 +115,10 @@ class Generator:
     keep the Generator alive while they are in use."""
 
     def __init__(self, d: int, ne: int, seed: int = 0, modulus_mode: int = 0, nu: float = 0.3,
-                 dirichlet: bool = True):
+                 dirichlet: bool = True, order: int = 1, agg_mode: int = 0):
         self._lib = _load()
-        self.d, self.ne, self.seed = d, ne, seed
-        self._h = self._lib.egen_create(d, ne, nu, seed, modulus_mode, 1 if dirichlet else 0)
+        self.d, self.ne, self.seed, self.order, self.agg_mode = d, ne, seed, order, agg_mode
+        self._h = self._lib.egen_create2(d, ne, nu, seed, modulus_mode, 1 if dirichlet else 0, order, agg_mode)
         if not self._h:
             raise ValueError("egen_create failed")
 
@@ -166,7 +171,7 @@ class Generator:
         """Blocked COO contribution stream of elements [e0, e1): (brow, bcol, blocks (n, d, d)),
         4^d contributions per element in element order; the clamped face is folded into the blocks (R4)."""
         e1 = self.nelements if e1 is None else e1
-        n = (e1 - e0) * 4 ** self.d
+        n = (e1 - e0) * (self.order + 1) ** (2 * self.d)
         brow, bcol = np.empty(n, dtype=np.int32), np.empty(n, dtype=np.int32)
         vals = np.empty((n, self.d, self.d)) if values else None
         rc = self._lib.egen_element_stream(self._h, e0, e1, brow.ctypes.data, bcol.ctypes.data,
@@ -179,7 +184,7 @@ class Generator:
         """(per-element moduli or None, reference element matrix for E = 1): inputs of the device-side emission."""
         em, ke = C.POINTER(C.c_double)(), C.POINTER(C.c_double)()
         self._lib.egen_element_data(self._h, em, ke)
-        nd = self.d * 2 ** self.d
+        nd = self.d * (self.order + 1) ** self.d
         K = np.ctypeslib.as_array(ke, shape=(nd, nd)).copy()
         E = np.ctypeslib.as_array(em, shape=(self.nelements,)).copy() if em else None
         return E, K
@@ -206,4 +211,5 @@ class Generator:
 def make_generator(cfg: int, **over) -> Generator:
     c = dict(CONFIGS[cfg])
     c.update(over)
-    return Generator(c["d"], c["ne"], c["seed"], c["modulus_mode"], dirichlet=c.get("dirichlet", True))
+    return Generator(c["d"], c["ne"], c["seed"], c["modulus_mode"], dirichlet=c.get("dirichlet", True),
+                     order=c.get("order", 1), agg_mode=c.get("agg_mode", 0))

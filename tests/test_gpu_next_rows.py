@@ -308,3 +308,44 @@ def test_fem_assembly_config3_headline_grid(bsr):
     assert sel_ref.size > 0
     assert torch.equal(vals, plan.set_values(bsr.fem_q1_blocks(3, ne, 0, g.nelements, dev(g.element_data()[1].reshape(-1)),
                                                                dev(g.element_data()[0]), True)))
+
+
+# ------------------------------------------------------------------ f4: second workload (Q2 rows, greedy aggregates)
+def _second_workload(kind, small):
+    if kind == "q2":
+        g = pr.Generator(3, 6, seed=5, order=2) if small else pr.make_generator(5)
+    else:
+        g = pr.Generator(3, 14, seed=6, agg_mode=1) if small else pr.make_generator(6)
+    g.build_prolongator(0)
+    return g
+
+
+@pytest.mark.parametrize("kind,small", [("q2", True), ("greedy", True), ("q2", False), ("greedy", False)])
+def test_second_workload_hot_path(bsr, kind, small):
+    """SpMV family (every entry), PtAP (structure ==, every block of AP and A_c against the oracle's form 2, a sample
+    of coarse rows against the long-double form 1) and prolongator smoothing on the denser (Q2, up to 125 blocks per
+    row, A_c rows of 125) and the irregular (greedy aggregates, A_c rows beyond 32 blocks) operators: rows that leave
+    the staged PtAP format run the gather kernels."""
+    from tests.test_gpu_fullsize import check_all_blocks, check_ptap_rows, check_spmv_family, sample_rows
+    g = _second_workload(kind, small)
+    A, P = g.A(0), g.P(0)
+    GA, GP = bsr.Bsr.from_host(A), bsr.Bsr.from_host(P)
+    check_spmv_family(bsr, GA, GP, A, P, g.seed)
+    plan = bsr.PtapPlan(GA, GP)
+    (rap, cap), st = orc.ptap_symbolic(A, P)
+    assert np.array_equal(plan.rowptr_c.cpu().numpy(), st[0]) and np.array_equal(plan.colidx_c.cpu().numpy(), st[1])
+    rap_g, cap_g, _ = plan.ap_host()
+    assert np.array_equal(rap_g, rap) and np.array_equal(cap_g, cap)
+    sched = plan.schedule()
+    if not small:
+        assert np.diff(st[0]).max() > 32 and not sched[2]["staged"]          # off the staged format: gather kernels
+        if kind == "q2":
+            assert (A.nbrows, A.nnzb) == (274625, 16974593) and not sched[1]["staged"]
+    vals = plan.numeric()
+    check_all_blocks(plan, vals, A, P, st, f"f4 {kind}")
+    check_ptap_rows(plan, vals, A, P, st, sample_rows(P.nbcols, 8 if not small else 4, 11))
+    import torch
+    assert torch.equal(vals, plan.numeric())
+    # prolongator smoothing on the same operator (P rows of up to 27 blocks for Q2)
+    sm, _, _, pv, ref = smooth_check(bsr, A, g.P_tent(0), g.level_info(0)["omega"])
+    assert np.abs(pv.cpu().numpy().reshape(ref.vals.shape) - P.vals).max() < 1e-13
