@@ -222,7 +222,9 @@ int prolongator_smooth_destroy(psmooth_plan_t plan);
  * "Each declared coordinate addresses a block, the value stream is a sequence of dense blocks (square or rectangular),
  * and the scatter writes and sums contiguous bs_r*bs_c runs".
  * bcoo_plan_create (COLD, synchronises): the caller declares ONCE the block coordinates (d_brow[c], d_bcol[c]),
- *   c = 0..n-1, of every contribution, duplicates included (device arrays, read here and not kept).  The plan holds
+ *   c = 0..n-1, of every contribution, duplicates included (device arrays, read here and not kept); a contribution
+ *   with a NEGATIVE coordinate is declared but ignored (its stream block is skipped by every bcoo_set_values), the
+ *   coordinate-format convention for entries the caller does not own.  The plan holds
  *   the structure of the assembled matrix (one block per distinct coordinate; rows with no contribution are empty;
  *   columns strictly ascending) and the duplicate-summation map in gather form.  Outputs *nnzb.
  *   Errors: BSR_ERR_NULL, BSR_ERR_SHAPE, BSR_ERR_BLOCK, BSR_ERR_STRUCTURE (coordinate out of range), BSR_ERR_LIMIT
@@ -237,6 +239,11 @@ int bcoo_structure(bcoo_plan_t plan, int32_t* d_rowptr, int32_t* d_colidx, void*
 int bcoo_set_values(bcoo_plan_t plan, const double* d_stream, double* d_vals, void* stream);
 int bcoo_get_info(bcoo_plan_t plan, int64_t* n_contrib, int64_t* nnzb, int64_t* algorithmic_bytes);
 int bcoo_destroy(bcoo_plan_t plan);
+/* d_dst block t = d_src block d_idx[t], t = 0..n-1, blocks of bs doubles (HOT, one kernel): packs the entries of a
+ * vector (bs = block size) or whole matrix blocks (bs = bs_r*bs_c) that a neighbouring rank needs -- the device-side
+ * staging of the halo / P_oth exchange ("the block payload is staged and exchanged directly from device
+ * memory").  Errors: BSR_ERR_NULL, BSR_ERR_SHAPE, BSR_ERR_LIMIT, BSR_ERR_CUDA. */
+int bsr_gather_blocks(int64_t n, const int32_t* d_idx, int32_t bs, const double* d_src, double* d_dst, void* stream);
 /* Finite-element driver of the primitive ("finite-element assembly the natural next application"): Q1
  * elasticity on the uniform grid of ne elements per side (d = 2 or 3), elements [e0, e1) in ascending order, 4^d
  * contributions (a, b) per element, a slowest; local node a sits at offset bit k of a in direction k.

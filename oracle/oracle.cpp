@@ -472,12 +472,14 @@ int orc_prolongator_smooth(const orc_bsr* Ap, const orc_bsr* Ptp, double omega, 
 // the caller declares once the (block row, block column) coordinate of every contribution,
 // duplicates included; the matrix has one block per distinct coordinate (rows in order, columns strictly ascending);
 // every numeric assembly sums, per destination block, the dense bs_r x bs_c blocks of the value stream that carry
-// its coordinate.  orc_bcoo_structure: pass colidx = null to count.  Returns nnzb, or -1 on a coordinate out of range.
+// its coordinate.  A contribution with a negative coordinate is ignored.  orc_bcoo_structure: pass colidx = null to
+// count.  Returns nnzb, or -1 on a coordinate out of range.
 int64_t orc_bcoo_structure(int64_t n, const int32_t* brow, const int32_t* bcol, int32_t nbrows, int32_t nbcols,
                            int32_t* rowptr, int32_t* colidx) {
   std::vector<std::vector<int32_t>> rows((size_t)nbrows);
   for (int64_t c = 0; c < n; ++c) {
-    if (brow[c] < 0 || brow[c] >= nbrows || bcol[c] < 0 || bcol[c] >= nbcols) return -1;
+    if (brow[c] < 0 || bcol[c] < 0) continue;   // declared but ignored (the COO convention for entries not owned)
+    if (brow[c] >= nbrows || bcol[c] >= nbcols) return -1;
     rows[(size_t)brow[c]].push_back(bcol[c]);
   }
   int64_t nnzb = 0;
@@ -501,6 +503,7 @@ int orc_bcoo_sum(int64_t n, const int32_t* brow, const int32_t* bcol, const doub
   const int64_t nnzb = rowptr[nbrows];
   std::vector<ld> acc((size_t)nnzb * bb, 0.0L);
   for (int64_t c = 0; c < n; ++c) {
+    if (brow[c] < 0 || bcol[c] < 0) continue;
     const int32_t* lo = colidx + rowptr[brow[c]];
     const int32_t* hi = colidx + rowptr[brow[c] + 1];
     const int32_t* it = std::lower_bound(lo, hi, bcol[c]);

@@ -68,6 +68,7 @@ SYMBOLS = {
     "bcoo_set_values": (C.c_int, [_V, _V, _V, _V]),
     "bcoo_get_info": (C.c_int, [_V, _PI64, _PI64, _PI64]),
     "bcoo_destroy": (C.c_int, [_V]),
+    "bsr_gather_blocks": (C.c_int, [_I64, _V, _I32, _V, _V, _V]),
     "fem_q1_element_coords": (C.c_int, [_I32, _I32, _I64, _I64, _V, _V, _V]),
     "fem_q1_element_blocks": (C.c_int, [_I32, _I32, _I64, _I64, _V, _V, _I32, _V, _V]),
 }
@@ -382,6 +383,17 @@ class BcooPlan:
 
     def matrix(self, vals) -> Bsr:
         return Bsr(self.nbrows, self.nbcols, self.bs_r, self.bs_c, self.rowptr, self.colidx, vals)
+
+
+def gather_blocks(idx, bs: int, src, dst=None):
+    """dst block t = src block idx[t] (bsr_gather_blocks): device-side packing for the halo / P_oth exchange."""
+    import torch
+    n = int(idx.numel())
+    if dst is None:
+        dst = torch.empty(n * bs, dtype=torch.float64, device=src.device)
+    assert idx.dtype == torch.int32 and dst.numel() == n * bs
+    _check(lib().bsr_gather_blocks(n, _dev(idx), bs, _dev(src), _dev(dst), _stream()))
+    return dst
 
 
 def fem_q1_coords(d: int, ne: int, e0: int, e1: int, device="cuda"):

@@ -51,6 +51,16 @@ bcoo_sum_kernel(int64_t nvals, const int32_t* __restrict__ segptr, const int32_t
   vals[t] = s;
 }
 
+// dst block t = src block idx[t] (bs doubles each): packs halo entries / prolongator rows for an exchange
+__global__ void __launch_bounds__(256)
+gather_blocks_kernel(int64_t nvals, int bs, const int32_t* __restrict__ idx, const double* __restrict__ src,
+                     double* __restrict__ dst) {
+  const int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= nvals) return;
+  const int64_t b = t / bs;
+  dst[t] = __ldg(src + (int64_t)__ldg(idx + b) * bs + (t - b * bs));
+}
+
 // ---- Q1 elasticity driver: element e = ex + ne*(ey + ne*ez), local node a has offset bit k of a in direction k
 __device__ __forceinline__ void q1_nodes(int d, int ne, int64_t e, int a, int b, int& ia, int& ib, int (&ca)[3], int (&cb)[3]) {
   const int n = ne + 1;
@@ -134,16 +144,20 @@ int bcoo_plan_create(bcoo_plan_t* out, int64_t n, const int32_t* d_brow, const i
   // counting sort of the contributions by block row (stable: declaration order inside a row)
   std::vector<int64_t> rstart((size_t)nbrows + 1, 0);
   int bad = 0;
+  int64_t nkept = 0;   // a contribution with a negative coordinate is declared but ignored (the COO convention)
   for (int64_t c = 0; c < n; ++c) {
-    if (br[(size_t)c] < 0 || br[(size_t)c] >= nbrows || bc[(size_t)c] < 0 || bc[(size_t)c] >= nbcols) { bad = 1; break; }
+    if (br[(size_t)c] < 0 || bc[(size_t)c] < 0) continue;
+    if (br[(size_t)c] >= nbrows || bc[(size_t)c] >= nbcols) { bad = 1; break; }
     rstart[(size_t)br[(size_t)c] + 1]++;
+    ++nkept;
   }
   if (bad) return fail(BSR_ERR_STRUCTURE, "block coordinate out of range");
   for (int32_t i = 0; i < nbrows; ++i) rstart[(size_t)i + 1] += rstart[(size_t)i];
-  std::vector<int32_t> byrow((size_t)n);
+  std::vector<int32_t> byrow((size_t)nkept);
   {
     std::vector<int64_t> fill(rstart.begin(), rstart.end() - 1);
-    for (int64_t c = 0; c < n; ++c) byrow[(size_t)fill[(size_t)br[(size_t)c]]++] = (int32_t)c;
+    for (int64_t c = 0; c < n; ++c)
+      if (br[(size_t)c] >= 0 && bc[(size_t)c] >= 0) byrow[(size_t)fill[(size_t)br[(size_t)c]]++] = (int32_t)c;
   }
   // inside each row: order by (column, declaration index); distinct columns become the row's blocks
   std::vector<int32_t> nblk((size_t)nbrows, 0);
@@ -162,7 +176,7 @@ int bcoo_plan_create(bcoo_plan_t* out, int64_t n, const int32_t* d_brow, const i
   for (int32_t i = 0; i < nbrows; ++i) { nnzb += nblk[(size_t)i]; rowptr[(size_t)i + 1] = (int32_t)nnzb; }
   if (nnzb * bs_r * bs_c >= (1LL << 31)) return fail(BSR_ERR_LIMIT, "the assembled matrix has 2^31 or more values");
   std::vector<int32_t> colidx((size_t)nnzb), segptr((size_t)nnzb + 1);
-  segptr[(size_t)nnzb] = (int32_t)n;
+  segptr[(size_t)nnzb] = (int32_t)nkept;
 #pragma omp parallel for schedule(dynamic, 1024)
   for (int32_t i = 0; i < nbrows; ++i) {
     int32_t s = rowptr[(size_t)i];
@@ -232,6 +246,16 @@ int bcoo_destroy(bcoo_plan_t pl) {
   if (!pl) return BSR_OK;
   if (pl->magic != BCOO_MAGIC) return fail(BSR_ERR_NULL, "invalid plan handle");
   bcoo_release(pl);
+  return BSR_OK;
+}
+
+int bsr_gather_blocks(int64_t n, const int32_t* d_idx, int32_t bs, const double* d_src, double* d_dst, void* stream) {
+  if (n < 0 || bs < 1) return fail(BSR_ERR_SHAPE, "bsr_gather_blocks: bad size");
+  if (n == 0) return BSR_OK;
+  if (!d_idx || !d_src || !d_dst) return fail(BSR_ERR_NULL, "bsr_gather_blocks: null array");
+  const int64_t nvals = n * bs;
+  if ((nvals + 255) / 256 >= (1LL << 31)) return fail(BSR_ERR_LIMIT, "too many values for one launch");
+  LAUNCH(gather_blocks_kernel, (unsigned)((nvals + 255) / 256), 256, 0, (cudaStream_t)stream, nvals, (int)bs, d_idx, d_src, d_dst);
   return BSR_OK;
 }
 

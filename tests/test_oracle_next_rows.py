@@ -133,6 +133,20 @@ def test_bcoo_without_duplicates_is_a_permutation():
     assert np.array_equal(M.vals, stream[order])          # bit for bit: nothing is added
 
 
+def test_bcoo_negative_coordinates_are_ignored():
+    rng = np.random.default_rng(8)
+    n, nb = 400, 13
+    brow, bcol = rng.integers(0, nb, n).astype(np.int32), rng.integers(0, nb, n).astype(np.int32)
+    stream = rng.uniform(-1, 1, (n, 2, 3))
+    drop = rng.random(n) < 0.3
+    b2, c2 = brow.copy(), bcol.copy()
+    b2[drop & (np.arange(n) % 2 == 0)] = -1
+    c2[drop & (np.arange(n) % 2 == 1)] = -7
+    M = orc.bcoo_assemble(b2, c2, stream, nb, nb)
+    ref = orc.bcoo_assemble(brow[~drop], bcol[~drop], stream[~drop], nb, nb)
+    assert np.array_equal(M.rowptr, ref.rowptr) and np.array_equal(M.colidx, ref.colidx) and np.array_equal(M.vals, ref.vals)
+
+
 def test_bcoo_rejects_bad_coordinates():
     with pytest.raises(RuntimeError):
         orc.bcoo_assemble(np.array([0, 4], np.int32), np.array([0, 0], np.int32), np.zeros((2, 2, 2)), 3, 3)
