@@ -244,6 +244,10 @@ int bcoo_destroy(bcoo_plan_t plan);
  * staging of the halo / P_oth exchange ("the block payload is staged and exchanged directly from device
  * memory").  Errors: BSR_ERR_NULL, BSR_ERR_SHAPE, BSR_ERR_LIMIT, BSR_ERR_CUDA. */
 int bsr_gather_blocks(int64_t n, const int32_t* d_idx, int32_t bs, const double* d_src, double* d_dst, void* stream);
+/* The reverse: d_dst block d_idx[t] += d_src block t (HOT, one kernel).  d_idx must hold DISTINCT blocks (the owner's
+ * rows a neighbour contributed to, each once): no atomics; contributions of several neighbours are added by
+ * consecutive calls in a fixed order (the "off-process reduce"). */
+int bsr_scatter_add_blocks(int64_t n, const int32_t* d_idx, int32_t bs, const double* d_src, double* d_dst, void* stream);
 /* Finite-element driver of the primitive ("finite-element assembly the natural next application"): Q1
  * elasticity on the uniform grid of ne elements per side (d = 2 or 3), elements [e0, e1) in ascending order, 4^d
  * contributions (a, b) per element, a slowest; local node a sits at offset bit k of a in direction k.

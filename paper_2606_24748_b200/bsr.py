@@ -69,6 +69,7 @@ SYMBOLS = {
     "bcoo_get_info": (C.c_int, [_V, _PI64, _PI64, _PI64]),
     "bcoo_destroy": (C.c_int, [_V]),
     "bsr_gather_blocks": (C.c_int, [_I64, _V, _I32, _V, _V, _V]),
+    "bsr_scatter_add_blocks": (C.c_int, [_I64, _V, _I32, _V, _V, _V]),
     "fem_q1_element_coords": (C.c_int, [_I32, _I32, _I64, _I64, _V, _V, _V]),
     "fem_q1_element_blocks": (C.c_int, [_I32, _I32, _I64, _I64, _V, _V, _I32, _V, _V]),
 }
@@ -393,6 +394,15 @@ def gather_blocks(idx, bs: int, src, dst=None):
         dst = torch.empty(n * bs, dtype=torch.float64, device=src.device)
     assert idx.dtype == torch.int32 and dst.numel() == n * bs
     _check(lib().bsr_gather_blocks(n, _dev(idx), bs, _dev(src), _dev(dst), _stream()))
+    return dst
+
+
+def scatter_add_blocks(idx, bs: int, src, dst):
+    """dst block idx[t] += src block t, idx distinct (bsr_scatter_add_blocks): the owner's side of the reduce."""
+    import torch
+    n = int(idx.numel())
+    assert idx.dtype == torch.int32 and src.numel() == n * bs
+    _check(lib().bsr_scatter_add_blocks(n, _dev(idx), bs, _dev(src), _dev(dst), _stream()))
     return dst
 
 

@@ -61,6 +61,16 @@ gather_blocks_kernel(int64_t nvals, int bs, const int32_t* __restrict__ idx, con
   dst[t] = __ldg(src + (int64_t)__ldg(idx + b) * bs + (t - b * bs));
 }
 
+// dst block idx[t] += src block t (idx holds distinct blocks: no two threads touch the same value, no atomics)
+__global__ void __launch_bounds__(256)
+scatter_add_blocks_kernel(int64_t nvals, int bs, const int32_t* __restrict__ idx, const double* __restrict__ src,
+                          double* __restrict__ dst) {
+  const int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= nvals) return;
+  const int64_t b = t / bs;
+  dst[(int64_t)__ldg(idx + b) * bs + (t - b * bs)] += __ldg(src + t);
+}
+
 // ---- Q1 elasticity driver: element e = ex + ne*(ey + ne*ez), local node a has offset bit k of a in direction k
 __device__ __forceinline__ void q1_nodes(int d, int ne, int64_t e, int a, int b, int& ia, int& ib, int (&ca)[3], int (&cb)[3]) {
   const int n = ne + 1;
@@ -256,6 +266,16 @@ int bsr_gather_blocks(int64_t n, const int32_t* d_idx, int32_t bs, const double*
   const int64_t nvals = n * bs;
   if ((nvals + 255) / 256 >= (1LL << 31)) return fail(BSR_ERR_LIMIT, "too many values for one launch");
   LAUNCH(gather_blocks_kernel, (unsigned)((nvals + 255) / 256), 256, 0, (cudaStream_t)stream, nvals, (int)bs, d_idx, d_src, d_dst);
+  return BSR_OK;
+}
+
+int bsr_scatter_add_blocks(int64_t n, const int32_t* d_idx, int32_t bs, const double* d_src, double* d_dst, void* stream) {
+  if (n < 0 || bs < 1) return fail(BSR_ERR_SHAPE, "bsr_scatter_add_blocks: bad size");
+  if (n == 0) return BSR_OK;
+  if (!d_idx || !d_src || !d_dst) return fail(BSR_ERR_NULL, "bsr_scatter_add_blocks: null array");
+  const int64_t nvals = n * bs;
+  if ((nvals + 255) / 256 >= (1LL << 31)) return fail(BSR_ERR_LIMIT, "too many values for one launch");
+  LAUNCH(scatter_add_blocks_kernel, (unsigned)((nvals + 255) / 256), 256, 0, (cudaStream_t)stream, nvals, (int)bs, d_idx, d_src, d_dst);
   return BSR_OK;
 }
 

@@ -62,6 +62,24 @@ __device__ __forceinline__ void bulk_g2s(void* dst_smem, const void* src, unsign
 }
 __device__ __forceinline__ void fence_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 
+}  // namespace bsramg
+namespace bsramg {
+// cold: opts `kern` in to the device's largest dynamic shared memory size.  The attribute belongs to the kernel, not
+// to a plan: it is always raised to the device limit, so that plans of different sizes (or built on different
+// threads) never lower it for one another; what a launch uses is the plan's own size.
+template <typename K>
+static int optin_shared_memory(K kern, int64_t need) {
+  int dev = 0, lim = 0;
+  CUDA_TRY(cudaGetDevice(&dev));
+  CUDA_TRY(cudaDeviceGetAttribute(&lim, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev));
+  cudaFuncAttributes fa;
+  CUDA_TRY(cudaFuncGetAttributes(&fa, kern));
+  lim -= (int)fa.sharedSizeBytes;   // the limit covers static + dynamic shared memory
+  if (need > lim) return fail(BSR_ERR_LIMIT, "a brick needs %lld bytes of shared memory, the device offers %d", (long long)need, lim);
+  CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, lim));
+  return BSR_OK;
+}
+
 template <int NE>
 __device__ __forceinline__ void lds_block(const double* __restrict__ p, double (&v)[NE]) {  // p 16-byte aligned if NE even
   if (NE % 2 == 0) {
@@ -268,18 +286,12 @@ static int stream_launch_mkn(const StreamArgs& a, bool persist, int64_t nbricks,
                              bool prepare) {
   if (persist) {
     auto kern = stream_product_kernel<M, K, N, STREAM_THREADS_PERSIST, true>;
-    if (prepare) {
-      CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-      return BSR_OK;
-    }
+    if (prepare) return optin_shared_memory(kern, smem);
     if (nbricks == 0) return BSR_OK;
     LAUNCH(kern, (unsigned)nbricks, STREAM_THREADS_PERSIST, (size_t)smem, st, a);
   } else {
     auto kern = stream_product_kernel<M, K, N, STREAM_THREADS_DIRECT, false>;
-    if (prepare) {
-      CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-      return BSR_OK;
-    }
+    if (prepare) return optin_shared_memory(kern, smem);
     if (nbricks == 0) return BSR_OK;
     LAUNCH(kern, (unsigned)nbricks, STREAM_THREADS_DIRECT, (size_t)smem, st, a);
   }
@@ -289,10 +301,7 @@ static int stream_launch_mkn(const StreamArgs& a, bool persist, int64_t nbricks,
 template <int M, int N>
 static int stream_launch_smooth_mn(const StreamArgs& a, int64_t nbricks, int64_t smem, cudaStream_t st, bool prepare) {
   auto kern = stream_product_kernel<M, M, N, STREAM_THREADS_DIRECT, false, 1>;
-  if (prepare) {
-    CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    return BSR_OK;
-  }
+  if (prepare) return optin_shared_memory(kern, smem);
   if (nbricks == 0) return BSR_OK;
   LAUNCH(kern, (unsigned)nbricks, STREAM_THREADS_DIRECT, (size_t)smem, st, a);
   return BSR_OK;

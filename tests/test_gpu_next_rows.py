@@ -349,3 +349,34 @@ def test_second_workload_hot_path(bsr, kind, small):
     # prolongator smoothing on the same operator (P rows of up to 27 blocks for Q2)
     sm, _, _, pv, ref = smooth_check(bsr, A, g.P_tent(0), g.level_info(0)["omega"])
     assert np.abs(pv.cpu().numpy().reshape(ref.vals.shape) - P.vals).max() < 1e-13
+
+
+# ------------------------------------------------------------------ f3: row sharding (library kernels per slab)
+@pytest.mark.parametrize("d,ne,world", [(3, 11, 2), (3, 20, 3), (2, 62, 4)])
+def test_row_sharded_hot_path_on_device(bsr, d, ne, world):
+    """The sharded path of paper_2606_24748_b200/shard.py with the LIBRARY as the local kernel provider (bsr_spmv,
+    bsr_gather_blocks, bsr_scatter_add_blocks, ptap_numeric, bcoo_set_values): `world` slabs of one problem driven by
+    one host thread each on this GPU, exchanging through host queues (no kernel waits on another; the NCCL
+    communicator of the multi-GPU launch is covered by the gloo test on the CPU).  Every slab must reproduce its rows
+    of the single-rank oracle results."""
+    import torch
+    from paper_2606_24748_b200 import shard
+    from tests.shard_util import LoopbackWorld, check_shard
+    g = pr.Generator(d, ne, seed=2, modulus_mode=1)
+    g.build_prolongator(0)
+    A, P = g.A(0), g.P(0)
+    agg = g.level_arrays(0)["agg"].copy()
+    x = pr.uniform(2, pr.PURPOSE_FINE, A.nbrows * A.bs_r)
+    xc = pr.uniform(2, pr.PURPOSE_COARSE, P.nbcols * P.bs_c)
+    Ac = orc.ptap(A, P)
+    dev0 = torch.device("cuda", 0)
+
+    def rank(comm):
+        torch.cuda.set_device(0)
+        return check_shard(comm, shard.LibOps(dev0), A, P, agg, x, xc, Ac, to_dev=lambda t: t.to(dev0))
+
+    res = LoopbackWorld(world).run(rank)
+    for r in res:
+        assert r["structure"], r
+        assert max(r["spmv_A"], r["spmv_P"], r["spmv_Pt"], r["ptap"], r["ptap_scaled"]) < 1e-12, r
+        assert r["gate_idle"] == 0 and r["gate_moved"] == 1, r
