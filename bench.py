@@ -219,6 +219,115 @@ def job_value(bytes_per_rank: int, world: int, seconds: float) -> float:
     return bytes_per_rank * world / seconds / 1e9
 
 
+# ------------------------------------------------------------------ strong scaling of ONE problem (row sharding, f3)
+def run_sharded(args) -> dict | None:
+    """`--sharded`: the config's problem is cut into one slab of block rows per GPU (paper_2606_24748_b200/shard.py;
+    PAPER.md:111 "one rank per GPU"); a step is the same hot path, now with its exchanges (x halo, coarse halo,
+    restriction reduce, cut rows of A_c) between NVLink neighbours.  value = the GLOBAL problem's algorithmic bytes
+    over the slowest rank's time: strong scaling.  Each rank generates the whole problem on the host and keeps its
+    slab (stand-in for a distributed assembly)."""
+    import torch
+    import torch.distributed as dist
+    from paper_2606_24748_b200 import bsr, problems as pr, shard
+
+    rank, world, local = rank_env()
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device -- the product path has no CPU fallback")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+    bsr.lib()
+    cfg = args.config
+    seed = pr.CONFIGS[cfg]["seed"]
+    gen, A, P = make_problem(cfg)
+    agg = gen.level_arrays(0)["agg"].copy()
+    comm = shard.DistComm(dev) if world > 1 else shard.SoloComm()
+    sh = shard.RowShard(A, P, agg, comm, shard.LibOps(dev))
+    sh.ptap_symbolic()
+    x = pr.uniform(seed, pr.PURPOSE_FINE, A.nbrows * A.bs_r)
+    xc = pr.uniform(seed, pr.PURPOSE_COARSE, P.nbcols * P.bs_c)
+    x_ext, xc_ext, yc_ext = sh.new_fine_ext(), sh.new_coarse_ext(), sh.new_coarse_ext()
+    sh.fine_local(x_ext).copy_(torch.from_numpy(x[sh.r0 * A.bs_r:sh.r1 * A.bs_r]).to(dev))
+    sh.coarse_local(xc_ext).copy_(torch.from_numpy(xc[sh.c0 * P.bs_c:sh.c1 * P.bs_c]).to(dev))
+    y = torch.empty(sh.nloc * A.bs_r, dtype=torch.float64, device=dev)
+    Rshape = pr.HostBSR(P.nbcols, P.nbrows, P.bs_c, P.bs_r, None, P.colidx, None)
+
+    def allsum(v: int) -> int:
+        if world == 1:
+            return int(v)
+        t = torch.tensor([v], dtype=torch.int64, device=dev)
+        dist.all_reduce(t)
+        return int(t.item())
+
+    # GLOBAL algorithmic bytes (the figures of the single-GPU line): AP and A_c block counts summed over the slabs
+    nnzb_ap = allsum(sh.plan.info()["nnzb_ap"])
+    nnzb_c = allsum(sh.coo.nnzb)
+    bAP = nnzb_ap * (8 * A.bs_r * P.bs_c + 4) + 4 * (A.nbrows + 1)
+    bAc = nnzb_c * (8 * P.bs_c * P.bs_c + 4) + 4 * (P.nbcols + 1)
+    nbytes = {"spmv_A": spmv_bytes(A), "spmv_P": spmv_bytes(P), "spmv_Pt": spmv_bytes(Rshape),
+              "ptap_numeric": bsr_bytes(A) + bsr_bytes(P) + bAP + bsr_bytes(Rshape) + bAP + bAc}
+    names = list(nbytes)
+
+    def step(ev=None):
+        if ev: ev[0].record()
+        sh.spmv_A(x_ext, y)
+        if ev: ev[1].record()
+        sh.spmv_P(xc_ext, y)
+        if ev: ev[2].record()
+        sh.spmv_Pt(sh.fine_local(x_ext), yc_ext)
+        if ev: ev[3].record()
+        sh.ptap_numeric()
+        if ev: ev[4].record()
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+            torch.cuda.synchronize()
+
+    for _ in range(max(args.warmup, 3)):
+        step()
+    evs = [[torch.cuda.Event(enable_timing=True) for _ in range(5)] for _ in range(args.steps)]
+    sampler = ClockSampler(local)
+    sampler.start()
+    barrier()
+    l0, _ = bsr.counters()
+    t0, t1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    t0.record()
+    for k in range(args.steps):
+        step(evs[k])
+    t1.record()
+    barrier()
+    l1, _ = bsr.counters()
+    clocks = sampler.stop()
+    ms_step = max_over_ranks(t0.elapsed_time(t1), world, dev) / args.steps
+    per = {n: max_over_ranks(float(np.median([evs[k][i].elapsed_time(evs[k][i + 1]) for k in range(args.steps)])), world, dev)
+           for i, n in enumerate(names)}
+    sent = {k: allsum(v) for k, v in sh.exchange_bytes().items()}
+    if world > 1:
+        dist.destroy_process_group()
+    if rank != 0:
+        return None
+    peak, peak_src = measured_peak()
+    total = sum(nbytes.values())
+    ops = {n: {"ms": per[n], "GB/s": nbytes[n] / (per[n] * 1e-3) / 1e9, "algorithmic_GB": nbytes[n] / 1e9,
+               "frac_of_measured_hbm_x_gpus": nbytes[n] / (per[n] * 1e-3) / 1e9 / (peak * world)} for n in names}
+    dom = max(names, key=lambda n: per[n])
+    return {"metric": METRIC, "value": total / (ms_step * 1e-3) / 1e9, "unit": "GB/s", "n_gpus": world, "steps": args.steps,
+            "warmup": max(args.warmup, 3), "ms_per_step": ms_step, "higher_is_better": True, "scaling": "strong",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": workload_name(cfg, A, P), "parallelism": f"row slabs x{world} (shard.py)",
+                       "l2": "inputs exceed L2; no flush", "step": "y=Ax, y=Px_c, y=P^T x, ptap_numeric, with their exchanges"},
+            "ops": ops, "exchange_bytes_sent_per_call_all_ranks": sent,
+            "roofline": {"bound": "hbm", "kernel": dom, "achieved": ops[dom]["GB/s"], "peak": peak * world,
+                         "peak_source": peak_src + f" x {world} GPUs", "unit": "GB/s",
+                         "frac": ops[dom]["GB/s"] / (peak * world), "traffic": None},
+            "clocks": clocks, "gpu_launches": int(l1 - l0),
+            "e2e": {"value": None, "unit": "GB/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0,
+                    "note": "the host-buffer leg is measured by the default (replica) mode"}}
+
+
 # ------------------------------------------------------------------ the CUDA arm
 def run_ours(args) -> dict | None:
     import torch
@@ -581,6 +690,8 @@ def main():
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-vcycle", action="store_true", help="skip the config-4 V-cycle timing")
+    ap.add_argument("--sharded", action="store_true", help="strong-scale ONE problem over the ranks (row slabs, "
+                    "paper_2606_24748_b200/shard.py) instead of one independent problem per rank")
     ap.add_argument("--no-second-workload", action="store_true", help="skip the f4 timings (configs 5 and 6)")
     ap.add_argument("--no-next-rows", action="store_true", help="skip the f1 / f2 timings (prolongator smoothing, "
                     "blocked COO assembly)")
@@ -590,7 +701,7 @@ def main():
             return
         print(json.dumps(run_reference(args)), flush=True)
         return
-    out = run_ours(args)
+    out = run_sharded(args) if args.sharded else run_ours(args)
     if out is not None:
         print(json.dumps(out), flush=True)
 

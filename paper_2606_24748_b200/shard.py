@@ -366,6 +366,23 @@ class DistComm:
         return self.exchange_arrays(sends, np.float64)
 
 
+class SoloComm:
+    """World of one rank (no neighbours): every exchange is empty."""
+    rank, world = 0, 1
+
+    def exchange(self, sends, recvs):
+        assert not sends and not recvs
+
+    def exchange_arrays(self, sends, dtype):
+        return {}
+
+    def exchange_ids(self, sends):
+        return {}
+
+    def exchange_host_values(self, sends):
+        return {}
+
+
 class LibOps:
     """The library behind the sharded path: every numeric step is one of libbsramg.so's kernels."""
 
