@@ -1,0 +1,116 @@
+// dense_gemm.cu -- register-tiled fp64 GEMM for the coarsest-level factorisation (vcycle_refresh).
+//
+// The coarsest operator of the V-cycle is "solved dense on device" (BASELINE.json config 4; reading R17):
+// a blocked Cholesky factorisation and the explicit triangular inverse that turns every later solve into two
+// mat-vecs.  Both are built from ONE kernel, C = beta*C + alpha * A * op(B) on 128x128 tiles: 256 threads, an 8x8
+// accumulator tile per thread held as a 4x4 grid of 2x2 patches (so that every shared-memory read is a conflict-free
+// 16-byte load and every global access a coalesced 16-byte one), k in chunks of 8 through shared memory with the next
+// chunk prefetched into registers.  Plain fp64 FMAs: the tensor cores' fp64 rate equals the vector pipe's on this part
+// and the operands here come with triangular structure (k-ranges per tile) rather than tensor-core friendly shapes.
+// All matrices are row-major; m and n multiples of 128, k ranges multiples of 8 (the caller pads).
+#include "internal.h"
+
+namespace bsramg {
+
+constexpr int GT = 128, GK = 8, GS = GT + 4;   // tile, k-chunk, padded shared-memory row (doubles)
+
+template <bool TRANSB>
+__global__ void __launch_bounds__(256)
+dgemm128_kernel(int k, double alpha, const double* __restrict__ A, int64_t lda, const double* __restrict__ B,
+                int64_t ldb, double beta, double* __restrict__ C, int64_t ldc, int64_t sA, int64_t sB, int64_t sC,
+                int tri, int klim) {
+  const int m0 = blockIdx.y * GT, n0 = blockIdx.x * GT;
+  if (tri && n0 > m0) return;                       // lower tiles only
+  A += (int64_t)blockIdx.z * sA; B += (int64_t)blockIdx.z * sB; C += (int64_t)blockIdx.z * sC;
+  int kbeg = 0, kend = k;
+  if (klim == 1) kbeg = min(n0, k);                 // B (k x n) is lower triangular: rows k < n0 of this tile are zero
+  if (klim == 2) kend = min(m0 + GT, k);            // A (m x k) is lower triangular: columns k >= m0+128 are zero
+  __shared__ __align__(16) double As[GK][GS];
+  __shared__ __align__(16) double Bs[GK][GS];
+  const int tid = threadIdx.x, tx = tid & 15, ty = tid >> 4;
+  double acc[4][2][4][2];
+#pragma unroll
+  for (int g = 0; g < 4; ++g)
+#pragma unroll
+    for (int a = 0; a < 2; ++a)
+#pragma unroll
+      for (int h = 0; h < 4; ++h) acc[g][a][h][0] = acc[g][a][h][1] = 0.0;
+  // staging roles: A (and B when TRANSB): row tid/2, four k values at (tid&1)*4;  B (k x n): k row tid/32, four columns
+  const int ar = tid >> 1, ak = (tid & 1) * 4;
+  const int bk = tid >> 5, bc = (tid & 31) * 4;
+  const double* ap = A + (int64_t)(m0 + ar) * lda + ak;
+  const double* bp = TRANSB ? B + (int64_t)(n0 + ar) * ldb + ak : B + (int64_t)bk * ldb + n0 + bc;
+  double2 pa0, pa1, pb0, pb1;
+  auto fetch = [&](int kk) {
+    pa0 = *reinterpret_cast<const double2*>(ap + kk);
+    pa1 = *reinterpret_cast<const double2*>(ap + kk + 2);
+    if (TRANSB) {
+      pb0 = *reinterpret_cast<const double2*>(bp + kk);
+      pb1 = *reinterpret_cast<const double2*>(bp + kk + 2);
+    } else {
+      pb0 = *reinterpret_cast<const double2*>(bp + (int64_t)kk * ldb);
+      pb1 = *reinterpret_cast<const double2*>(bp + (int64_t)kk * ldb + 2);
+    }
+  };
+  if (kbeg < kend) fetch(kbeg);
+  for (int kk = kbeg; kk < kend; kk += GK) {
+    As[ak][ar] = pa0.x; As[ak + 1][ar] = pa0.y; As[ak + 2][ar] = pa1.x; As[ak + 3][ar] = pa1.y;
+    if (TRANSB) {
+      Bs[ak][ar] = pb0.x; Bs[ak + 1][ar] = pb0.y; Bs[ak + 2][ar] = pb1.x; Bs[ak + 3][ar] = pb1.y;
+    } else {
+      *reinterpret_cast<double2*>(&Bs[bk][bc]) = pb0;
+      *reinterpret_cast<double2*>(&Bs[bk][bc + 2]) = pb1;
+    }
+    __syncthreads();
+    if (kk + GK < kend) fetch(kk + GK);             // next chunk in flight while this one is multiplied
+#pragma unroll
+    for (int q = 0; q < GK; ++q) {
+      double2 a2[4], b2[4];
+#pragma unroll
+      for (int g = 0; g < 4; ++g) a2[g] = *reinterpret_cast<const double2*>(&As[q][ty * 2 + 32 * g]);
+#pragma unroll
+      for (int h = 0; h < 4; ++h) b2[h] = *reinterpret_cast<const double2*>(&Bs[q][tx * 2 + 32 * h]);
+#pragma unroll
+      for (int g = 0; g < 4; ++g)
+#pragma unroll
+        for (int h = 0; h < 4; ++h) {
+          acc[g][0][h][0] = fma(a2[g].x, b2[h].x, acc[g][0][h][0]);
+          acc[g][0][h][1] = fma(a2[g].x, b2[h].y, acc[g][0][h][1]);
+          acc[g][1][h][0] = fma(a2[g].y, b2[h].x, acc[g][1][h][0]);
+          acc[g][1][h][1] = fma(a2[g].y, b2[h].y, acc[g][1][h][1]);
+        }
+    }
+    __syncthreads();
+  }
+#pragma unroll
+  for (int g = 0; g < 4; ++g)
+#pragma unroll
+    for (int a = 0; a < 2; ++a) {
+      double* crow = C + (int64_t)(m0 + ty * 2 + 32 * g + a) * ldc + n0 + tx * 2;
+#pragma unroll
+      for (int h = 0; h < 4; ++h) {
+        double2* cp = reinterpret_cast<double2*>(crow + 32 * h);
+        double2 v = make_double2(alpha * acc[g][a][h][0], alpha * acc[g][a][h][1]);
+        if (beta != 0.0) {
+          const double2 o = *cp;
+          v.x = fma(beta, o.x, v.x);
+          v.y = fma(beta, o.y, v.y);
+        }
+        *cp = v;
+      }
+    }
+}
+
+int dgemm128(bool transB, int m, int n, int k, double alpha, const double* A, int64_t lda, const double* B, int64_t ldb,
+             double beta, double* C, int64_t ldc, int batch, int64_t sA, int64_t sB, int64_t sC, int tri, int klim,
+             cudaStream_t st) {
+  if (m <= 0 || n <= 0 || batch <= 0) return BSR_OK;
+  if (m % GT || n % GT || k % GK || (lda & 1) || (ldb & 1) || (ldc & 1))
+    return fail(BSR_ERR_SHAPE, "dgemm128: sizes must be multiples of the tile (m %d n %d k %d)", m, n, k);
+  const dim3 grid((unsigned)(n / GT), (unsigned)(m / GT), (unsigned)batch);
+  if (transB) LAUNCH(dgemm128_kernel<true>, grid, 256, 0, st, k, alpha, A, lda, B, ldb, beta, C, ldc, sA, sB, sC, tri, klim);
+  else LAUNCH(dgemm128_kernel<false>, grid, 256, 0, st, k, alpha, A, lda, B, ldb, beta, C, ldc, sA, sB, sC, tri, klim);
+  return BSR_OK;
+}
+
+}  // namespace bsramg

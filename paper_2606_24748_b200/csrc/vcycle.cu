@@ -9,8 +9,10 @@
 //   k=1..deg-1: r-=A d_{k-1}; rho_k=1/(2 sigma-rho_{k-1}); d_k=rho_k rho_{k-1} d_{k-1}+(2 rho_k/delta) D^-1 r; x+=d_k
 // Every SpMV runs in the blocked kernels of bsr.cu with the vector update fused into its epilogue
 // (r = b - A x, r -= A d, x += P e); D^-1 r and the d/x update are one small kernel.
-// Coarsest level (reading R17): dense Cholesky A = L L^T on the device (blocked, 32x32 tiles), then the
-// explicit triangular inverse L^-1 so that every later solve is two fully parallel triangular mat-vecs.
+// Coarsest level (reading R17): dense Cholesky A = L L^T on the device -- right-looking with 128-wide panels
+// (32x32 tile kernels inside a panel, ONE register-tiled fp64 GEMM, dense_gemm.cu, for every trailing update) -- then
+// the explicit triangular inverse L^-1 by recursive doubling (X21 = -X22 (L21 X11), two batched GEMMs per level), so
+// that every later solve is two fully parallel triangular mat-vecs.
 #include <algorithm>
 #include <cmath>
 
@@ -38,6 +40,7 @@ struct vcycle_s {
   // coarsest level, dense
   int64_t nc = 0, npad = 0;
   double *dense = nullptr, *diaginv = nullptr, *linv = nullptr, *linvT = nullptr, *ytmp = nullptr;
+  int32_t* coarse_rowidx = nullptr;   // block row of every stored block of the coarsest operator (dense fill)
   int* d_status = nullptr;
   // PCG work space
   double *pr = nullptr, *pz = nullptr, *pp = nullptr, *pq = nullptr, *partial = nullptr, *scal = nullptr;
@@ -260,19 +263,21 @@ syrk_tile_kernel(int64_t npad, int j, double* __restrict__ dense) {
   *c -= s;
 }
 
-// X = L^-1, one CTA per tile column j, tile rows in order (each needs the ones above it in the same column):
-//   X_jj = inv(L_jj);  X_ij = -inv(L_ii) * sum_{k=j}^{i-1} L_ik X_kj
+// X = L^-1 of one diagonal block, one CTA per tile column j, tile rows in order (each needs the ones above it in the
+// same column):  X_jj = inv(L_jj);  X_ij = -inv(L_ii) * sum_{k=j}^{i-1} L_ik X_kj
+// restricted to the PANEL x PANEL diagonal blocks (tiles 4J..4J+3 of block J = blockIdx.y): the base case of the
+// recursive-doubling inverse below
+constexpr int PANEL = 128, PT = PANEL / TS;
 __global__ void __launch_bounds__(TS * TS)
-trinv_kernel(int64_t npad, int nb, const double* __restrict__ dense, const double* __restrict__ diaginv,
-             double* linv) {
+trinv_block_kernel(int64_t npad, const double* __restrict__ dense, const double* __restrict__ diaginv, double* linv) {
   __shared__ double a[TS][TS + 1];
   __shared__ double b[TS][TS + 1];
   const int tx = threadIdx.x, ty = threadIdx.y;
-  const int j = blockIdx.x;
+  const int t0 = blockIdx.y * PT, j = t0 + blockIdx.x;
   linv[((int64_t)j * TS + ty) * npad + (int64_t)j * TS + tx] = diaginv[((int64_t)j * TS + ty) * TS + tx];
   __threadfence();
   __syncthreads();
-  for (int i = j + 1; i < nb; ++i) {
+  for (int i = j + 1; i < t0 + PT; ++i) {
     double s = 0.0;
     for (int k = j; k < i; ++k) {
       a[ty][tx] = dense[((int64_t)i * TS + ty) * npad + (int64_t)k * TS + tx];
@@ -318,27 +323,50 @@ trigemv_kernel(int64_t n, int64_t npad, const double* __restrict__ M, const doub
   if (lane == 0) y[i] = s;
 }
 
-static int coarse_factor(vcycle_t vc, const int32_t* rowidx_slot, cudaStream_t st) {
+static int coarse_factor(vcycle_t vc, cudaStream_t st) {
   bsr_t A = vc->L[vc->nlevels - 1].A;
-  const int64_t np = vc->npad;
-  const int nb = (int)(np / TS);
+  const int64_t np = vc->npad;            // a multiple of PANEL
+  const int nb = (int)(np / TS), npan = (int)(np / PANEL);
   CUDA_TRY(cudaMemsetAsync(vc->dense, 0, (size_t)np * np * 8, st));
   CUDA_TRY(cudaMemsetAsync(vc->linv, 0, (size_t)np * np * 8, st));
   if (np > vc->nc) LAUNCH(dense_pad_kernel, (unsigned)((np - vc->nc + 63) / 64), 64, 0, st, vc->nc, np, vc->dense);
   const int64_t nvals = A->nnzb * A->bs_r * A->bs_c;
   if (nvals)
-    LAUNCH(dense_fill_kernel, (unsigned)((nvals + 255) / 256), 256, 0, st, nvals, (int)A->bs_r, rowidx_slot,
+    LAUNCH(dense_fill_kernel, (unsigned)((nvals + 255) / 256), 256, 0, st, nvals, (int)A->bs_r, vc->coarse_rowidx,
            A->d_colidx, A->d_vals, np, vc->dense);
   const dim3 tb(TS, TS);
-  for (int j = 0; j < nb; ++j) {
-    LAUNCH(potrf_tile_kernel, 1, tb, 0, st, np, j, vc->dense, vc->diaginv, vc->d_status);
-    const int rest = nb - j - 1;
-    if (rest > 0) {
-      LAUNCH(trsm_tile_kernel, (unsigned)rest, tb, 0, st, np, j, vc->dense, vc->diaginv);
-      LAUNCH(syrk_tile_kernel, dim3(rest, rest), tb, 0, st, np, j, vc->dense);
+  // ---- A = L L^T, right-looking over 128-wide panels
+  for (int J = 0; J < npan; ++J) {
+    for (int s = 0; s < PT; ++s) {        // the panel itself, 32x32 tiles: factor, solve below, update the panel's own columns
+      const int c = J * PT + s, rest = nb - c - 1, pc = PT - 1 - s;
+      LAUNCH(potrf_tile_kernel, 1, tb, 0, st, np, c, vc->dense, vc->diaginv, vc->d_status);
+      if (rest > 0) LAUNCH(trsm_tile_kernel, (unsigned)rest, tb, 0, st, np, c, vc->dense, vc->diaginv);
+      if (rest > 0 && pc > 0) LAUNCH(syrk_tile_kernel, dim3(pc, rest), tb, 0, st, np, c, vc->dense);
+    }
+    const int64_t r0 = (int64_t)(J + 1) * PANEL;
+    const int m = (int)(np - r0);
+    if (m > 0) {                          // trailing update: one GEMM over the lower tiles, k = the panel
+      const double* Lp = vc->dense + r0 * np + (int64_t)J * PANEL;
+      BSR_TRY(dgemm128(true, m, m, PANEL, -1.0, Lp, np, Lp, np, 1.0, vc->dense + r0 * np + r0, np, 1, 0, 0, 0, 1, 0, st));
     }
   }
-  LAUNCH(trinv_kernel, (unsigned)nb, tb, 0, st, np, nb, vc->dense, vc->diaginv, vc->linv);
+  // ---- X = L^-1: the diagonal 128-blocks by the tile recurrence, then doubling: for the pair (X11, X22) of two
+  // consecutive inverted blocks of size b, X21 = -X22 (L21 X11); linvT is the workspace for L21 X11
+  LAUNCH(trinv_block_kernel, dim3(PT, npan), tb, 0, st, np, vc->dense, vc->diaginv, vc->linv);
+  for (int64_t b = PANEL; b < np; b *= 2) {
+    const int64_t step = 2 * b;
+    const int nfull = (int)(np / step);                       // pairs with a full second block
+    const int64_t rem = np - (int64_t)nfull * step;           // a last pair with a shorter second block, if rem > b
+    auto pair = [&](int64_t r0, int64_t b2, int batch) -> int {
+      const int64_t o21 = (r0 + b) * np + r0, o11 = r0 * np + r0, o22 = (r0 + b) * np + (r0 + b), sp = step * np + step;
+      BSR_TRY(dgemm128(false, (int)b2, (int)b, (int)b, 1.0, vc->dense + o21, np, vc->linv + o11, np, 0.0, vc->linvT + o21, np,
+                       batch, sp, sp, sp, 0, 1, st));
+      return dgemm128(false, (int)b2, (int)b, (int)b2, -1.0, vc->linv + o22, np, vc->linvT + o21, np, 0.0, vc->linv + o21, np,
+                      batch, sp, sp, sp, 0, 2, st);
+    };
+    if (nfull > 0) BSR_TRY(pair(0, b, nfull));
+    if (rem > b) BSR_TRY(pair((int64_t)nfull * step, rem - b, 1));
+  }
   LAUNCH(transpose_tile_kernel, dim3(nb, nb), tb, 0, st, np, vc->linv, vc->linvT);
   return BSR_OK;
 }
@@ -429,7 +457,7 @@ static void vc_release(vcycle_t vc) {
   if (!vc) return;
   for (auto& lv : vc->L) { dev_free(lv.Dinv); dev_free(lv.r); dev_free(lv.d); dev_free(lv.b); dev_free(lv.x); }
   dev_free(vc->dense); dev_free(vc->diaginv); dev_free(vc->linv); dev_free(vc->linvT); dev_free(vc->ytmp);
-  dev_free(vc->d_status); dev_free(vc->pr); dev_free(vc->pz); dev_free(vc->pp); dev_free(vc->pq);
+  dev_free(vc->coarse_rowidx); dev_free(vc->d_status); dev_free(vc->pr); dev_free(vc->pz); dev_free(vc->pp); dev_free(vc->pq);
   dev_free(vc->partial); dev_free(vc->scal);
   vc->magic = 0;
   delete vc;
@@ -452,7 +480,8 @@ int vcycle_refresh(vcycle_t vc, void* stream) {
     BSR_TRY(launch_dinv(vc->L[l], vc->d_status, st));
     BSR_TRY(transpose_ensure(vc->L[l].P, st));
   }
-  return coarse_factor(vc, reinterpret_cast<const int32_t*>(vc->L[vc->nlevels - 1].Dinv), st);
+  NvtxRange nv("vcycle_refresh");
+  return coarse_factor(vc, st);
 }
 
 int vcycle_status(vcycle_t vc, void* stream) {
@@ -508,8 +537,8 @@ int vcycle_create(vcycle_t* out, int32_t nlevels, const bsr_t* A, const bsr_t* P
     }
   }
   vc->nc = nc;
-  vc->npad = ((nc + TS - 1) / TS) * TS;
-  if (vc->npad == 0) vc->npad = TS;
+  vc->npad = ((nc + PANEL - 1) / PANEL) * PANEL;   // whole 128-wide panels (rows / columns >= nc carry the identity)
+  if (vc->npad == 0) vc->npad = PANEL;
   const size_t np2 = (size_t)vc->npad * vc->npad;
   if (rc == BSR_OK) rc = dev_alloc_t(&vc->dense, np2);
   if (rc == BSR_OK) rc = dev_alloc_t(&vc->linv, np2);
@@ -525,14 +554,11 @@ int vcycle_create(vcycle_t* out, int32_t nlevels, const bsr_t* A, const bsr_t* P
   if (rc == BSR_OK) rc = dev_alloc_t(&vc->partial, (size_t)DOT_BLOCKS);
   if (rc == BSR_OK) rc = dev_alloc_t(&vc->scal, 8);
   if (rc == BSR_OK) {
-    // block row of every stored block of the coarsest operator (for the dense fill); kept in the coarsest
-    // level's otherwise unused Dinv slot
+    // block row of every stored block of the coarsest operator (for the dense fill)
     std::vector<int32_t> rowidx((size_t)Ac->nnzb);
     for (int32_t i = 0; i < Ac->nbrows; ++i)
       for (int32_t k = Ac->h_rowptr[i]; k < Ac->h_rowptr[(size_t)i + 1]; ++k) rowidx[(size_t)k] = i;
-    int32_t* d = nullptr;
-    rc = upload(&d, rowidx, st);
-    vc->L[nlevels - 1].Dinv = reinterpret_cast<double*>(d);
+    rc = upload(&vc->coarse_rowidx, rowidx, st);
     if (rc == BSR_OK && cudaStreamSynchronize(st) != cudaSuccess) rc = fail(BSR_ERR_CUDA, "upload failed");
   }
   if (rc == BSR_OK) {
@@ -551,6 +577,7 @@ int vcycle_create(vcycle_t* out, int32_t nlevels, const bsr_t* A, const bsr_t* P
 int vcycle_apply(vcycle_t vc, const double* d_b, double* d_x, void* stream) {
   if (!vc_ok(vc)) return fail(BSR_ERR_NULL, "invalid vcycle handle");
   if (!d_b || !d_x) return fail(BSR_ERR_NULL, "null vector");
+  NvtxRange nv("vcycle_apply");
   return cycle(vc, 0, d_b, d_x, (cudaStream_t)stream);
 }
 
