@@ -4,15 +4,15 @@
 // a blocked Cholesky factorisation and the explicit triangular inverse that turns every later solve into two
 // mat-vecs.  Both are built from ONE kernel, C = beta*C + alpha * A * op(B) on 128x128 tiles: 256 threads, an 8x8
 // accumulator tile per thread held as a 4x4 grid of 2x2 patches (so that every shared-memory read is a conflict-free
-// 16-byte load and every global access a coalesced 16-byte one), k in chunks of 8 through shared memory with the next
+// 16-byte load and every global access a coalesced 16-byte one), k in chunks of 16 through shared memory with the next
 // chunk prefetched into registers.  Plain fp64 FMAs: the tensor cores' fp64 rate equals the vector pipe's on this part
 // and the operands here come with triangular structure (k-ranges per tile) rather than tensor-core friendly shapes.
-// All matrices are row-major; m and n multiples of 128, k ranges multiples of 8 (the caller pads).
+// All matrices are row-major; m and n multiples of 128, k ranges multiples of 16 (the caller pads).
 #include "internal.h"
 
 namespace bsramg {
 
-constexpr int GT = 128, GK = 8, GS = GT + 4;   // tile, k-chunk, padded shared-memory row (doubles)
+constexpr int GT = 128, GK = 16, GS = GT + 4;   // tile, k-chunk, padded shared-memory row (doubles)
 
 template <bool TRANSB>
 __global__ void __launch_bounds__(256)
@@ -35,31 +35,38 @@ dgemm128_kernel(int k, double alpha, const double* __restrict__ A, int64_t lda, 
     for (int a = 0; a < 2; ++a)
 #pragma unroll
       for (int h = 0; h < 4; ++h) acc[g][a][h][0] = acc[g][a][h][1] = 0.0;
-  // staging roles: A (and B when TRANSB): row tid/2, four k values at (tid&1)*4;  B (k x n): k row tid/32, four columns
-  const int ar = tid >> 1, ak = (tid & 1) * 4;
+  // staging roles: A (and B when TRANSB): row tid/2, eight k values at (tid&1)*8;  B (k x n): k rows tid/32 and
+  // tid/32 + 8, four columns each
+  const int ar = tid >> 1, ak = (tid & 1) * 8;
   const int bk = tid >> 5, bc = (tid & 31) * 4;
   const double* ap = A + (int64_t)(m0 + ar) * lda + ak;
   const double* bp = TRANSB ? B + (int64_t)(n0 + ar) * ldb + ak : B + (int64_t)bk * ldb + n0 + bc;
-  double2 pa0, pa1, pb0, pb1;
+  double2 pa[4], pb[4];
   auto fetch = [&](int kk) {
-    pa0 = *reinterpret_cast<const double2*>(ap + kk);
-    pa1 = *reinterpret_cast<const double2*>(ap + kk + 2);
+#pragma unroll
+    for (int u = 0; u < 4; ++u) pa[u] = *reinterpret_cast<const double2*>(ap + kk + 2 * u);
     if (TRANSB) {
-      pb0 = *reinterpret_cast<const double2*>(bp + kk);
-      pb1 = *reinterpret_cast<const double2*>(bp + kk + 2);
+#pragma unroll
+      for (int u = 0; u < 4; ++u) pb[u] = *reinterpret_cast<const double2*>(bp + kk + 2 * u);
     } else {
-      pb0 = *reinterpret_cast<const double2*>(bp + (int64_t)kk * ldb);
-      pb1 = *reinterpret_cast<const double2*>(bp + (int64_t)kk * ldb + 2);
+      pb[0] = *reinterpret_cast<const double2*>(bp + (int64_t)kk * ldb);
+      pb[1] = *reinterpret_cast<const double2*>(bp + (int64_t)kk * ldb + 2);
+      pb[2] = *reinterpret_cast<const double2*>(bp + (int64_t)(kk + 8) * ldb);
+      pb[3] = *reinterpret_cast<const double2*>(bp + (int64_t)(kk + 8) * ldb + 2);
     }
   };
   if (kbeg < kend) fetch(kbeg);
   for (int kk = kbeg; kk < kend; kk += GK) {
-    As[ak][ar] = pa0.x; As[ak + 1][ar] = pa0.y; As[ak + 2][ar] = pa1.x; As[ak + 3][ar] = pa1.y;
+#pragma unroll
+    for (int u = 0; u < 4; ++u) { As[ak + 2 * u][ar] = pa[u].x; As[ak + 2 * u + 1][ar] = pa[u].y; }
     if (TRANSB) {
-      Bs[ak][ar] = pb0.x; Bs[ak + 1][ar] = pb0.y; Bs[ak + 2][ar] = pb1.x; Bs[ak + 3][ar] = pb1.y;
+#pragma unroll
+      for (int u = 0; u < 4; ++u) { Bs[ak + 2 * u][ar] = pb[u].x; Bs[ak + 2 * u + 1][ar] = pb[u].y; }
     } else {
-      *reinterpret_cast<double2*>(&Bs[bk][bc]) = pb0;
-      *reinterpret_cast<double2*>(&Bs[bk][bc + 2]) = pb1;
+      *reinterpret_cast<double2*>(&Bs[bk][bc]) = pb[0];
+      *reinterpret_cast<double2*>(&Bs[bk][bc + 2]) = pb[1];
+      *reinterpret_cast<double2*>(&Bs[bk + 8][bc]) = pb[2];
+      *reinterpret_cast<double2*>(&Bs[bk + 8][bc + 2]) = pb[3];
     }
     __syncthreads();
     if (kk + GK < kend) fetch(kk + GK);             // next chunk in flight while this one is multiplied

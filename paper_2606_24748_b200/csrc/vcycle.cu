@@ -198,8 +198,10 @@ potrf_tile_kernel(int64_t npad, int j, double* __restrict__ dense, double* __res
   const int tx = threadIdx.x, ty = threadIdx.y;
   double* tile = dense + ((int64_t)j * TS) * npad + (int64_t)j * TS;
   a[ty][tx] = tile[(int64_t)ty * npad + tx];
-  inv[ty][tx] = 0.0;
+  inv[ty][tx] = (tx == ty) ? 1.0 : 0.0;
   __syncthreads();
+  // right-looking Cholesky of the tile and, with the same column of L as soon as it is final, forward substitution of
+  // the identity (X <- L^-1): every step updates the whole trailing part of both with all 1024 threads
   for (int k = 0; k < TS; ++k) {
     if (tx == k && ty == k) {
       double p = a[k][k];
@@ -207,22 +209,18 @@ potrf_tile_kernel(int64_t npad, int j, double* __restrict__ dense, double* __res
       a[k][k] = sqrt(p);
     }
     __syncthreads();
-    if (tx == k && ty > k) a[ty][k] /= a[k][k];
+    const double d = a[k][k];
+    if (tx == k && ty > k) a[ty][k] /= d;
+    if (ty == k && tx <= k) inv[k][tx] /= d;
     __syncthreads();
-    if (tx > k && ty >= tx) a[ty][tx] = fma(-a[ty][k], a[tx][k], a[ty][tx]);
+    if (ty > k) {
+      const double l = a[ty][k];
+      if (tx > k && ty >= tx) a[ty][tx] = fma(-l, a[tx][k], a[ty][tx]);
+      if (tx <= k) inv[ty][tx] = fma(-l, inv[k][tx], inv[ty][tx]);
+    }
     __syncthreads();
   }
   if (tx > ty) a[ty][tx] = 0.0;
-  __syncthreads();
-  if (ty == 0) {  // column tx of the inverse by forward substitution
-    const int c = tx;
-    inv[c][c] = 1.0 / a[c][c];
-    for (int r = c + 1; r < TS; ++r) {
-      double s = 0.0;
-      for (int k = c; k < r; ++k) s = fma(a[r][k], inv[k][c], s);
-      inv[r][c] = -s / a[r][r];
-    }
-  }
   __syncthreads();
   tile[(int64_t)ty * npad + tx] = a[ty][tx];
   diaginv[((int64_t)j * TS + ty) * TS + tx] = inv[ty][tx];
