@@ -165,24 +165,30 @@ static const uint64_t BSR_MAGIC = 0x425352414d473031ull;
 // segmented scatter of SURVEY.md 8(a) a7.
 namespace bsramg {
 
-struct StreamEntry {   // 16 bytes: one X row piece inside a pass
-  int32_t out;         // first slot of C's row (direct) / first accumulator of the row (persist)
+struct StreamEntry {   // 16 bytes: the lanes of one X row piece inside a pass, all in ONE window of the row's slots
+  int32_t out;         // first C slot of the window (direct); unused (persist: the brick header carries it)
   int32_t xbase;       // staged X block index of the piece's first block
-  int32_t len;         // number of X blocks (steps)
-  uint8_t lane0;       // first lane of this entry in the warp
-  uint8_t nslots;      // output blocks of the row held by this entry's lanes
-  uint8_t slot0;       // first of them inside the row (a row's blocks may be split over two passes)
-  uint8_t pad1;
+  int32_t mbase;       // staged meta index of the piece's first block FOR THIS WINDOW
+  uint32_t packed;     // len (16 bits: X blocks = steps) | lane0 (5) | nslots-1 (5) | slot0 inside the window (5)
+  static uint32_t pack(int len, int lane0, int nslots, int slot0) {
+    return (uint32_t)len | ((uint32_t)lane0 << 16) | ((uint32_t)(nslots - 1) << 21) | ((uint32_t)slot0 << 26);
+  }
+  __host__ __device__ int len() const { return (int)(packed & 0xffffu); }
+  __host__ __device__ int lane0() const { return (int)((packed >> 16) & 31u); }
+  __host__ __device__ int nslots() const { return (int)((packed >> 21) & 31u) + 1; }
+  __host__ __device__ int slot0() const { return (int)((packed >> 26) & 31u); }
 };
 struct StreamPass { int32_t e0, e1, steps, pad; };   // entries [e0, e1) (relative to the chunk), max len
-struct StreamMeta { uint32_t mask, ybase; };          // per staged X block: receiving slots, staged Y row start
+struct StreamMeta { uint32_t mask, ybase; };          // per (staged X block, window): receiving slots of the window and
+                                                      // the staged Y block of the first of them
 struct StreamRun { int32_t src, n, dst; };            // copy n blocks from global block src to staged block dst
 struct StreamBrickHdr { int32_t chunk0, nchunks, out, nslots; };   // out / nslots: persist bricks (C row of the brick)
 struct StreamChunkHdr {   // 64 bytes: everything a CTA needs to know about a chunk, fetched with one load
   int64_t meta0;          // first staged X block in StreamPlan::meta
-  int32_t nx, ny;         // staged X blocks (even, padded) and Y blocks
+  int32_t nx, ny;         // staged X blocks and Y blocks
   int32_t ent0, nent, pass0, npass, xr0, nxr, yr0, nyr;
-  int32_t pad[4];
+  int32_t nmeta;          // staged metas (even, padded): one per X block and window of its row
+  int32_t pad[3];
 };
 static_assert(sizeof(StreamChunkHdr) == 64 && sizeof(StreamBrickHdr) == 16, "headers are fetched with 16-byte loads");
 
@@ -204,12 +210,16 @@ struct StreamPlan {
 
 struct StreamShape { int M, K, N; };   // C blocks M x N, X blocks M x K, Y blocks K x N
 inline int stream_xs(int M, int K) { return (M * K + 1) & ~1; }   // staged X block stride in doubles (16-byte rows)
-int64_t stream_smem_bytes(const StreamShape& sh, int64_t nx, int64_t ny, int64_t nentries, int64_t npasses);
+int64_t stream_smem_bytes(const StreamShape& sh, int64_t nx, int64_t nmeta, int64_t ny, int64_t nentries, int64_t npasses);
 
 // piece of an X row: blocks [t0, t1) of row `row`
 struct StreamPiece { int32_t row, t0, t1; };
 struct StreamChunkDef { std::vector<StreamPiece> pieces; };
-struct StreamBrickDef { std::vector<StreamChunkDef> chunks; bool direct = true; };
+struct StreamBrickDef {
+  std::vector<StreamChunkDef> chunks;
+  bool direct = true;
+  int32_t s0 = 0, s1 = 0;   // persist bricks: the window [s0, s1) of the C row's slots this brick computes (at most 32)
+};
 
 // builds the flat plan of C = X*Y for the given bricks.  pairptr/off_x: per C slot the ordered products (HostPlan).
 void stream_build(const StreamShape& sh, int nwarps, int64_t smem_budget, const std::vector<StreamBrickDef>& bricks,

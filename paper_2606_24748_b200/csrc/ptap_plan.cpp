@@ -227,7 +227,7 @@ int ptap_host_stream_stats(void* handle, int32_t bs_f, int32_t bs_c, int32_t sta
   }
   int64_t bits = 0, lanes = 0, steps = 0;
   for (const StreamMeta& m : sp.meta) bits += __builtin_popcount(m.mask);
-  for (const StreamEntry& e : sp.entries) lanes += e.nslots;
+  for (const StreamEntry& e : sp.entries) lanes += e.nslots();
   for (const StreamPass& p : sp.passes) steps += p.steps;
   out8[0] = sp.ok ? 1 : 0; out8[1] = sp.nbricks(); out8[2] = sp.nchunks(); out8[3] = sp.max_smem;
   out8[4] = bits; out8[5] = lanes; out8[6] = (int64_t)sp.passes.size(); out8[7] = steps;

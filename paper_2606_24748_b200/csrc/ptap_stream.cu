@@ -123,12 +123,13 @@ stream_product_kernel(const StreamArgs a) {
     const int4* hp = reinterpret_cast<const int4*>(a.chunks + ch);
     const int4 h0 = __ldg(hp), h1 = __ldg(hp + 1), h2 = __ldg(hp + 2);
     const int64_t meta0 = ((int64_t)(uint32_t)h0.x) | ((int64_t)h0.y << 32);
-    const int nx = h0.z, ny = h0.w;              // nx even (padded by the plan)
+    const int nx = h0.z, ny = h0.w;
     const int ent0 = h1.x, nent = h1.y, pass0 = h1.z, npass = h1.w;
     const int xr0 = h2.x, nxr = h2.y, yr0 = h2.z, nyr = h2.w;
+    const int nmeta = __ldg(reinterpret_cast<const int*>(hp + 3));   // even (padded by the plan)
     double* Xs = reinterpret_cast<double*>(smem);
     StreamMeta* metas = reinterpret_cast<StreamMeta*>(smem + up16d((int64_t)nx * XS * 8));
-    double* Ys = reinterpret_cast<double*>(reinterpret_cast<unsigned char*>(metas) + up16d((int64_t)nx * 8));
+    double* Ys = reinterpret_cast<double*>(reinterpret_cast<unsigned char*>(metas) + up16d((int64_t)nmeta * 8));
     StreamEntry* entries = reinterpret_cast<StreamEntry*>(reinterpret_cast<unsigned char*>(Ys) + up16d((int64_t)ny * KN * 8));
     StreamPass* passes = reinterpret_cast<StreamPass*>(entries + nent);
     // ---- stage X (padded to XS doubles per block), masks, Y, entries, passes.  Runs are dealt to the warps; a warp
@@ -173,7 +174,7 @@ stream_product_kernel(const StreamArgs a) {
     }
     {
       const uint4* msrc = reinterpret_cast<const uint4*>(a.meta + meta0);
-      for (int e = tid; e < nx / 2; e += NT) cp_async<16>(reinterpret_cast<uint4*>(metas) + e, msrc + e);
+      for (int e = tid; e < nmeta / 2; e += NT) cp_async<16>(reinterpret_cast<uint4*>(metas) + e, msrc + e);
       const uint4* esrc = reinterpret_cast<const uint4*>(a.entries + ent0);
       for (int e = tid; e < nent; e += NT) cp_async<16>(reinterpret_cast<uint4*>(entries) + e, esrc + e);
       const uint4* psrc = reinterpret_cast<const uint4*>(a.passes + pass0);
@@ -188,11 +189,12 @@ stream_product_kernel(const StreamArgs a) {
     // ---- the passes of this warp
     for (int p = warp; p < npass; p += NW) {
       const StreamPass ps = passes[p];
-      int xbase = 0, len = 0, out = 0, slot = -1;
+      int xbase = 0, mbase = 0, len = 0, out = 0, slot = -1;   // slot: inside the entry's window of the row's slots
       for (int e = ps.e0; e < ps.e1; ++e) {
         const StreamEntry en = entries[e];
-        if (lane >= en.lane0 && lane < en.lane0 + en.nslots) {
-          xbase = en.xbase; len = en.len; out = en.out; slot = en.slot0 + lane - en.lane0;
+        const int l0 = en.lane0();
+        if (lane >= l0 && lane < l0 + en.nslots()) {
+          xbase = en.xbase; mbase = en.mbase; len = en.len(); out = en.out; slot = en.slot0() + lane - l0;
         }
       }
       if (!PERSIST) {
@@ -201,10 +203,10 @@ stream_product_kernel(const StreamArgs a) {
       }
       const uint32_t below = slot >= 0 ? ((1u << slot) - 1u) : 0u;
       // the mask of step k+1 is fetched while step k computes (one shared-memory latency off the critical path)
-      StreamMeta nxt = metas[xbase];
+      StreamMeta nxt = metas[mbase];
       for (int k = 0; k < ps.steps; ++k) {
         const StreamMeta mt = nxt;
-        nxt = metas[xbase + min(k + 1, max(len - 1, 0))];
+        nxt = metas[mbase + min(k + 1, max(len - 1, 0))];
         if (slot >= 0 && k < len) {
           if ((mt.mask >> slot) & 1u) {
             const double* xp = Xs + (int64_t)(xbase + k) * XS;

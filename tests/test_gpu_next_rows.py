@@ -324,8 +324,9 @@ def _second_workload(kind, small):
 def test_second_workload_hot_path(bsr, kind, small):
     """SpMV family (every entry), PtAP (structure ==, every block of AP and A_c against the oracle's form 2, a sample
     of coarse rows against the long-double form 1) and prolongator smoothing on the denser (Q2, up to 125 blocks per
-    row, A_c rows of 125) and the irregular (greedy aggregates, A_c rows beyond 32 blocks) operators: rows that leave
-    the staged PtAP format run the gather kernels."""
+    row, A_c rows of 125) and the irregular (greedy aggregates, A_c rows beyond 32 blocks) operators: output rows of
+    more than 32 blocks run the staged kernels window by window; stage 1 of the Q2 operator, whose single rows exceed
+    a brick's shared memory, runs the gather kernel."""
     from tests.test_gpu_fullsize import check_all_blocks, check_ptap_rows, check_spmv_family, sample_rows
     g = _second_workload(kind, small)
     A, P = g.A(0), g.P(0)
@@ -338,9 +339,11 @@ def test_second_workload_hot_path(bsr, kind, small):
     assert np.array_equal(rap_g, rap) and np.array_equal(cap_g, cap)
     sched = plan.schedule()
     if not small:
-        assert np.diff(st[0]).max() > 32 and not sched[2]["staged"]          # off the staged format: gather kernels
-        if kind == "q2":
-            assert (A.nbrows, A.nnzb) == (274625, 16974593) and not sched[1]["staged"]
+        assert np.diff(st[0]).max() > 32 and sched[2]["staged"]              # rows of several 32-slot windows, staged
+        if kind == "q2":                                                    # one row of A with its P rows exceeds a brick
+            assert (A.nbrows, A.nbrows * 3, A.nnzb) == (274625, 823875, 16974593) and not sched[1]["staged"]
+        else:
+            assert sched[1]["staged"]
     vals = plan.numeric()
     check_all_blocks(plan, vals, A, P, st, f"f4 {kind}")
     check_ptap_rows(plan, vals, A, P, st, sample_rows(P.nbcols, 8 if not small else 4, 11))
