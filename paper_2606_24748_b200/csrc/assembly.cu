@@ -40,14 +40,18 @@ bcoo_sum_kernel(int64_t nvals, const int32_t* __restrict__ segptr, const int32_t
   const int e = (int)(t - slot * BB);
   const int32_t p0 = __ldg(segptr + slot), p1 = __ldg(segptr + slot + 1);
   double s = 0.0;
-  int32_t p = p0;
-  for (; p + 1 < p1; p += 2) {   // two independent loads in flight, added in declaration order
-    const double v0 = __ldg(stream + (int64_t)__ldg(perm + p) * BB + e);
-    const double v1 = __ldg(stream + (int64_t)__ldg(perm + p + 1) * BB + e);
-    s += v0;
-    s += v1;
+  // up to four contributions in flight (positions first, then values; indices clamped instead of predicated so that
+  // the loads are issued back to back), added in declaration order
+  for (int32_t p = p0; p < p1; p += 4) {
+    int32_t q[4];
+    double v[4];
+#pragma unroll
+    for (int u = 0; u < 4; ++u) q[u] = __ldg(perm + min(p + u, p1 - 1));
+#pragma unroll
+    for (int u = 0; u < 4; ++u) v[u] = __ldg(stream + (int64_t)q[u] * BB + e);
+#pragma unroll
+    for (int u = 0; u < 4; ++u) s += (p + u < p1) ? v[u] : 0.0;
   }
-  if (p < p1) s += __ldg(stream + (int64_t)__ldg(perm + p) * BB + e);
   vals[t] = s;
 }
 
@@ -94,33 +98,54 @@ q1_coords_kernel(int d, int ne, int64_t e0, int64_t ncontrib, int32_t* __restric
   bcol[c] = ib;
 }
 
-// stream value (c, i, j) = E_e * Ke[a*d+i][b*d+j]; with `dirichlet` the face ix = 0 is clamped in the stream itself
+// stream block c = E_e * Ke[a][b] (d x d); with `dirichlet` the face ix = 0 is clamped in the stream itself
 // (reading R4): a block whose row or column node is clamped is zero, except the node's own diagonal block,
-// which carries I / (number of elements adjacent to the node) so that the assembled block is exactly I
+// which carries I / (number of elements adjacent to the node) so that the assembled block is exactly I.
+// One thread per contribution block: the element / local-node arithmetic is done once per block, the reference element
+// matrix sits in shared memory; the CTA's 256 blocks go through shared memory so that the stream is written with
+// fully coalesced stores.
+template <int D>
 __global__ void __launch_bounds__(256)
-q1_blocks_kernel(int d, int ne, int64_t e0, int64_t nvals, const double* __restrict__ Ke, const double* __restrict__ E,
+q1_blocks_kernel(int ne, int64_t e0, int64_t ncontrib, const double* __restrict__ Ke, const double* __restrict__ E,
                  int dirichlet, double* __restrict__ stream) {
-  const int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (t >= nvals) return;
-  const int nen = 1 << d, nn = nen * nen, bb = d * d, nd = d * nen;
-  const int64_t c = t / bb;
-  const int ij = (int)(t - c * bb), i = ij / d, j = ij - i * d;
-  const int64_t e = e0 + c / nn;
-  const int ab = (int)(c % nn), a = ab / nen, b = ab % nen;
-  double v = (E ? __ldg(E + e) : 1.0) * __ldg(Ke + (a * d + i) * nd + (b * d + j));
+  constexpr int NEN = 1 << D, NN = NEN * NEN, BB = D * D, ND = D * NEN;
+  __shared__ double ke[ND * ND];
+  __shared__ double outb[256 * BB];
+  for (int t = threadIdx.x; t < ND * ND; t += blockDim.x) ke[t] = Ke[t];
+  __syncthreads();
+  const int64_t c0 = (int64_t)blockIdx.x * blockDim.x;
+  const int64_t c = c0 + threadIdx.x;
+  const bool live = c < ncontrib;
+  if (live) {
+  const int64_t e = e0 + c / NN;
+  const int ab = (int)(c % NN), a = ab / NEN, b = ab % NEN;
+  const double Ee = E ? __ldg(E + e) : 1.0;
+  double v[BB];
+#pragma unroll
+  for (int i = 0; i < D; ++i)
+#pragma unroll
+    for (int j = 0; j < D; ++j) v[i * D + j] = Ee * ke[(a * D + i) * ND + (b * D + j)];
   if (dirichlet) {
     int ia, ib, ca[3], cb[3];
-    q1_nodes(d, ne, e, a, b, ia, ib, ca, cb);
+    q1_nodes(D, ne, e, a, b, ia, ib, ca, cb);
     if (ca[0] == 0 || cb[0] == 0) {
-      v = 0.0;
-      if (a == b && i == j) {
+#pragma unroll
+      for (int t = 0; t < BB; ++t) v[t] = 0.0;
+      if (a == b) {
         const int cy = (ca[1] > 0 && ca[1] < ne) ? 2 : 1;
-        const int cz = (d == 3 && ca[2] > 0 && ca[2] < ne) ? 2 : 1;
-        v = 1.0 / (double)(cy * cz);
+        const int cz = (D == 3 && ca[2] > 0 && ca[2] < ne) ? 2 : 1;
+#pragma unroll
+        for (int i = 0; i < D; ++i) v[i * D + i] = 1.0 / (double)(cy * cz);
       }
     }
   }
-  stream[t] = v;
+#pragma unroll
+  for (int t = 0; t < BB; ++t) outb[threadIdx.x * BB + t] = v[t];   // odd stride (9) / 4: conflict-free enough
+  }
+  __syncthreads();
+  const int64_t nlive = min((int64_t)blockDim.x, ncontrib - c0) * BB;
+  double* dst = stream + c0 * BB;
+  for (int64_t t = threadIdx.x; t < nlive; t += blockDim.x) dst[t] = outb[t];
 }
 
 static void bcoo_release(bcoo_plan_s* pl) {
@@ -296,12 +321,13 @@ int fem_q1_element_blocks(int32_t d, int32_t ne, int64_t e0, int64_t e1, const d
   if ((d != 2 && d != 3) || ne < 1 || e0 < 0 || e1 < e0) return fail(BSR_ERR_SHAPE, "fem_q1_element_blocks: bad argument");
   const int64_t nel = (d == 3) ? (int64_t)ne * ne * ne : (int64_t)ne * ne;
   if (e1 > nel) return fail(BSR_ERR_SHAPE, "element range outside the grid");
-  const int64_t nv = ((e1 - e0) << (2 * d)) * d * d;
-  if (nv == 0) return BSR_OK;
+  const int64_t nc = (e1 - e0) << (2 * d);
+  if (nc == 0) return BSR_OK;
   if (!d_Ke || !d_stream) return fail(BSR_ERR_NULL, "null array");
-  const int64_t nblocks = (nv + 255) / 256;
+  const int64_t nblocks = (nc + 255) / 256;
   if (nblocks >= (1LL << 31)) return fail(BSR_ERR_LIMIT, "stream too long for one launch");
-  LAUNCH(q1_blocks_kernel, (unsigned)nblocks, 256, 0, (cudaStream_t)stream, d, ne, e0, nv, d_Ke, d_E, dirichlet, d_stream);
+  if (d == 3) LAUNCH(q1_blocks_kernel<3>, (unsigned)nblocks, 256, 0, (cudaStream_t)stream, ne, e0, nc, d_Ke, d_E, dirichlet, d_stream);
+  else LAUNCH(q1_blocks_kernel<2>, (unsigned)nblocks, 256, 0, (cudaStream_t)stream, ne, e0, nc, d_Ke, d_E, dirichlet, d_stream);
   return BSR_OK;
 }
 
