@@ -1,8 +1,8 @@
 """Turn an `ncu --set full` capture into the text evidence kept under profiles/.
 
     ncu -i gpurun_out/prof.ncu-rep --page raw --csv > gpurun_out/prof_raw.csv
-    python -m paper_2606_24748_b200.ncu_summary gpurun_out/prof_raw.csv --traffic profiles/ncu_traffic.csv \
-        --table profiles/<name>.md
+    python -m paper_2606_24748_b200.ncu_summary gpurun_out/prof_raw.csv [more_raw.csv ...] \
+        --traffic profiles/ncu_traffic.csv --table profiles/<name>.md
 
 Reads the raw-page CSV (one row per profiled launch, a units row under the header), averages the launches of each
 kernel and writes (a) `--traffic`: bench.py's kernel name, dram__bytes_read.sum + dram__bytes_write.sum per launch
@@ -68,12 +68,17 @@ def mean(v):
 
 def main():
     ap = argparse.ArgumentParser()
-    ap.add_argument("raw_csv")
+    ap.add_argument("raw_csv", nargs="+")
     ap.add_argument("--traffic", help="write bench.py's traffic table (profiles/ncu_traffic.csv)")
     ap.add_argument("--table", help="write a markdown table of the counters")
     ap.add_argument("--command", default="", help="the capture command, recorded in the table's header")
     a = ap.parse_args()
-    data = load(a.raw_csv)
+    data = OrderedDict()
+    for path in a.raw_csv:
+        for k, rec in load(path).items():
+            tgt = data.setdefault(k, {m: [] for m in METRICS})
+            for m in METRICS:
+                tgt[m] += rec[m]
     if a.traffic:
         with open(a.traffic, "w") as f:
             f.write("kernel,dram_bytes_per_launch,launches,kernel_name\n")
