@@ -30,6 +30,7 @@
 #ifndef BSR_AMG_H
 #define BSR_AMG_H
 
+#include <stddef.h>
 #include <stdint.h>
 
 #ifdef __cplusplus
@@ -267,6 +268,17 @@ int bsr_counters(int64_t* n_kernel_launches, int64_t* n_allocs);
 /* Measured fp64 FMA peak of the current device in TFLOP/s (register-resident FMA chains, CUDA events, best of 5):
  * the ALU roof reported beside the HBM roof of the PtAP kernels.  COLD: allocates, synchronises. */
 int bsr_measure_fp64_peak(double* tflops, void* stream);
+
+/* ------------------------------------------------------------------ workspace allocator (ownership)
+ * Library-private workspace (the cached transpose, AP, plans, D^-1, work vectors, the dense factor) is obtained in COLD
+ * calls only.  By default it comes from cudaMalloc; a caller that owns device memory (the Python harness: torch's caching
+ * allocator) registers a pair of callbacks and every later allocation goes through them: alloc_fn(bytes, ctx) returns a
+ * 256-byte aligned DEVICE pointer or null, free_fn(ptr, ctx) releases one.  A block is returned to the source it came
+ * from; pass (null, null, null) to go back to cudaMalloc (blocks already handed out stay valid until the library frees
+ * them through the free_fn registered at that time).  Process-wide; thread-safe.  Errors: BSR_ERR_NULL. */
+typedef void* (*bsr_alloc_fn)(size_t bytes, void* ctx);
+typedef void (*bsr_free_fn)(void* ptr, void* ctx);
+int bsr_set_allocator(bsr_alloc_fn alloc_fn, bsr_free_fn free_fn, void* ctx);
 
 /* ------------------------------------------------------------------ options of the COLD calls (tests, tuning)
  * Process-wide; read by ptap_symbolic only, never by a hot call.  Names: "ptap_force_gather" (1: keep the

@@ -55,6 +55,7 @@ SYMBOLS = {
     "pcg_solve": (C.c_int, [_V, _V, _V, _I32, _V, _V]),
     "vcycle_apply_host": (C.c_int, [_V, _V, _V, _V]),
     "vcycle_destroy": (C.c_int, [_V]),
+    "bsr_set_allocator": (C.c_int, [_V, _V, _V]),
     "bsr_counters": (C.c_int, [_PI64, _PI64]),
     "bsr_measure_fp64_peak": (C.c_int, [C.POINTER(_D), _V]),
     "prolongator_smooth_symbolic": (C.c_int, [_PV, _V, _V, _PI64, _V]),
@@ -81,6 +82,56 @@ class BsrError(RuntimeError):
         self.code = code
 
 
+_ALLOC_FN = C.CFUNCTYPE(C.c_void_p, C.c_size_t, C.c_void_p)
+_FREE_FN = C.CFUNCTYPE(None, C.c_void_p, C.c_void_p)
+_workspace = {}      # device pointer -> the torch tensor that backs it (kept alive until the library frees it)
+_alloc_cb = _free_cb = None
+
+
+def _torch_alloc(nbytes, _ctx):
+    import torch
+    try:
+        t = torch.empty(int(nbytes), dtype=torch.uint8, device=torch.device("cuda", torch.cuda.current_device()))
+    except Exception:
+        return None
+    _workspace[t.data_ptr()] = t
+    return t.data_ptr()
+
+
+def _torch_free(ptr, _ctx):
+    _workspace.pop(ptr, None)
+
+
+def use_torch_allocator(enable: bool = True):
+    """Library workspace from torch's caching allocator (bsr_set_allocator): "PyTorch for device memory".  On by
+    default once a CUDA device is present; `enable=False` goes back to cudaMalloc."""
+    global _alloc_cb, _free_cb
+    if enable:
+        if _alloc_cb is None:
+            _alloc_cb, _free_cb = _ALLOC_FN(_torch_alloc), _FREE_FN(_torch_free)
+        _check(lib().bsr_set_allocator(C.cast(_alloc_cb, C.c_void_p), C.cast(_free_cb, C.c_void_p), None))
+    else:
+        _check(lib().bsr_set_allocator(None, None, None))
+
+
+def _allocator_off_at_exit():
+    # blocks still held at interpreter shutdown are left to the process teardown instead of calling back into Python
+    try:
+        if _lib is not None and _alloc_cb is not None:
+            _lib.bsr_set_allocator(None, None, None)
+    except Exception:
+        pass
+
+
+import atexit  # noqa: E402
+atexit.register(_allocator_off_at_exit)
+
+
+def workspace_bytes() -> int:
+    """Bytes of library workspace currently held through the torch allocator."""
+    return sum(int(t.numel()) for t in _workspace.values())
+
+
 def lib():
     """Loads (building if stale) the CUDA library.  Fails loudly when it cannot be built or loaded."""
     global _lib
@@ -91,6 +142,12 @@ def lib():
             f = getattr(L, name)  # AttributeError if the library does not export a declared symbol
             f.restype, f.argtypes = res, args
         _lib = L
+        try:
+            import torch
+            if torch.cuda.is_available():
+                use_torch_allocator(True)
+        except ImportError:
+            pass
     return _lib
 
 

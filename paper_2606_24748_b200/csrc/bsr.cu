@@ -16,6 +16,9 @@
 #include <cstdlib>
 #include <cstring>
 
+#include <mutex>
+#include <unordered_set>
+
 #include "internal.h"
 
 namespace bsramg {
@@ -34,8 +37,28 @@ int fail(int code, const char* fmt, ...) {
   return code;
 }
 
+// library workspace: through the caller's allocator when one is registered (bsr_set_allocator), else cudaMalloc.
+// Memory obtained from one source is returned to the same source.
+static bsr_alloc_fn g_alloc = nullptr;
+static bsr_free_fn g_free = nullptr;
+static void* g_alloc_ctx = nullptr;
+static std::mutex g_alloc_mu;
+static std::unordered_set<void*> g_from_caller;
+
 int dev_alloc(void** p, size_t bytes) {
   *p = nullptr;
+  bsr_alloc_fn af;
+  void* ctx;
+  { std::lock_guard<std::mutex> lk(g_alloc_mu); af = g_alloc; ctx = g_alloc_ctx; }
+  if (af) {
+    void* q = af(bytes ? bytes : 16, ctx);
+    if (!q) return fail(BSR_ERR_ALLOC, "the caller's allocator returned null for %zu bytes", bytes);
+    if ((uintptr_t)q & 255) { return fail(BSR_ERR_ALIGN, "the caller's allocator returned memory that is not 256-byte aligned"); }
+    { std::lock_guard<std::mutex> lk(g_alloc_mu); g_from_caller.insert(q); }
+    *p = q;
+    g_allocs.fetch_add(1, std::memory_order_relaxed);
+    return BSR_OK;
+  }
   cudaError_t e = cudaMalloc(p, bytes ? bytes : 16);
   if (e != cudaSuccess) {
     cudaGetLastError();
@@ -46,7 +69,16 @@ int dev_alloc(void** p, size_t bytes) {
   return BSR_OK;
 }
 void dev_free(void* p) {
-  if (p) cudaFree(p);
+  if (!p) return;
+  bsr_free_fn ff = nullptr;
+  void* ctx = nullptr;
+  {
+    std::lock_guard<std::mutex> lk(g_alloc_mu);
+    auto it = g_from_caller.find(p);
+    if (it != g_from_caller.end()) { g_from_caller.erase(it); ff = g_free; ctx = g_alloc_ctx; if (!ff) return; }
+  }
+  if (ff) ff(p, ctx);
+  else cudaFree(p);
 }
 
 // ------------------------------------------------------------------ lane mapping of one block shape
@@ -498,6 +530,13 @@ using namespace bsramg;
 extern "C" {
 
 const char* bsr_last_error(void) { return t_err.c_str(); }
+
+int bsr_set_allocator(bsr_alloc_fn alloc_fn, bsr_free_fn free_fn, void* ctx) {
+  if ((alloc_fn == nullptr) != (free_fn == nullptr)) return fail(BSR_ERR_NULL, "bsr_set_allocator: give both functions or neither");
+  std::lock_guard<std::mutex> lk(g_alloc_mu);
+  g_alloc = alloc_fn; g_free = free_fn; g_alloc_ctx = ctx;
+  return BSR_OK;
+}
 
 int bsr_counters(int64_t* n_kernel_launches, int64_t* n_allocs) {
   if (n_kernel_launches) *n_kernel_launches = g_launches.load();

@@ -295,3 +295,35 @@ def test_spmv_host_end_to_end(bsr, probs):
     ref = orc.ptap(A, P)
     mag = orc.ptap(abs_copy(A), abs_copy(P)).vals
     assert blockwise_rel_err(h_out.reshape(ref.vals.shape), 1.5 * ref.vals, 1.5 * mag) < TOL
+
+
+def test_workspace_comes_from_the_callers_allocator(bsr, probs):
+    """Library workspace is obtained through bsr_set_allocator (torch's caching allocator in the harness), in cold
+    calls only, and returned when the handles are destroyed; an allocator that fails surfaces as BSR_ERR_ALLOC."""
+    import ctypes as C
+    import torch
+    g = probs["cfg0"]
+    A, P = g.A(0), g.P(0)
+    GA, GP = bsr.Bsr.from_host(A), bsr.Bsr.from_host(P)
+    w0 = bsr.workspace_bytes()
+    plan = bsr.PtapPlan(GA, GP)
+    w1 = bsr.workspace_bytes()
+    assert w1 > w0 + plan.info()["nnzb_ap"] * 18 * 8            # at least AP's values live in torch memory now
+    a0 = bsr.counters()[1]
+    v = plan.numeric()
+    assert bsr.counters()[1] == a0 and bsr.workspace_bytes() == w1   # hot call: no allocation
+    plan.close(); GP.close()
+    assert bsr.workspace_bytes() <= w0
+    # a failing allocator: the cold call reports BSR_ERR_ALLOC and nothing leaks
+    fail_alloc = bsr._ALLOC_FN(lambda n, ctx: None)
+    noop_free = bsr._FREE_FN(lambda p, ctx: None)
+    bsr._check(bsr.lib().bsr_set_allocator(C.cast(fail_alloc, C.c_void_p), C.cast(noop_free, C.c_void_p), None))
+    try:
+        GP2 = bsr.Bsr.from_host(P)
+        with pytest.raises(bsr.BsrError) as e:
+            bsr.PtapPlan(GA, GP2)
+        assert e.value.code == 5
+    finally:
+        bsr.use_torch_allocator(True)
+    plan2 = bsr.PtapPlan(GA, GP2)                               # and the library works again afterwards
+    assert torch.equal(plan2.numeric(), v)

@@ -120,3 +120,21 @@ def test_staged_schedule_covers_every_product_once():
         assert s2["bricks"] == P.nbcols and s2["chunks"] >= s2["bricks"]
         assert s1["lanes"] == hp.colidx_ap.shape[0]       # one lane per AP block
         assert s1["passes"] * 32 >= s1["lanes"] and s1["steps"] > 0
+
+
+def test_limit_errors_without_device():
+    """BSR_ERR_LIMIT: 32-bit counts that would overflow are refused before any device work."""
+    L = bsr.lib()
+    h = C.c_void_p()
+    fake = C.c_void_p(256)                                   # never dereferenced: the size check comes first
+    nnzb = (1 << 31) // 9 + 1
+    rc = L.bsr_create(C.byref(h), 10, 10, 3, 3, nnzb, fake, fake, fake, None)
+    assert rc == 10 and b"2^31" in L.bsr_last_error() and not h.value
+    nn = C.c_int64()
+    rc = L.bcoo_plan_create(C.byref(h), 1 << 31, fake, fake, 10, 10, 3, 3, C.byref(nn), None)
+    assert rc == 10 and not h.value
+    rc = L.bsr_gather_blocks(1 << 40, fake, 9, fake, fake, None)
+    assert rc == 10
+    # the allocator registration wants both callbacks or neither
+    assert L.bsr_set_allocator(fake, None, None) == 1
+    assert L.bsr_set_allocator(None, None, None) == 0
