@@ -18,13 +18,15 @@ template <bool TRANSB>
 __global__ void __launch_bounds__(256)
 dgemm128_kernel(int k, double alpha, const double* __restrict__ A, int64_t lda, const double* __restrict__ B,
                 int64_t ldb, double beta, double* __restrict__ C, int64_t ldc, int64_t sA, int64_t sB, int64_t sC,
-                int tri, int klim) {
+                int tri, int klim, int koff, int kcap) {
   const int m0 = blockIdx.y * GT, n0 = blockIdx.x * GT;
   if (tri && n0 > m0) return;                       // lower tiles only
   A += (int64_t)blockIdx.z * sA; B += (int64_t)blockIdx.z * sB; C += (int64_t)blockIdx.z * sC;
   int kbeg = 0, kend = k;
   if (klim == 1) kbeg = min(n0, k);                 // B (k x n) is lower triangular: rows k < n0 of this tile are zero
   if (klim == 2) kend = min(m0 + GT, k);            // A (m x k) is lower triangular: columns k >= m0+128 are zero
+  kbeg = max(kbeg, min((koff + m0) & ~(GK - 1), k));   // A banded: row m0 + i is zero left of column koff + m0 + i
+  kend = min(kend, kcap);                           // B has no nonzero row at or beyond kcap
   __shared__ __align__(16) double As[GK][GS];
   __shared__ __align__(16) double Bs[GK][GS];
   const int tid = threadIdx.x, tx = tid & 15, ty = tid >> 4;
@@ -110,13 +112,15 @@ dgemm128_kernel(int k, double alpha, const double* __restrict__ A, int64_t lda, 
 
 int dgemm128(bool transB, int m, int n, int k, double alpha, const double* A, int64_t lda, const double* B, int64_t ldb,
              double beta, double* C, int64_t ldc, int batch, int64_t sA, int64_t sB, int64_t sC, int tri, int klim,
-             cudaStream_t st) {
+             cudaStream_t st, int koff, int kcap) {
   if (m <= 0 || n <= 0 || batch <= 0) return BSR_OK;
   if (m % GT || n % GT || k % GK || (lda & 1) || (ldb & 1) || (ldc & 1))
     return fail(BSR_ERR_SHAPE, "dgemm128: sizes must be multiples of the tile (m %d n %d k %d)", m, n, k);
   const dim3 grid((unsigned)(n / GT), (unsigned)(m / GT), (unsigned)batch);
-  if (transB) LAUNCH(dgemm128_kernel<true>, grid, 256, 0, st, k, alpha, A, lda, B, ldb, beta, C, ldc, sA, sB, sC, tri, klim);
-  else LAUNCH(dgemm128_kernel<false>, grid, 256, 0, st, k, alpha, A, lda, B, ldb, beta, C, ldc, sA, sB, sC, tri, klim);
+  if (kcap <= 0 || kcap > k) kcap = k;
+  if (koff < -(1 << 29)) koff = -(1 << 29);
+  if (transB) LAUNCH(dgemm128_kernel<true>, grid, 256, 0, st, k, alpha, A, lda, B, ldb, beta, C, ldc, sA, sB, sC, tri, klim, koff, kcap);
+  else LAUNCH(dgemm128_kernel<false>, grid, 256, 0, st, k, alpha, A, lda, B, ldb, beta, C, ldc, sA, sB, sC, tri, klim, koff, kcap);
   return BSR_OK;
 }
 

@@ -77,10 +77,11 @@ int spmv_launch(bsr_t A, const double* d_x, double* d_y, const double* d_b, Epil
 int block_diag_inverse(bsr_t A, double* dinv, int* status, cudaStream_t st);
 // C (m x n) = beta*C + alpha * A (m x k) * op(B), row-major, 128x128 tiles (dense_gemm.cu).  transB: B is n x k, else
 // k x n.  batch problems at strides sA/sB/sC.  tri = 1: lower tiles only.  klim = 1: B lower triangular (k >= tile
-// column start), 2: A lower triangular (k < tile row end).  m, n multiples of 128, k of 16.
+// column start), 2: A lower triangular (k < tile row end).  koff: A is banded, row i has no nonzero left of column
+// koff + i (very negative: none).  kcap: rows >= kcap of B are zero (0: none).  m, n multiples of 128, k of 16.
 int dgemm128(bool transB, int m, int n, int k, double alpha, const double* A, int64_t lda, const double* B, int64_t ldb,
              double beta, double* C, int64_t ldc, int batch, int64_t sA, int64_t sB, int64_t sC, int tri, int klim,
-             cudaStream_t st);
+             cudaStream_t st, int koff = -(1 << 30), int kcap = 0);
 // makes sure the cached transpose exists and its values are current; hot when nothing changed
 int transpose_ensure(bsr_t A, cudaStream_t st);
 

@@ -39,6 +39,7 @@ struct vcycle_s {
   std::vector<bsramg::Level> L;
   // coarsest level, dense
   int64_t nc = 0, npad = 0;
+  int64_t band = 0;   // scalar half-bandwidth of the coarsest operator, rounded up to whole panels (npad: not banded)
   double *dense = nullptr, *diaginv = nullptr, *linv = nullptr, *linvT = nullptr, *ytmp = nullptr;
   int32_t* coarse_rowidx = nullptr;   // block row of every stored block of the coarsest operator (dense fill)
   int* d_status = nullptr;
@@ -334,15 +335,19 @@ static int coarse_factor(vcycle_t vc, cudaStream_t st) {
            A->d_colidx, A->d_vals, np, vc->dense);
   const dim3 tb(TS, TS);
   // ---- A = L L^T, right-looking over 128-wide panels
+  // A banded operator (the lexicographic 27-point coarse grid: half-bandwidth 666 of 6000) keeps its band in L: below
+  // the band every tile is zero and is skipped -- rows of a panel, of the trailing update and k-ranges of the inverse
+  const int64_t band = std::min(vc->band, np);
+  const int btiles = (int)(band / TS) + PT;   // tile rows below a tile column that can hold nonzeros
   for (int J = 0; J < npan; ++J) {
     for (int s = 0; s < PT; ++s) {        // the panel itself, 32x32 tiles: factor, solve below, update the panel's own columns
-      const int c = J * PT + s, rest = nb - c - 1, pc = PT - 1 - s;
+      const int c = J * PT + s, rest = std::min(nb - c - 1, btiles), pc = PT - 1 - s;
       LAUNCH(potrf_tile_kernel, 1, tb, 0, st, np, c, vc->dense, vc->diaginv, vc->d_status);
       if (rest > 0) LAUNCH(trsm_tile_kernel, (unsigned)rest, tb, 0, st, np, c, vc->dense, vc->diaginv);
       if (rest > 0 && pc > 0) LAUNCH(syrk_tile_kernel, dim3(pc, rest), tb, 0, st, np, c, vc->dense);
     }
     const int64_t r0 = (int64_t)(J + 1) * PANEL;
-    const int m = (int)(np - r0);
+    const int m = (int)std::min(np - r0, band);
     if (m > 0) {                          // trailing update: one GEMM over the lower tiles, k = the panel
       const double* Lp = vc->dense + r0 * np + (int64_t)J * PANEL;
       BSR_TRY(dgemm128(true, m, m, PANEL, -1.0, Lp, np, Lp, np, 1.0, vc->dense + r0 * np + r0, np, 1, 0, 0, 0, 1, 0, st));
@@ -357,10 +362,13 @@ static int coarse_factor(vcycle_t vc, cudaStream_t st) {
     const int64_t rem = np - (int64_t)nfull * step;           // a last pair with a shorter second block, if rem > b
     auto pair = [&](int64_t r0, int64_t b2, int batch) -> int {
       const int64_t o21 = (r0 + b) * np + r0, o11 = r0 * np + r0, o22 = (r0 + b) * np + (r0 + b), sp = step * np + step;
-      BSR_TRY(dgemm128(false, (int)b2, (int)b, (int)b, 1.0, vc->dense + o21, np, vc->linv + o11, np, 0.0, vc->linvT + o21, np,
-                       batch, sp, sp, sp, 0, 1, st));
+      // L21 is banded: its row i is zero left of column b + i - band and entirely zero for i >= band, so T = L21 X11
+      // has `mt` nonzero rows and the second product stops at k = mt
+      const int64_t mt = std::min(b2, band);
+      BSR_TRY(dgemm128(false, (int)mt, (int)b, (int)b, 1.0, vc->dense + o21, np, vc->linv + o11, np, 0.0, vc->linvT + o21, np,
+                       batch, sp, sp, sp, 0, 1, st, (int)(b - band), 0));
       return dgemm128(false, (int)b2, (int)b, (int)b2, -1.0, vc->linv + o22, np, vc->linvT + o21, np, 0.0, vc->linv + o21, np,
-                      batch, sp, sp, sp, 0, 2, st);
+                      batch, sp, sp, sp, 0, 2, st, -(1 << 30), (int)mt);
     };
     if (nfull > 0) BSR_TRY(pair(0, b, nfull));
     if (rem > b) BSR_TRY(pair((int64_t)nfull * step, rem - b, 1));
@@ -557,6 +565,12 @@ int vcycle_create(vcycle_t* out, int32_t nlevels, const bsr_t* A, const bsr_t* P
     for (int32_t i = 0; i < Ac->nbrows; ++i)
       for (int32_t k = Ac->h_rowptr[i]; k < Ac->h_rowptr[(size_t)i + 1]; ++k) rowidx[(size_t)k] = i;
     rc = upload(&vc->coarse_rowidx, rowidx, st);
+    // half-bandwidth of the coarsest operator in scalars, rounded up to whole panels
+    int64_t hb = 0;
+    for (int32_t i = 0; i < Ac->nbrows; ++i)
+      for (int32_t k = Ac->h_rowptr[i]; k < Ac->h_rowptr[(size_t)i + 1]; ++k)
+        hb = std::max<int64_t>(hb, std::abs((int64_t)Ac->h_colidx[(size_t)k] - i));
+    vc->band = std::min<int64_t>(vc->npad, (((hb + 1) * Ac->bs_r + PANEL - 1) / PANEL) * PANEL);
     if (rc == BSR_OK && cudaStreamSynchronize(st) != cudaSuccess) rc = fail(BSR_ERR_CUDA, "upload failed");
   }
   if (rc == BSR_OK) {
