@@ -14,6 +14,7 @@
 //   orc_ptap_form2      the same through a materialised AP and R (timed)    PAPER.md:103 ("local blocked triple product")
 //   orc_hier_*          block-Jacobi/Chebyshev V-cycle and PCG              PAPER.md:42 (cycle), 113 (pbjacobi, CG,
 //                                                                           unpreconditioned residual norm)
+//   orc_power_lambda    lambda of D^-1 A by 20 power iterations (omega = 4/(3 lambda))   PAPER.md:54-56; reading R10
 //   orc_prolongator_smooth  P = (I - omega D^-1 A) P~ over the pattern of A P~   PAPER.md:54-56 (eq.), 244 (block AXPY
 //                                                                           with SUBSET_NONZERO_PATTERN)
 //   orc_bcoo_structure / orc_bcoo_sum   blocked COO assembly: coordinates declared once incl. duplicates, the value
@@ -466,6 +467,38 @@ int orc_prolongator_smooth(const orc_bsr* Ap, const orc_bsr* Ptp, double omega, 
     }
   }
   return bad ? -2 : 0;
+}
+
+// lambda of D^-1 A by power iteration (reading R10): v <- v0/||v0||_2; `iters` times: w = D^-1 (A v),
+// lambda = ||w||_2, v = w / lambda; the last lambda is returned (omega = 4 / (3 lambda)).  D the
+// bs x bs block diagonal (R11).  Long double sums.  Returns a negative value on a missing / singular diagonal block.
+double orc_power_lambda(const orc_bsr* Ap, const double* v0, int iters) {
+  const orc_bsr& A = *Ap;
+  if (A.bs_r != A.bs_c || A.nbrows != A.nbcols || A.bs_r > 6) return -1.0;
+  const int bs = A.bs_r;
+  const int64_t n = (int64_t)A.nbrows * bs;
+  std::vector<double> dinv((size_t)A.nbrows * bs * bs), v(v0, v0 + n), t(n), w(n);
+  for (int32_t i = 0; i < A.nbrows; ++i) {
+    bool ok = false;
+    for (int64_t k = A.rowptr[i]; k < A.rowptr[i + 1]; ++k)
+      if (A.colidx[k] == i) { ok = invert_block(bs, A.vals + (size_t)k * bs * bs, &dinv[(size_t)i * bs * bs]); break; }
+    if (!ok) return -2.0;
+  }
+  double nv = std::sqrt(dot(n, v.data(), v.data()));
+  for (int64_t i = 0; i < n; ++i) v[i] /= nv;
+  double lambda = 0.0;
+  for (int it = 0; it < iters; ++it) {
+    spmv(A, v.data(), t.data());
+    for (int32_t i = 0; i < A.nbrows; ++i)
+      for (int a = 0; a < bs; ++a) {
+        ld sacc = 0;
+        for (int b = 0; b < bs; ++b) sacc += (ld)dinv[((size_t)i * bs + a) * bs + b] * (ld)t[(size_t)i * bs + b];
+        w[(size_t)i * bs + a] = (double)sacc;
+      }
+    lambda = std::sqrt(dot(n, w.data(), w.data()));
+    for (int64_t i = 0; i < n; ++i) v[i] = w[i] / lambda;
+  }
+  return lambda;
 }
 
 // ------------------------------------------------------------------ blocked COO assembly

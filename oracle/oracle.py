@@ -67,6 +67,8 @@ def _load():
         lib.orc_spgemm_symbolic.argtypes = [C.c_int32, V, V, V, V, V, V]
         lib.orc_ptap_form1.argtypes = [P, P, V, V, V, C.c_int32, V]
         lib.orc_ptap_form2.argtypes = [P, P, P, V, V, V, V, V, V]
+        lib.orc_power_lambda.restype = C.c_double
+        lib.orc_power_lambda.argtypes = [P, V, C.c_int]
         lib.orc_prolongator_smooth.argtypes = [P, P, C.c_double, V, V, V]
         lib.orc_bcoo_structure.restype = C.c_int64
         lib.orc_bcoo_structure.argtypes = [C.c_int64, V, V, C.c_int32, C.c_int32, V, V]
@@ -201,6 +203,16 @@ class PtapForm2:
         if rcode != 0:
             raise RuntimeError(f"orc_ptap_form2 failed ({rcode})")
         return OBsr(self.P.nbcols, self.P.nbcols, self.P.bs_c, self.P.bs_c, self.rc, self.cc, self.vals_c)
+
+
+def power_lambda(A, v0, iters: int = 20) -> float:
+    """lambda of D^-1 A after `iters` power iterations from v0 (reading R10); omega = 4 / (3 lambda)."""
+    h, v0 = _Held(A), _vec(v0)
+    assert v0.shape[0] == A.nbrows * A.bs_r
+    lam = float(_load().orc_power_lambda(h.c, v0.ctypes.data, int(iters)))
+    if lam < 0:
+        raise RuntimeError(f"orc_power_lambda failed ({lam})")
+    return lam
 
 
 def prolongator_smooth(A, Pt, omega: float) -> OBsr:

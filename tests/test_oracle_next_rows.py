@@ -79,6 +79,32 @@ def test_prolongator_smooth_level2_six_by_six_blocks():
     assert np.abs(P.vals - g.P(1).vals).max() < 1e-14
 
 
+@pytest.mark.parametrize("fix", ["cfg0", "grid2d"])
+def test_power_lambda(fix, request):
+    """R10: 20 power iterations on D^-1 A from the seeded start vector -- against the generator's own loop, a dense
+    numpy iteration through numpy's solver, and the bound by the true spectral radius (scipy eigenvalues)."""
+    g = request.getfixturevalue(fix)
+    A = g.A(0)
+    n, bs = A.nbrows * A.bs_r, A.bs_r
+    v0 = pr.uniform(g.seed, pr.PURPOSE_POWER, n)
+    lam = orc.power_lambda(A, v0, 20)
+    assert lam == pytest.approx(g.level_info(0)["lam"], rel=1e-13)
+    Ad = A.to_dense()
+    D = np.zeros_like(Ad)
+    for i in range(0, n, bs):
+        D[i:i + bs, i:i + bs] = Ad[i:i + bs, i:i + bs]
+    v = v0 / np.linalg.norm(v0)
+    for _ in range(20):
+        w = np.linalg.solve(D, Ad @ v)
+        ref = np.linalg.norm(w)
+        v = w / ref
+    assert lam == pytest.approx(ref, rel=1e-12)
+    rho = np.abs(np.linalg.eigvals(np.linalg.solve(D, Ad))).max()
+    assert 0.8 * rho < lam <= rho * (1 + 1e-12)            # a lower estimate of the spectral radius (D^-1 A ~ SPD)
+    assert orc.power_lambda(A, 3.7 * v0, 20) == pytest.approx(lam, rel=1e-14)    # the start vector is normalised
+    assert orc.power_lambda(A, v0, 1) != pytest.approx(lam, rel=1e-6)            # and the iteration count matters
+
+
 def test_prolongator_smooth_rejects_missing_diagonal():
     A = pr.HostBSR(2, 2, 2, 2, np.array([0, 1, 2], np.int32), np.array([1, 0], np.int32), np.ones((2, 2, 2)))
     Pt = pr.HostBSR(2, 1, 2, 3, np.array([0, 1, 2], np.int32), np.array([0, 0], np.int32), np.ones((2, 2, 3)))
