@@ -210,11 +210,17 @@ int vcycle_destroy(vcycle_t vc);
  *   (16-byte aligned) = values of P for the CURRENT values of A and P~ and the given omega.  A singular or missing
  *   diagonal block is reported by prolongator_smooth_status (COLD: synchronises) as BSR_ERR_NUMERIC.
  * prolongator_smooth_get_info: block products A(i,j)*P~(j,J), algorithmic bytes bytes(A)+bytes(P~)+bytes(P), and
- *   whether the staged kernel (1) or the gather fallback (0) runs. */
+ *   whether the staged kernel (1) or the gather fallback (0) runs.
+ * prolongator_smooth_lambda (COLD: allocates two work vectors at first use, synchronises): the eigenvalue estimate of
+ *   D^-1 A the damping is derived from (omega = 4 / (3 lambda), reading R10): v <- v0/||v0||_2, then `iters`
+ *   times w = D^-1 (A v), lambda = ||w||_2, v = w / lambda, entirely on the device (bsr_spmv's kernel, a block-diagonal
+ *   apply with a fixed-order norm); *lambda (HOST) receives the last lambda.  d_v0[nbrows*bs] is not modified. */
 int prolongator_smooth_symbolic(psmooth_plan_t* out, bsr_t A, bsr_t P_tent, int64_t* nnzb_p, void* stream);
 int prolongator_smooth_structure(psmooth_plan_t plan, int32_t* d_rowptr_p, int32_t* d_colidx_p, void* stream);
 int prolongator_smooth_numeric(psmooth_plan_t plan, bsr_t A, bsr_t P_tent, double omega, double* d_vals_p,
                                void* stream);
+int prolongator_smooth_lambda(psmooth_plan_t plan, bsr_t A, const double* d_v0, int32_t iters, double* lambda,
+                              void* stream);
 int prolongator_smooth_status(psmooth_plan_t plan, void* stream);
 int prolongator_smooth_get_info(psmooth_plan_t plan, int64_t* n_products, int64_t* algorithmic_bytes, int32_t* staged);
 int prolongator_smooth_destroy(psmooth_plan_t plan);

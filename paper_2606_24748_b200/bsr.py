@@ -61,6 +61,7 @@ SYMBOLS = {
     "prolongator_smooth_symbolic": (C.c_int, [_PV, _V, _V, _PI64, _V]),
     "prolongator_smooth_structure": (C.c_int, [_V, _V, _V, _V]),
     "prolongator_smooth_numeric": (C.c_int, [_V, _V, _V, _D, _V, _V]),
+    "prolongator_smooth_lambda": (C.c_int, [_V, _V, _V, _I32, C.POINTER(_D), _V]),
     "prolongator_smooth_status": (C.c_int, [_V, _V]),
     "prolongator_smooth_get_info": (C.c_int, [_V, _PI64, _PI64, _PI32]),
     "prolongator_smooth_destroy": (C.c_int, [_V]),
@@ -390,6 +391,14 @@ class ProlongatorSmoother:
         if check:
             _check(lib().prolongator_smooth_status(self.h, _stream()))
         return vals_p
+
+    def lambda_estimate(self, v0, iters: int = 20) -> float:
+        """lambda of D^-1 A after `iters` power iterations from v0 on the device (prolongator_smooth_lambda);
+        omega = 4 / (3 lambda)."""
+        lam = C.c_double()
+        assert v0.numel() == self.A.nbrows * self.A.bs_r
+        _check(lib().prolongator_smooth_lambda(self.h, self.A.h, _dev(v0), int(iters), C.byref(lam), _stream()))
+        return lam.value
 
     def matrix(self, vals_p) -> Bsr:
         """Wrap P (structure of the plan, given values) as a Bsr."""

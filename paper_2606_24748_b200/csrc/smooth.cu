@@ -27,6 +27,7 @@ struct psmooth_plan_s {
   void* pairs = nullptr;
   double* dinv = nullptr;
   int* status = nullptr;
+  double *pw_v = nullptr, *pw_t = nullptr, *pw_part = nullptr, *pw_scal = nullptr;   // power iteration (first use)
   bsramg::StreamDev s1;
 };
 static const uint64_t PSM_MAGIC = 0x50534d4f4f544831ull;
@@ -87,8 +88,77 @@ static int smooth_gather_launch(psmooth_plan_s* pl, double omega, double* d_vals
   return BSR_OK;
 }
 
+// ---- lambda of D^-1 A by power iteration (reading R10), all on the device, fixed summation order
+constexpr int PW_BLOCKS = 592;   // 4 per SM on 148 SMs; fixed so that the order of the norm's partial sums never changes
+
+// w = D^-1 t in place (block row wise); partial[blockIdx] = sum of w^2 over this CTA's rows
+template <int BS>
+__global__ void __launch_bounds__(256)
+dinv_apply_norm_kernel(int64_t nbrows, const double* __restrict__ dinv, double* __restrict__ t, double* __restrict__ partial) {
+  __shared__ double sh[8];
+  double s = 0.0;
+  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < nbrows; i += (int64_t)gridDim.x * blockDim.x) {
+    double r[BS], w[BS];
+#pragma unroll
+    for (int b = 0; b < BS; ++b) r[b] = t[i * BS + b];
+#pragma unroll
+    for (int a = 0; a < BS; ++a) {
+      double z = 0.0;
+#pragma unroll
+      for (int b = 0; b < BS; ++b) z = fma(dinv[(i * BS + a) * BS + b], r[b], z);
+      w[a] = z;
+      s = fma(z, z, s);
+    }
+#pragma unroll
+    for (int a = 0; a < BS; ++a) t[i * BS + a] = w[a];
+  }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
+  if ((threadIdx.x & 31) == 0) sh[threadIdx.x >> 5] = s;
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    double tt = 0.0;
+    for (int w = 0; w < 8; ++w) tt += sh[w];
+    partial[blockIdx.x] = tt;
+  }
+}
+
+__global__ void __launch_bounds__(256)
+sumsq_partial_kernel(int64_t n, const double* __restrict__ v, double* __restrict__ partial) {
+  __shared__ double sh[8];
+  double s = 0.0;
+  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) s = fma(v[i], v[i], s);
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
+  if ((threadIdx.x & 31) == 0) sh[threadIdx.x >> 5] = s;
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    double tt = 0.0;
+    for (int w = 0; w < 8; ++w) tt += sh[w];
+    partial[blockIdx.x] = tt;
+  }
+}
+
+// scal[0] = sqrt(sum(partial))
+__global__ void __launch_bounds__(32)
+norm_final_kernel(int nparts, const double* __restrict__ partial, double* __restrict__ scal) {
+  double s = 0.0;
+  for (int i = threadIdx.x; i < nparts; i += 32) s += partial[i];
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
+  if (threadIdx.x == 0) scal[0] = sqrt(s);
+}
+
+// v = w / scal[0]
+__global__ void __launch_bounds__(256)
+scale_by_norm_kernel(int64_t n, const double* __restrict__ w, const double* __restrict__ scal, double* __restrict__ v) {
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < n) v[i] = w[i] / scal[0];
+}
+
 static void psmooth_release(psmooth_plan_s* pl) {
   if (!pl) return;
+  dev_free(pl->pw_v); dev_free(pl->pw_t); dev_free(pl->pw_part); dev_free(pl->pw_scal);
   dev_free(pl->rowptr_p); dev_free(pl->colidx_p); dev_free(pl->out_row); dev_free(pl->own_slot);
   dev_free(pl->pairptr); dev_free(pl->pstart); dev_free(pl->pairs); dev_free(pl->dinv); dev_free(pl->status);
   stream_release(pl->s1);
@@ -210,6 +280,43 @@ int prolongator_smooth_numeric(psmooth_plan_t pl, bsr_t A, bsr_t Pt, double omeg
     case 66: return smooth_gather_launch<6, 6>(pl, omega, d_vals_p, st);
   }
   return fail(BSR_ERR_BLOCK, "unsupported block shapes in prolongator smoothing");
+}
+
+int prolongator_smooth_lambda(psmooth_plan_t pl, bsr_t A, const double* d_v0, int32_t iters, double* lambda, void* stream) {
+  if (!pl || pl->magic != PSM_MAGIC) return fail(BSR_ERR_NULL, "invalid plan handle");
+  if (!A || A->magic != BSR_MAGIC || A != pl->A) return fail(BSR_ERR_PLAN, "plan was built from a different matrix");
+  if (!d_v0 || !lambda) return fail(BSR_ERR_NULL, "null argument");
+  if (iters < 1) return fail(BSR_ERR_SHAPE, "iters must be positive");
+  if ((uintptr_t)d_v0 & 15) return fail(BSR_ERR_ALIGN, "d_v0 must be 16-byte aligned");
+  cudaStream_t st = (cudaStream_t)stream;
+  NvtxRange nv("prolongator_smooth_lambda");
+  const int64_t n = (int64_t)A->nbrows * A->bs_r;
+  if (!pl->pw_v) {   // cold: work vectors at first use
+    BSR_TRY(dev_alloc_t(&pl->pw_v, (size_t)n));
+    BSR_TRY(dev_alloc_t(&pl->pw_t, (size_t)n));
+    BSR_TRY(dev_alloc_t(&pl->pw_part, (size_t)PW_BLOCKS));
+    BSR_TRY(dev_alloc_t(&pl->pw_scal, 2));
+  }
+  BSR_TRY(block_diag_inverse(A, pl->dinv, pl->status, st));
+  const unsigned gv = (unsigned)((n + 255) / 256);
+  // v <- v0 / ||v0||
+  LAUNCH(sumsq_partial_kernel, PW_BLOCKS, 256, 0, st, n, d_v0, pl->pw_part);
+  LAUNCH(norm_final_kernel, 1, 32, 0, st, PW_BLOCKS, pl->pw_part, pl->pw_scal);
+  LAUNCH(scale_by_norm_kernel, gv, 256, 0, st, n, d_v0, pl->pw_scal, pl->pw_v);
+  for (int it = 0; it < iters; ++it) {
+    BSR_TRY(spmv_launch(A, pl->pw_v, pl->pw_t, nullptr, EPI_ASSIGN, st));               // t = A v
+    switch (A->bs_r) {                                                                  // w = D^-1 t, ||w||^2 partials
+      case 2: LAUNCH(dinv_apply_norm_kernel<2>, PW_BLOCKS, 256, 0, st, (int64_t)A->nbrows, pl->dinv, pl->pw_t, pl->pw_part); break;
+      case 3: LAUNCH(dinv_apply_norm_kernel<3>, PW_BLOCKS, 256, 0, st, (int64_t)A->nbrows, pl->dinv, pl->pw_t, pl->pw_part); break;
+      case 6: LAUNCH(dinv_apply_norm_kernel<6>, PW_BLOCKS, 256, 0, st, (int64_t)A->nbrows, pl->dinv, pl->pw_t, pl->pw_part); break;
+      default: return fail(BSR_ERR_BLOCK, "unsupported block size %d", A->bs_r);
+    }
+    LAUNCH(norm_final_kernel, 1, 32, 0, st, PW_BLOCKS, pl->pw_part, pl->pw_scal);        // lambda = ||w||
+    LAUNCH(scale_by_norm_kernel, gv, 256, 0, st, n, pl->pw_t, pl->pw_scal, pl->pw_v);    // v = w / lambda
+  }
+  CUDA_TRY(cudaMemcpyAsync(lambda, pl->pw_scal, sizeof(double), cudaMemcpyDeviceToHost, st));
+  CUDA_TRY(cudaStreamSynchronize(st));
+  return BSR_OK;
 }
 
 int prolongator_smooth_status(psmooth_plan_t pl, void* stream) {

@@ -91,6 +91,33 @@ def test_prolongator_smooth_small(bsr, name):
         bsr.set_option("ptap_force_gather", 0)
 
 
+@pytest.mark.parametrize("name", ["cfg0", "quad40", "level2_6x6", "cfg2"])
+def test_power_iteration_lambda_on_device(bsr, name):
+    """The eigenvalue estimate behind omega (reading R10) on the device against the oracle's power iteration; with it
+    new A -> omega -> new P needs no host arithmetic."""
+    if name == "cfg0":
+        g = pr.make_generator(0); g.build_prolongator(0); A, Pt, lvl = g.A(0), g.P_tent(0), 0
+    elif name == "quad40":
+        g = pr.Generator(2, 40, seed=1); g.build_prolongator(0); A, Pt, lvl = g.A(0), g.P_tent(0), 0
+    elif name == "level2_6x6":
+        g, A = level2_problem(3, 11, 4); Pt, lvl = g.P_tent(1), 1
+    else:
+        g = pr.make_generator(2); g.build_prolongator(0); A, Pt, lvl = g.A(0), g.P_tent(0), 0
+    v0 = pr.uniform(g.seed, pr.PURPOSE_POWER + 16 * lvl, A.nbrows * A.bs_r)
+    GA, GT = bsr.Bsr.from_host(A), bsr.Bsr.from_host(Pt)
+    sm = bsr.ProlongatorSmoother(GA, GT)
+    lam = sm.lambda_estimate(dev(v0), 20)
+    ref = orc.power_lambda(A, v0, 20)
+    assert abs(lam / ref - 1) < 1e-11, (lam, ref)
+    assert abs(lam / g.level_info(lvl)["lam"] - 1) < 1e-11           # = the generator's estimate
+    assert lam == sm.lambda_estimate(dev(v0), 20)                    # fixed summation order: bit-reproducible
+    # omega from the device estimate gives the oracle's P
+    om = 4.0 / (3.0 * lam)
+    got = sm.numeric(om, check=True).cpu().numpy()
+    refP = orc.prolongator_smooth(A, Pt, 4.0 / (3.0 * ref))
+    assert blockwise_rel_err(got.reshape(refP.vals.shape), refP.vals) < 1e-11
+
+
 def test_ptap_on_device_built_prolongator(bsr):
     """New A -> new P -> new A_c without the host: smooth on the device, then ptap_numeric on that P."""
     g = pr.Generator(3, 12, seed=6, modulus_mode=1)
