@@ -205,6 +205,7 @@ struct StreamPlan {
   std::vector<StreamEntry> entries;
   std::vector<StreamPass> passes;
   std::vector<StreamMeta> meta;
+  std::vector<int32_t> brick_maxrow;   // per brick: the largest X row it reads (direct) / its C row (persist)
   int64_t nbricks() const { return (int64_t)bricks.size(); }
   int64_t nchunks() const { return (int64_t)chunks.size(); }
 };

@@ -30,7 +30,11 @@ struct ptap_plan_s {
   void *pairs1 = nullptr, *pairs2 = nullptr;
   double* vals_ap = nullptr;
   bsramg::StreamDev s1, s2;  // brick-staged schedules of the two stages (ok == false: gather kernels)
+  // the chunked host-buffer path (ptap_numeric_host): a copy stream and events, created at its first use (cold)
+  cudaStream_t copy_stream = nullptr;
+  cudaEvent_t ev_main = nullptr, ev_copy[16] = {};
 };
+static const int HOST_CHUNKS_IN = 8, HOST_CHUNKS_OUT = 4;
 static const uint64_t PLAN_MAGIC = 0x5054415031303030ull;
 
 namespace bsramg {
@@ -147,6 +151,13 @@ int stream_upload(const StreamShape& sh, const StreamPlan& sp, StreamDev& sd, cu
   if (rc == BSR_OK && cudaStreamSynchronize(st) != cudaSuccess) rc = fail(BSR_ERR_CUDA, "stream plan upload failed");
   if (rc != BSR_OK) { stream_release(sd); return rc; }
   sd.ok = true; sd.persist = sp.persist; sd.nbricks = sp.nbricks(); sd.smem = sp.max_smem;
+  sd.brick_maxrow_prefix = sp.brick_maxrow;
+  for (size_t b = 1; b < sd.brick_maxrow_prefix.size(); ++b)
+    sd.brick_maxrow_prefix[b] = std::max(sd.brick_maxrow_prefix[b], sd.brick_maxrow_prefix[b - 1]);
+  if (sp.persist) {
+    sd.brick_out_end.resize(sp.bricks.size());
+    for (size_t b = 0; b < sp.bricks.size(); ++b) sd.brick_out_end[b] = sp.bricks[b].out + sp.bricks[b].nslots;
+  }
   return BSR_OK;
 }
 
@@ -242,6 +253,9 @@ static int upload_pairs(void** d, bool wide, const std::vector<uint16_t>& ox, co
 
 static void plan_release(ptap_plan_t pl) {
   if (!pl) return;
+  if (pl->copy_stream) cudaStreamDestroy(pl->copy_stream);
+  if (pl->ev_main) cudaEventDestroy(pl->ev_main);
+  for (cudaEvent_t e : pl->ev_copy) if (e) cudaEventDestroy(e);
   dev_free(pl->rowptr_ap); dev_free(pl->colidx_ap); dev_free(pl->rowidx_ap); dev_free(pl->pairptr1);
   dev_free(pl->pstart); dev_free(pl->rowptr_c); dev_free(pl->colidx_c); dev_free(pl->rowidx_c);
   dev_free(pl->pairptr2); dev_free(pl->apstart); dev_free(pl->pairs1); dev_free(pl->pairs2); dev_free(pl->vals_ap);
@@ -402,10 +416,75 @@ int ptap_numeric_host(ptap_plan_t pl, bsr_t A, bsr_t P, const double* h_vals_a, 
   if (!h_vals_a || !h_vals_c || !d_vals_c) return fail(BSR_ERR_NULL, "null array");
   if ((uintptr_t)d_vals_c & 15) return fail(BSR_ERR_ALIGN, "d_vals_c must be 16-byte aligned");
   cudaStream_t st = (cudaStream_t)stream;
-  CUDA_TRY(cudaMemcpyAsync(A->d_vals, h_vals_a, (size_t)A->nnzb * A->bs_r * A->bs_c * 8, cudaMemcpyHostToDevice, st));
+  const size_t bba = (size_t)A->bs_r * A->bs_c * 8, bbc = (size_t)pl->bc * pl->bc * 8;
+  if (!pl->s1.ok || !pl->s2.ok || pl->s1.nbricks < HOST_CHUNKS_IN || pl->s2.nbricks < HOST_CHUNKS_OUT) {
+    // gather plans / tiny problems: copy, compute, copy
+    CUDA_TRY(cudaMemcpyAsync(A->d_vals, h_vals_a, (size_t)A->nnzb * bba, cudaMemcpyHostToDevice, st));
+    A->state++;
+    BSR_TRY(ptap_numeric(pl, A, P, d_vals_c, stream));
+    CUDA_TRY(cudaMemcpyAsync(h_vals_c, d_vals_c, (size_t)pl->nnzb_c * bbc, cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(cudaStreamSynchronize(st));
+    return BSR_OK;
+  }
+  // staged plans: A's values arrive in row chunks on a copy stream; the bricks of stage 1 whose rows are complete are
+  // launched behind each chunk, so AP = A*P hides under the transfer; A_c leaves in pieces behind stage 2 the same way
+  if (!pl->copy_stream) {   // cold, once
+    CUDA_TRY(cudaStreamCreateWithFlags(&pl->copy_stream, cudaStreamNonBlocking));
+    CUDA_TRY(cudaEventCreateWithFlags(&pl->ev_main, cudaEventDisableTiming));
+    for (cudaEvent_t& e : pl->ev_copy) CUDA_TRY(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+  }
+  NvtxRange nv("ptap_numeric_host");
+  cudaStream_t cs = pl->copy_stream;
+  CUDA_TRY(cudaEventRecord(pl->ev_main, st));            // earlier work on `stream` may still read A's old values
+  CUDA_TRY(cudaStreamWaitEvent(cs, pl->ev_main, 0));
   A->state++;
-  BSR_TRY(ptap_numeric(pl, A, P, d_vals_c, stream));
-  CUDA_TRY(cudaMemcpyAsync(h_vals_c, d_vals_c, (size_t)pl->nnzb_c * pl->bc * pl->bc * 8, cudaMemcpyDeviceToHost, st));
+  BSR_TRY(transpose_ensure(P, st));                      // state gate
+  const std::vector<int32_t>& rp = A->h_rowptr;
+  const std::vector<int32_t>& need = pl->s1.brick_maxrow_prefix;
+  int32_t row0 = 0;
+  int64_t b0 = 0;
+  for (int g = 0; g < HOST_CHUNKS_IN; ++g) {
+    // rows [row0, row1): about 1/8 of the blocks each
+    const int64_t target = A->nnzb * (g + 1) / HOST_CHUNKS_IN;
+    int32_t row1 = (g + 1 == HOST_CHUNKS_IN) ? A->nbrows
+                                             : (int32_t)(std::upper_bound(rp.begin(), rp.end(), (int32_t)target) - rp.begin() - 1);
+    row1 = std::max(row1, row0);
+    const size_t o0 = (size_t)rp[(size_t)row0] * bba, o1 = (size_t)rp[(size_t)row1] * bba;
+    if (o1 > o0)
+      CUDA_TRY(cudaMemcpyAsync((char*)A->d_vals + o0, (const char*)h_vals_a + o0, o1 - o0, cudaMemcpyHostToDevice, cs));
+    CUDA_TRY(cudaEventRecord(pl->ev_copy[g], cs));
+    CUDA_TRY(cudaStreamWaitEvent(st, pl->ev_copy[g], 0));
+    // leading bricks that read no row at or beyond row1
+    const int64_t b1 = (g + 1 == HOST_CHUNKS_IN)
+                           ? pl->s1.nbricks
+                           : (int64_t)(std::lower_bound(need.begin(), need.end(), row1) - need.begin());
+    if (b1 > b0) {
+      StreamArgs a = pl->s1.args;
+      a.xvals = A->d_vals; a.yvals = P->d_vals; a.cvals = pl->vals_ap; a.brick0 = (int32_t)b0;
+      BSR_TRY(stream_launch(pl->bf, pl->bf, pl->bc, a, false, b1 - b0, pl->s1.smem, st));
+      b0 = b1;
+    }
+    row0 = row1;
+  }
+  // stage 2 in pieces; each piece's rows of A_c go home as soon as it is done
+  bsr_t R = P->T;
+  int64_t c0 = 0;
+  size_t out0 = 0;
+  for (int g = 0; g < HOST_CHUNKS_OUT; ++g) {
+    const int64_t c1 = pl->s2.nbricks * (g + 1) / HOST_CHUNKS_OUT;
+    if (c1 <= c0) continue;
+    StreamArgs a = pl->s2.args;
+    a.xvals = R->d_vals; a.yvals = pl->vals_ap; a.cvals = d_vals_c; a.brick0 = (int32_t)c0;
+    BSR_TRY(stream_launch(pl->bc, pl->bf, pl->bc, a, true, c1 - c0, pl->s2.smem, st));
+    CUDA_TRY(cudaEventRecord(pl->ev_copy[HOST_CHUNKS_IN + g], st));
+    CUDA_TRY(cudaStreamWaitEvent(cs, pl->ev_copy[HOST_CHUNKS_IN + g], 0));
+    const size_t out1 = (size_t)pl->s2.brick_out_end[(size_t)c1 - 1] * bbc;   // bricks write A_c in slot order
+    if (out1 > out0)
+      CUDA_TRY(cudaMemcpyAsync((char*)h_vals_c + out0, (const char*)d_vals_c + out0, out1 - out0, cudaMemcpyDeviceToHost, cs));
+    out0 = out1;
+    c0 = c1;
+  }
+  CUDA_TRY(cudaStreamSynchronize(cs));
   CUDA_TRY(cudaStreamSynchronize(st));
   return BSR_OK;
 }

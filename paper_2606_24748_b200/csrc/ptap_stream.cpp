@@ -244,6 +244,10 @@ void stream_build(const StreamShape& sh, int nwarps, int64_t smem_budget, const 
   for (const auto& lb : L) nchunks += (int64_t)lb.chunks.size();
   out.bricks.resize((size_t)nb);
   out.chunks.resize((size_t)nchunks);
+  out.brick_maxrow.assign((size_t)nb, 0);
+  for (int64_t b = 0; b < nb; ++b)
+    for (const auto& cd : bricks[(size_t)b].chunks)
+      for (const auto& pc : cd.pieces) out.brick_maxrow[(size_t)b] = std::max(out.brick_maxrow[(size_t)b], pc.row);
   int64_t c = 0, nxr = 0, nyr = 0, nen = 0, npa = 0, nme = 0;
   for (int64_t b = 0; b < nb; ++b) {
     const LocalBrick& lb = L[(size_t)b];

@@ -102,7 +102,7 @@ stream_product_kernel(const StreamArgs a) {
   constexpr int MK = M * K, KN = K * N, MN = M * N, XS = (MK + 1) & ~1, NW = NT / 32;
   extern __shared__ __align__(16) unsigned char smem[];
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  const int b = blockIdx.x;
+  const int b = blockIdx.x + a.brick0;
   // brick and chunk headers: one 16-byte and one 64-byte broadcast load (a direct brick is its own single chunk, so
   // both loads are issued together)
   const int4 bh = __ldg(reinterpret_cast<const int4*>(a.bricks + b));  // chunk0, nchunks, out, nslots

@@ -25,6 +25,7 @@ struct StreamArgs {  // all device pointers
   const int32_t* out_row = nullptr;   // per output slot: its row
   const int32_t* own_slot = nullptr;  // per output slot: the tentative block with the same coordinate, or -1
   double omega = 0.0;
+  int32_t brick0 = 0;                 // first brick of this launch (a plan may be launched in several pieces)
 };
 
 // device copy of a StreamPlan
@@ -33,6 +34,9 @@ struct StreamDev {
   int64_t nbricks = 0, smem = 0, bytes = 0;
   StreamArgs args{};
   std::vector<void*> owned;
+  // host copies for the chunked host-buffer path: the largest X row every leading run of bricks needs (direct plans)
+  // and, for persist plans, the end of every brick's output in C slots
+  std::vector<int32_t> brick_maxrow_prefix, brick_out_end;
 };
 
 int stream_upload(const StreamShape& sh, const StreamPlan& sp, StreamDev& sd, cudaStream_t st, bool smooth = false);

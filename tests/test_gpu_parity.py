@@ -327,3 +327,25 @@ def test_workspace_comes_from_the_callers_allocator(bsr, probs):
         bsr.use_torch_allocator(True)
     plan2 = bsr.PtapPlan(GA, GP2)                               # and the library works again afterwards
     assert torch.equal(plan2.numeric(), v)
+
+
+def test_ptap_host_buffer_path_is_chunked_and_exact(bsr, probs):
+    """ptap_numeric_host: A's values arrive from a HOST buffer in row chunks on a copy stream, stage 1 runs behind the
+    chunks, A_c leaves in pieces behind stage 2 -- the result must be bit-identical to ptap_numeric on device values,
+    call after call with changing values."""
+    import torch
+    for name in ("hex13", "quad40", "cfg0"):
+        g = probs[name]
+        A, P = g.A(0), g.P(0)
+        GA, GP = bsr.Bsr.from_host(A), bsr.Bsr.from_host(P)
+        plan = bsr.PtapPlan(GA, GP)
+        vals_c = plan.new_values()
+        hc = torch.empty(vals_c.numel(), dtype=torch.float64).pin_memory()
+        for k, scale in enumerate((1.0, 0.37, 2.5)):
+            ha = torch.from_numpy(np.ascontiguousarray(A.vals.reshape(-1) * scale)).pin_memory()
+            plan.numeric_host(ha.numpy(), hc.numpy(), vals_c)
+            GA2 = bsr.Bsr.from_host(pr.HostBSR(A.nbrows, A.nbcols, A.bs_r, A.bs_c, A.rowptr, A.colidx, A.vals * scale))
+            ref = bsr.PtapPlan(GA2, GP).numeric()
+            assert torch.equal(vals_c, ref), (name, k)
+            assert np.array_equal(hc.numpy(), ref.cpu().numpy()), (name, k)
+            assert np.array_equal(GA.vals.cpu().numpy(), ha.numpy())        # the device copy of A holds the new values
