@@ -1,12 +1,14 @@
-// dense_gemm.cu -- register-tiled fp64 GEMM for the coarsest-level factorisation (vcycle_refresh).
+// dense_gemm.cu -- fp64 tensor-core (DMMA) GEMM for the coarsest-level factorisation (vcycle_refresh).
 //
 // The coarsest operator of the V-cycle is "solved dense on device" (BASELINE.json config 4; reading R17):
 // a blocked Cholesky factorisation and the explicit triangular inverse that turns every later solve into two
-// mat-vecs.  Both are built from ONE kernel, C = beta*C + alpha * A * op(B) on 128x128 tiles: 256 threads, an 8x8
-// accumulator tile per thread held as a 4x4 grid of 2x2 patches (so that every shared-memory read is a conflict-free
-// 16-byte load and every global access a coalesced 16-byte one), k in chunks of 16 through shared memory with the next
-// chunk prefetched into registers.  Plain fp64 FMAs: the tensor cores' fp64 rate equals the vector pipe's on this part
-// and the operands here come with triangular structure (k-ranges per tile) rather than tensor-core friendly shapes.
+// mat-vecs.  Both are built from ONE kernel, C = beta*C + alpha * A * op(B) on 128x128 tiles: 256 threads, k in chunks of
+// 16 through shared memory with the next chunk prefetched into registers, and the products on the fp64 tensor-core path
+// (mma.sync m8n8k4, DMMA): a warp owns a 32x64 piece of the tile as 4x8 fragments of 8x8, so a k-step of 4 costs 12
+// 8-byte shared-memory loads per lane for 32 MMAs.  The DMMA rate equals the plain FMA rate on this part (37 TFLOP/s
+// either way, measured); what the tensor path buys is operand traffic: the register-tiled FMA version of this kernel
+// (8x8 per thread) needed 8 LDS.128 per 64 FMAs, which kept the shared-memory pipe as busy as the fp64 pipe and held
+// the kernel to ~12.5 TFLOP/s.  Triangular and banded operands arrive as k-ranges per tile.
 // All matrices are row-major; m and n multiples of 128, k ranges multiples of 16 (the caller pads).
 #include "internal.h"
 
@@ -29,14 +31,14 @@ dgemm128_kernel(int k, double alpha, const double* __restrict__ A, int64_t lda, 
   kend = min(kend, kcap);                           // B has no nonzero row at or beyond kcap
   __shared__ __align__(16) double As[GK][GS];
   __shared__ __align__(16) double Bs[GK][GS];
-  const int tid = threadIdx.x, tx = tid & 15, ty = tid >> 4;
-  double acc[4][2][4][2];
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int wm = (warp & 3) * 32, wn = (warp >> 2) * 64;      // this warp's 32 x 64 piece of the tile
+  const int fk = lane & 3, fr = lane >> 2;                     // fragment coordinates of this lane
+  double acc[4][8][2];
 #pragma unroll
-  for (int g = 0; g < 4; ++g)
+  for (int i = 0; i < 4; ++i)
 #pragma unroll
-    for (int a = 0; a < 2; ++a)
-#pragma unroll
-      for (int h = 0; h < 4; ++h) acc[g][a][h][0] = acc[g][a][h][1] = 0.0;
+    for (int j = 0; j < 8; ++j) acc[i][j][0] = acc[i][j][1] = 0.0;
   // staging roles: A (and B when TRANSB): row tid/2, eight k values at (tid&1)*8;  B (k x n): k rows tid/32 and
   // tid/32 + 8, four columns each
   const int ar = tid >> 1, ak = (tid & 1) * 8;
@@ -73,41 +75,37 @@ dgemm128_kernel(int k, double alpha, const double* __restrict__ A, int64_t lda, 
     __syncthreads();
     if (kk + GK < kend) fetch(kk + GK);             // next chunk in flight while this one is multiplied
 #pragma unroll
-    for (int q = 0; q < GK; ++q) {
-      double2 a2[4], b2[4];
+    for (int q = 0; q < GK; q += 4) {
+      double af[4], bf[8];
 #pragma unroll
-      for (int g = 0; g < 4; ++g) a2[g] = *reinterpret_cast<const double2*>(&As[q][ty * 2 + 32 * g]);
+      for (int i = 0; i < 4; ++i) af[i] = As[q + fk][wm + 8 * i + fr];
 #pragma unroll
-      for (int h = 0; h < 4; ++h) b2[h] = *reinterpret_cast<const double2*>(&Bs[q][tx * 2 + 32 * h]);
+      for (int j = 0; j < 8; ++j) bf[j] = Bs[q + fk][wn + 8 * j + fr];
 #pragma unroll
-      for (int g = 0; g < 4; ++g)
+      for (int i = 0; i < 4; ++i)
 #pragma unroll
-        for (int h = 0; h < 4; ++h) {
-          acc[g][0][h][0] = fma(a2[g].x, b2[h].x, acc[g][0][h][0]);
-          acc[g][0][h][1] = fma(a2[g].x, b2[h].y, acc[g][0][h][1]);
-          acc[g][1][h][0] = fma(a2[g].y, b2[h].x, acc[g][1][h][0]);
-          acc[g][1][h][1] = fma(a2[g].y, b2[h].y, acc[g][1][h][1]);
-        }
+        for (int j = 0; j < 8; ++j)
+          asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
+                       : "+d"(acc[i][j][0]), "+d"(acc[i][j][1]) : "d"(af[i]), "d"(bf[j]));
     }
     __syncthreads();
   }
+  // fragment (i, j): row 8 i + lane / 4, columns 8 j + 2 (lane % 4) + {0, 1}
 #pragma unroll
-  for (int g = 0; g < 4; ++g)
+  for (int i = 0; i < 4; ++i) {
+    double* crow = C + (int64_t)(m0 + wm + 8 * i + fr) * ldc + n0 + wn + 2 * fk;
 #pragma unroll
-    for (int a = 0; a < 2; ++a) {
-      double* crow = C + (int64_t)(m0 + ty * 2 + 32 * g + a) * ldc + n0 + tx * 2;
-#pragma unroll
-      for (int h = 0; h < 4; ++h) {
-        double2* cp = reinterpret_cast<double2*>(crow + 32 * h);
-        double2 v = make_double2(alpha * acc[g][a][h][0], alpha * acc[g][a][h][1]);
-        if (beta != 0.0) {
-          const double2 o = *cp;
-          v.x = fma(beta, o.x, v.x);
-          v.y = fma(beta, o.y, v.y);
-        }
-        *cp = v;
+    for (int j = 0; j < 8; ++j) {
+      double2* cp = reinterpret_cast<double2*>(crow + 8 * j);
+      double2 v = make_double2(alpha * acc[i][j][0], alpha * acc[i][j][1]);
+      if (beta != 0.0) {
+        const double2 o = *cp;
+        v.x = fma(beta, o.x, v.x);
+        v.y = fma(beta, o.y, v.y);
       }
+      *cp = v;
     }
+  }
 }
 
 int dgemm128(bool transB, int m, int n, int k, double alpha, const double* A, int64_t lda, const double* B, int64_t ldb,

@@ -190,41 +190,54 @@ dense_fill_kernel(int64_t nvals, int bs, const int32_t* __restrict__ rowidx_of_s
   dense[((int64_t)rowidx_of_slot[k] * bs + r) * npad + (int64_t)colidx[k] * bs + c] = vals[e];
 }
 
-// factor the diagonal tile j in place (lower Cholesky) and store its inverse in diaginv[j]
-__global__ void __launch_bounds__(TS * TS)
+// factor the diagonal tile j in place (lower Cholesky) and store its inverse in diaginv[j].
+// The 32 steps are a dependent chain (pivot -> 1/sqrt -> column -> update of the next pivot), so ONE warp runs them out
+// of registers with no barrier: lane r holds row r of the tile and COLUMN r of X = L^-1 (forward substitution of the
+// identity with each column of L as soon as it is final), so that the value both updates need in step k,
+// l_i = L[i][k], comes from the same shuffle:
+//   a[r][i] -= l_r l_i  (k < i <= r)        X[i][c] -= l_i X[k][c]  (c <= k < i, lane c)
+// Both run unpredicated: l_r is 0 for r <= k, X[k][c] is still exactly 0 for c > k, and what lands above the diagonal
+// of a row is never read.  The pivot's reciprocal square root (rsqrt, <= 1 ulp) replaces sqrt followed by divisions on
+// the critical path; L[k][k] itself is p * rsqrt(p).
+__global__ void __launch_bounds__(TS)
 potrf_tile_kernel(int64_t npad, int j, double* __restrict__ dense, double* __restrict__ diaginv,
                   int* __restrict__ status) {
   __shared__ double a[TS][TS + 1];
-  __shared__ double inv[TS][TS + 1];
-  const int tx = threadIdx.x, ty = threadIdx.y;
+  const int r = threadIdx.x;
   double* tile = dense + ((int64_t)j * TS) * npad + (int64_t)j * TS;
-  a[ty][tx] = tile[(int64_t)ty * npad + tx];
-  inv[ty][tx] = (tx == ty) ? 1.0 : 0.0;
-  __syncthreads();
-  // right-looking Cholesky of the tile and, with the same column of L as soon as it is final, forward substitution of
-  // the identity (X <- L^-1): every step updates the whole trailing part of both with all 1024 threads
+#pragma unroll
+  for (int y = 0; y < TS; ++y) a[y][r] = tile[(int64_t)y * npad + r];
+  __syncwarp();
+  double ar[TS], xc[TS];
+#pragma unroll
+  for (int c = 0; c < TS; ++c) { ar[c] = a[r][c]; xc[c] = (c == r) ? 1.0 : 0.0; }
+  __syncwarp();
+  bool bad = false;
+#pragma unroll
   for (int k = 0; k < TS; ++k) {
-    if (tx == k && ty == k) {
-      double p = a[k][k];
-      if (!(p > 0.0)) { atomicOr(status, 2); p = 1.0; }
-      a[k][k] = sqrt(p);
+    double p = __shfl_sync(0xffffffffu, ar[k], k);
+    if (!(p > 0.0)) { bad = true; p = 1.0; }
+    const double rd = rsqrt(p);
+    const double l = (r > k) ? ar[k] * rd : 0.0;             // L[r][k] below the diagonal
+    ar[k] = (r == k) ? p * rd : l;
+    xc[k] *= rd;                                              // row k of X (zero right of the diagonal)
+    const double xk = xc[k];
+#pragma unroll
+    for (int i = k + 1; i < TS; ++i) {
+      const double li = __shfl_sync(0xffffffffu, l, i);
+      ar[i] = fma(-l, li, ar[i]);
+      xc[i] = fma(-li, xk, xc[i]);
     }
-    __syncthreads();
-    const double d = a[k][k];
-    if (tx == k && ty > k) a[ty][k] /= d;
-    if (ty == k && tx <= k) inv[k][tx] /= d;
-    __syncthreads();
-    if (ty > k) {
-      const double l = a[ty][k];
-      if (tx > k && ty >= tx) a[ty][tx] = fma(-l, a[tx][k], a[ty][tx]);
-      if (tx <= k) inv[ty][tx] = fma(-l, inv[k][tx], inv[ty][tx]);
-    }
-    __syncthreads();
   }
-  if (tx > ty) a[ty][tx] = 0.0;
-  __syncthreads();
-  tile[(int64_t)ty * npad + tx] = a[ty][tx];
-  diaginv[((int64_t)j * TS + ty) * TS + tx] = inv[ty][tx];
+  if (bad && r == 0) atomicOr(status, 2);
+#pragma unroll
+  for (int c = 0; c < TS; ++c) a[r][c] = (c <= r) ? ar[c] : 0.0;
+  __syncwarp();
+#pragma unroll
+  for (int y = 0; y < TS; ++y) tile[(int64_t)y * npad + r] = a[y][r];
+  // X: lane r holds column r, X[i][r] = xc[i] for i >= r
+#pragma unroll
+  for (int y = 0; y < TS; ++y) diaginv[((int64_t)j * TS + y) * TS + r] = (y >= r) ? xc[y] : 0.0;
 }
 
 // panel below the diagonal tile: L_ij = A_ij * inv(L_jj)^T for i = j+1+blockIdx.x
@@ -342,7 +355,7 @@ static int coarse_factor(vcycle_t vc, cudaStream_t st) {
   for (int J = 0; J < npan; ++J) {
     for (int s = 0; s < PT; ++s) {        // the panel itself, 32x32 tiles: factor, solve below, update the panel's own columns
       const int c = J * PT + s, rest = std::min(nb - c - 1, btiles), pc = PT - 1 - s;
-      LAUNCH(potrf_tile_kernel, 1, tb, 0, st, np, c, vc->dense, vc->diaginv, vc->d_status);
+      LAUNCH(potrf_tile_kernel, 1, TS, 0, st, np, c, vc->dense, vc->diaginv, vc->d_status);
       if (rest > 0) LAUNCH(trsm_tile_kernel, (unsigned)rest, tb, 0, st, np, c, vc->dense, vc->diaginv);
       if (rest > 0 && pc > 0) LAUNCH(syrk_tile_kernel, dim3(pc, rest), tb, 0, st, np, c, vc->dense);
     }
