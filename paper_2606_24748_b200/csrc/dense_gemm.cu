@@ -14,10 +14,11 @@
 
 namespace bsramg {
 
-constexpr int GT = 128, GK = 16, GS = GT + 4;   // tile, k-chunk, padded shared-memory row (doubles)
+constexpr int GK = 16;   // k-chunk
 
-template <bool TRANSB>
-__global__ void __launch_bounds__(256)
+// GT: the CTA's tile (128, or 64 for launches that would leave most SMs without a 128-tile); 2 GT threads
+template <int GT, bool TRANSB>
+__global__ void __launch_bounds__(2 * GT)
 dgemm128_kernel(int k, double alpha, const double* __restrict__ A, int64_t lda, const double* __restrict__ B,
                 int64_t ldb, double beta, double* __restrict__ C, int64_t ldc, int64_t sA, int64_t sB, int64_t sC,
                 int tri, int klim, int koff, int kcap) {
@@ -29,20 +30,22 @@ dgemm128_kernel(int k, double alpha, const double* __restrict__ A, int64_t lda, 
   if (klim == 2) kend = min(m0 + GT, k);            // A (m x k) is lower triangular: columns k >= m0+128 are zero
   kbeg = max(kbeg, min((koff + m0) & ~(GK - 1), k));   // A banded: row m0 + i is zero left of column koff + m0 + i
   kend = min(kend, kcap);                           // B has no nonzero row at or beyond kcap
+  constexpr int GS = GT + 4;                        // padded shared-memory row: fragment loads hit 16 distinct banks
+  constexpr int NJ = GT / 16;                       // 8x8 fragments across the warp's piece (32 x GT/2)
   __shared__ __align__(16) double As[GK][GS];
   __shared__ __align__(16) double Bs[GK][GS];
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  const int wm = (warp & 3) * 32, wn = (warp >> 2) * 64;      // this warp's 32 x 64 piece of the tile
+  const int wm = (warp % (GT / 32)) * 32, wn = (warp / (GT / 32)) * (GT / 2);   // this warp's 32 x GT/2 piece
   const int fk = lane & 3, fr = lane >> 2;                     // fragment coordinates of this lane
-  double acc[4][8][2];
+  double acc[4][NJ][2];
 #pragma unroll
   for (int i = 0; i < 4; ++i)
 #pragma unroll
-    for (int j = 0; j < 8; ++j) acc[i][j][0] = acc[i][j][1] = 0.0;
-  // staging roles: A (and B when TRANSB): row tid/2, eight k values at (tid&1)*8;  B (k x n): k rows tid/32 and
-  // tid/32 + 8, four columns each
+    for (int j = 0; j < NJ; ++j) acc[i][j][0] = acc[i][j][1] = 0.0;
+  // staging roles: A (and B when TRANSB): row tid/2, eight k values at (tid&1)*8;  B (k x n): k rows bk and bk + 8,
+  // four columns each
   const int ar = tid >> 1, ak = (tid & 1) * 8;
-  const int bk = tid >> 5, bc = (tid & 31) * 4;
+  const int bk = tid / (GT / 4), bc = (tid % (GT / 4)) * 4;
   const double* ap = A + (int64_t)(m0 + ar) * lda + ak;
   const double* bp = TRANSB ? B + (int64_t)(n0 + ar) * ldb + ak : B + (int64_t)bk * ldb + n0 + bc;
   double2 pa[4], pb[4];
@@ -76,15 +79,15 @@ dgemm128_kernel(int k, double alpha, const double* __restrict__ A, int64_t lda, 
     if (kk + GK < kend) fetch(kk + GK);             // next chunk in flight while this one is multiplied
 #pragma unroll
     for (int q = 0; q < GK; q += 4) {
-      double af[4], bf[8];
+      double af[4], bf[NJ];
 #pragma unroll
       for (int i = 0; i < 4; ++i) af[i] = As[q + fk][wm + 8 * i + fr];
 #pragma unroll
-      for (int j = 0; j < 8; ++j) bf[j] = Bs[q + fk][wn + 8 * j + fr];
+      for (int j = 0; j < NJ; ++j) bf[j] = Bs[q + fk][wn + 8 * j + fr];
 #pragma unroll
       for (int i = 0; i < 4; ++i)
 #pragma unroll
-        for (int j = 0; j < 8; ++j)
+        for (int j = 0; j < NJ; ++j)
           asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
                        : "+d"(acc[i][j][0]), "+d"(acc[i][j][1]) : "d"(af[i]), "d"(bf[j]));
     }
@@ -95,7 +98,7 @@ dgemm128_kernel(int k, double alpha, const double* __restrict__ A, int64_t lda, 
   for (int i = 0; i < 4; ++i) {
     double* crow = C + (int64_t)(m0 + wm + 8 * i + fr) * ldc + n0 + wn + 2 * fk;
 #pragma unroll
-    for (int j = 0; j < 8; ++j) {
+    for (int j = 0; j < NJ; ++j) {
       double2* cp = reinterpret_cast<double2*>(crow + 8 * j);
       double2 v = make_double2(alpha * acc[i][j][0], alpha * acc[i][j][1]);
       if (beta != 0.0) {
@@ -112,13 +115,20 @@ int dgemm128(bool transB, int m, int n, int k, double alpha, const double* A, in
              double beta, double* C, int64_t ldc, int batch, int64_t sA, int64_t sB, int64_t sC, int tri, int klim,
              cudaStream_t st, int koff, int kcap) {
   if (m <= 0 || n <= 0 || batch <= 0) return BSR_OK;
-  if (m % GT || n % GT || k % GK || (lda & 1) || (ldb & 1) || (ldc & 1))
+  if (m % 128 || n % 128 || k % GK || (lda & 1) || (ldb & 1) || (ldc & 1))
     return fail(BSR_ERR_SHAPE, "dgemm128: sizes must be multiples of the tile (m %d n %d k %d)", m, n, k);
-  const dim3 grid((unsigned)(n / GT), (unsigned)(m / GT), (unsigned)batch);
   if (kcap <= 0 || kcap > k) kcap = k;
   if (koff < -(1 << 29)) koff = -(1 << 29);
-  if (transB) LAUNCH(dgemm128_kernel<true>, grid, 256, 0, st, k, alpha, A, lda, B, ldb, beta, C, ldc, sA, sB, sC, tri, klim, koff, kcap);
-  else LAUNCH(dgemm128_kernel<false>, grid, 256, 0, st, k, alpha, A, lda, B, ldb, beta, C, ldc, sA, sB, sC, tri, klim, koff, kcap);
+  // fewer 128-tiles than SMs: quarter tiles, four times the CTAs (a 128-tile is ~17 us of one SM's fp64 rate per 128 k)
+  const int64_t t128 = (int64_t)(m / 128) * (tri ? (n / 128 + 1) / 2 : n / 128) * batch;
+  const bool small = t128 < 148;
+  const int gt = small ? 64 : 128;
+  const dim3 grid((unsigned)(n / gt), (unsigned)(m / gt), (unsigned)batch);
+#define DGEMM_LAUNCH(GT, TB) \
+  LAUNCH((dgemm128_kernel<GT, TB>), grid, 2 * GT, 0, st, k, alpha, A, lda, B, ldb, beta, C, ldc, sA, sB, sC, tri, klim, koff, kcap)
+  if (small) { if (transB) DGEMM_LAUNCH(64, true); else DGEMM_LAUNCH(64, false); }
+  else       { if (transB) DGEMM_LAUNCH(128, true); else DGEMM_LAUNCH(128, false); }
+#undef DGEMM_LAUNCH
   return BSR_OK;
 }
 

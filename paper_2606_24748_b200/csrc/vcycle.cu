@@ -40,7 +40,7 @@ struct vcycle_s {
   // coarsest level, dense
   int64_t nc = 0, npad = 0;
   int64_t band = 0;   // scalar half-bandwidth of the coarsest operator, rounded up to whole panels (npad: not banded)
-  double *dense = nullptr, *diaginv = nullptr, *linv = nullptr, *linvT = nullptr, *ytmp = nullptr;
+  double *dense = nullptr, *linv = nullptr, *linvT = nullptr, *ytmp = nullptr;
   int32_t* coarse_rowidx = nullptr;   // block row of every stored block of the coarsest operator (dense fill)
   int* d_status = nullptr;
   // PCG work space
@@ -190,27 +190,30 @@ dense_fill_kernel(int64_t nvals, int bs, const int32_t* __restrict__ rowidx_of_s
   dense[((int64_t)rowidx_of_slot[k] * bs + r) * npad + (int64_t)colidx[k] * bs + c] = vals[e];
 }
 
-// factor the diagonal tile j in place (lower Cholesky) and store its inverse in diaginv[j].
-// The 32 steps are a dependent chain (pivot -> 1/sqrt -> column -> update of the next pivot), so ONE warp runs them out
-// of registers with no barrier: lane r holds row r of the tile and COLUMN r of X = L^-1 (forward substitution of the
-// identity with each column of L as soon as it is final), so that the value both updates need in step k,
-// l_i = L[i][k], comes from the same shuffle:
+// ---- the diagonal 128-block of a panel: Cholesky factor AND inverse in one CTA, all in shared memory.
+// The block lives as its ten lower 32x32 tiles (rows padded to PL doubles).  Per tile column s: one warp factors the
+// diagonal tile out of registers (below), then the tiles under it are solved (L_is = A_is X_ss^T) and the rest of the
+// block updated (A_ik -= L_is L_ks^T) on the fp64 tensor-core path, a 32x32 tile product shared by four warps (a 16x16
+// quadrant = 2x2 mma.sync m8n8k4 fragments each).  The inverse follows by the tile recurrence
+//   X_ij = -X_ii * sum_{k=j}^{i-1} L_ik X_kj   (i > j, one sub-diagonal after the other).
+constexpr int PANEL = 128, PT = PANEL / TS;
+constexpr int PL = 36;                                  // padded tile row: fragment loads hit 16 distinct banks
+constexpr int PTILES = PT * (PT + 1) / 2;
+constexpr int PANEL_SMEM = 2 * PTILES * TS * PL * 8;    // L tiles + X tiles: 184,320 bytes
+__device__ __forceinline__ int ltile(int i, int j) { return (i * (i + 1) / 2 + j) * TS * PL; }
+
+// The 32 steps of a tile are a dependent chain (pivot -> 1/sqrt -> column -> update of the next pivot), so ONE warp runs
+// them with no barrier: lane r holds row r of the tile and COLUMN r of X = L^-1 (forward substitution of the identity
+// with each column of L as soon as it is final), so that the value both updates need in step k, l_i = L[i][k], comes
+// from the same shuffle:
 //   a[r][i] -= l_r l_i  (k < i <= r)        X[i][c] -= l_i X[k][c]  (c <= k < i, lane c)
 // Both run unpredicated: l_r is 0 for r <= k, X[k][c] is still exactly 0 for c > k, and what lands above the diagonal
 // of a row is never read.  The pivot's reciprocal square root (rsqrt, <= 1 ulp) replaces sqrt followed by divisions on
 // the critical path; L[k][k] itself is p * rsqrt(p).
-__global__ void __launch_bounds__(TS)
-potrf_tile_kernel(int64_t npad, int j, double* __restrict__ dense, double* __restrict__ diaginv,
-                  int* __restrict__ status) {
-  __shared__ double a[TS][TS + 1];
-  const int r = threadIdx.x;
-  double* tile = dense + ((int64_t)j * TS) * npad + (int64_t)j * TS;
-#pragma unroll
-  for (int y = 0; y < TS; ++y) a[y][r] = tile[(int64_t)y * npad + r];
-  __syncwarp();
+__device__ __forceinline__ void potrf_warp(double* __restrict__ a, double* __restrict__ x, int r, int* status) {
   double ar[TS], xc[TS];
 #pragma unroll
-  for (int c = 0; c < TS; ++c) { ar[c] = a[r][c]; xc[c] = (c == r) ? 1.0 : 0.0; }
+  for (int c = 0; c < TS; ++c) { ar[c] = a[r * PL + c]; xc[c] = (c == r) ? 1.0 : 0.0; }
   __syncwarp();
   bool bad = false;
 #pragma unroll
@@ -231,83 +234,109 @@ potrf_tile_kernel(int64_t npad, int j, double* __restrict__ dense, double* __res
   }
   if (bad && r == 0) atomicOr(status, 2);
 #pragma unroll
-  for (int c = 0; c < TS; ++c) a[r][c] = (c <= r) ? ar[c] : 0.0;
-  __syncwarp();
+  for (int c = 0; c < TS; ++c) {
+    a[r * PL + c] = (c <= r) ? ar[c] : 0.0;
+    x[c * PL + r] = (c >= r) ? xc[c] : 0.0;                   // X[c][r]
+  }
+}
+
+// acc += A[qm.., :] * op(B)[:, qn..] over the 32 k of a tile; op(B)[k][n] = B[n][k] when TB (B given as n x k)
+template <bool TB>
+__device__ __forceinline__ void quad_mma(double (&acc)[2][2][2], const double* __restrict__ A,
+                                         const double* __restrict__ B, int qm, int qn, int lane) {
+  const int fk = lane & 3, fr = lane >> 2;
 #pragma unroll
-  for (int y = 0; y < TS; ++y) tile[(int64_t)y * npad + r] = a[y][r];
-  // X: lane r holds column r, X[i][r] = xc[i] for i >= r
+  for (int k0 = 0; k0 < TS; k0 += 4) {
+    double af[2], bf[2];
 #pragma unroll
-  for (int y = 0; y < TS; ++y) diaginv[((int64_t)j * TS + y) * TS + r] = (y >= r) ? xc[y] : 0.0;
+    for (int i = 0; i < 2; ++i) af[i] = A[(qm + 8 * i + fr) * PL + k0 + fk];
+#pragma unroll
+    for (int j = 0; j < 2; ++j) bf[j] = TB ? B[(qn + 8 * j + fr) * PL + k0 + fk] : B[(k0 + fk) * PL + qn + 8 * j + fr];
+#pragma unroll
+    for (int i = 0; i < 2; ++i)
+#pragma unroll
+      for (int j = 0; j < 2; ++j)
+        asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
+                     : "+d"(acc[i][j][0]), "+d"(acc[i][j][1]) : "d"(af[i]), "d"(bf[j]));
+  }
 }
 
-// panel below the diagonal tile: L_ij = A_ij * inv(L_jj)^T for i = j+1+blockIdx.x
-__global__ void __launch_bounds__(TS * TS)
-trsm_tile_kernel(int64_t npad, int j, double* __restrict__ dense, const double* __restrict__ diaginv) {
-  __shared__ double a[TS][TS + 1];
-  __shared__ double w[TS][TS + 1];
-  const int tx = threadIdx.x, ty = threadIdx.y;
-  const int i = j + 1 + blockIdx.x;
-  double* tile = dense + ((int64_t)i * TS) * npad + (int64_t)j * TS;
-  a[ty][tx] = tile[(int64_t)ty * npad + tx];
-  w[ty][tx] = diaginv[((int64_t)j * TS + ty) * TS + tx];
-  __syncthreads();
-  double s = 0.0;
-#pragma unroll 8
-  for (int k = 0; k < TS; ++k) s = fma(a[ty][k], w[tx][k], s);
-  tile[(int64_t)ty * npad + tx] = s;
+// C[quadrant] = beta * C + alpha * acc
+__device__ __forceinline__ void quad_store(double* __restrict__ C, const double (&acc)[2][2][2], int qm, int qn, int lane,
+                                           double alpha, double beta) {
+  const int fk = lane & 3, fr = lane >> 2;
+#pragma unroll
+  for (int i = 0; i < 2; ++i)
+#pragma unroll
+    for (int j = 0; j < 2; ++j) {
+      double2* cp = reinterpret_cast<double2*>(C + (qm + 8 * i + fr) * PL + qn + 8 * j + 2 * fk);
+      double2 v = make_double2(alpha * acc[i][j][0], alpha * acc[i][j][1]);
+      if (beta != 0.0) { const double2 o = *cp; v.x = fma(beta, o.x, v.x); v.y = fma(beta, o.y, v.y); }
+      *cp = v;
+    }
 }
 
-// trailing update: A_ik -= L_ij * L_kj^T for the lower tiles i >= k > j
-__global__ void __launch_bounds__(TS * TS)
-syrk_tile_kernel(int64_t npad, int j, double* __restrict__ dense) {
-  const int bi = j + 1 + blockIdx.y, bk = j + 1 + blockIdx.x;
-  if (bk > bi) return;
-  __shared__ double li[TS][TS + 1];
-  __shared__ double lk[TS][TS + 1];
-  const int tx = threadIdx.x, ty = threadIdx.y;
-  li[ty][tx] = dense[((int64_t)bi * TS + ty) * npad + (int64_t)j * TS + tx];
-  lk[ty][tx] = dense[((int64_t)bk * TS + ty) * npad + (int64_t)j * TS + tx];
+__global__ void __launch_bounds__(256)
+potrf_panel_kernel(int64_t npad, int J, double* __restrict__ dense, double* __restrict__ linv, int* __restrict__ status) {
+  extern __shared__ __align__(16) double panel_sm[];
+  double* Lt = panel_sm;
+  double* Xt = panel_sm + PTILES * TS * PL;
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int group = warp >> 2, qm = ((warp >> 1) & 1) * 16, qn = (warp & 1) * 16;   // two groups of four warps
+  double* blk = dense + ((int64_t)J * PANEL) * npad + (int64_t)J * PANEL;
+  double* xblk = linv + ((int64_t)J * PANEL) * npad + (int64_t)J * PANEL;
+  for (int e = tid; e < PTILES * TS * TS; e += 256) {
+    const int tl = e >> 10, r = (e >> 5) & 31, c = e & 31;
+    const int ti = (tl >= 6) ? 3 : (tl >= 3) ? 2 : (tl >= 1) ? 1 : 0, tj = tl - ti * (ti + 1) / 2;
+    Lt[tl * TS * PL + r * PL + c] = blk[(int64_t)(ti * TS + r) * npad + tj * TS + c];
+  }
   __syncthreads();
-  double s = 0.0;
-#pragma unroll 8
-  for (int m = 0; m < TS; ++m) s = fma(li[ty][m], lk[tx][m], s);
-  double* c = dense + ((int64_t)bi * TS + ty) * npad + (int64_t)bk * TS + tx;
-  *c -= s;
-}
-
-// X = L^-1 of one diagonal block, one CTA per tile column j, tile rows in order (each needs the ones above it in the
-// same column):  X_jj = inv(L_jj);  X_ij = -inv(L_ii) * sum_{k=j}^{i-1} L_ik X_kj
-// restricted to the PANEL x PANEL diagonal blocks (tiles 4J..4J+3 of block J = blockIdx.y): the base case of the
-// recursive-doubling inverse below
-constexpr int PANEL = 128, PT = PANEL / TS;
-__global__ void __launch_bounds__(TS * TS)
-trinv_block_kernel(int64_t npad, const double* __restrict__ dense, const double* __restrict__ diaginv, double* linv) {
-  __shared__ double a[TS][TS + 1];
-  __shared__ double b[TS][TS + 1];
-  const int tx = threadIdx.x, ty = threadIdx.y;
-  const int t0 = blockIdx.y * PT, j = t0 + blockIdx.x;
-  linv[((int64_t)j * TS + ty) * npad + (int64_t)j * TS + tx] = diaginv[((int64_t)j * TS + ty) * TS + tx];
-  __threadfence();
-  __syncthreads();
-  for (int i = j + 1; i < t0 + PT; ++i) {
-    double s = 0.0;
-    for (int k = j; k < i; ++k) {
-      a[ty][tx] = dense[((int64_t)i * TS + ty) * npad + (int64_t)k * TS + tx];
-      b[ty][tx] = linv[((int64_t)k * TS + ty) * npad + (int64_t)j * TS + tx];  // written by this CTA
+  for (int s = 0; s < PT; ++s) {
+    if (warp == 0) potrf_warp(Lt + ltile(s, s), Xt + ltile(s, s), lane, status);
+    __syncthreads();
+    const int nt = PT - 1 - s;
+    for (int j0 = 0; j0 < nt; j0 += 2) {                       // tiles below: L_is = A_is X_ss^T
+      const int i = s + 1 + j0 + group;
+      const bool on = j0 + group < nt;
+      double acc[2][2][2] = {};
+      if (on) quad_mma<true>(acc, Lt + ltile(i, s), Xt + ltile(s, s), qm, qn, lane);
+      __syncthreads();                                         // every quadrant has read the tile it is about to overwrite
+      if (on) quad_store(Lt + ltile(i, s), acc, qm, qn, lane, 1.0, 0.0);
+    }
+    __syncthreads();
+    const int njobs = nt * (nt + 1) / 2;                       // A_ik -= L_is L_ks^T, s < k <= i
+    for (int job = group; job < njobs; job += 2) {
+      const int di = (job >= 3) ? 2 : (job >= 1) ? 1 : 0, dk = job - di * (di + 1) / 2;
+      const int i = s + 1 + di, k = s + 1 + dk;
+      double acc[2][2][2] = {};
+      quad_mma<true>(acc, Lt + ltile(i, s), Lt + ltile(k, s), qm, qn, lane);
+      quad_store(Lt + ltile(i, k), acc, qm, qn, lane, -1.0, 1.0);
+    }
+    __syncthreads();
+  }
+  for (int d = 1; d < PT; ++d) {                               // X, one sub-diagonal of tiles after the other
+    const int nj = PT - d;
+    for (int j0 = 0; j0 < nj; j0 += 2) {
+      const int j = j0 + group, i = j + d;
+      const bool on = j < nj;
+      double acc[2][2][2] = {};
+      if (on) {
+        for (int k = j; k < i; ++k) quad_mma<false>(acc, Lt + ltile(i, k), Xt + ltile(k, j), qm, qn, lane);
+        quad_store(Xt + ltile(i, j), acc, qm, qn, lane, 1.0, 0.0);   // T = sum_k L_ik X_kj, staged in X_ij's place
+      }
       __syncthreads();
-#pragma unroll 8
-      for (int m = 0; m < TS; ++m) s = fma(a[ty][m], b[m][tx], s);
+      double acc2[2][2][2] = {};
+      if (on) quad_mma<false>(acc2, Xt + ltile(i, i), Xt + ltile(i, j), qm, qn, lane);
+      __syncthreads();
+      if (on) quad_store(Xt + ltile(i, j), acc2, qm, qn, lane, -1.0, 0.0);
       __syncthreads();
     }
-    a[ty][tx] = diaginv[((int64_t)i * TS + ty) * TS + tx];
-    b[ty][tx] = s;
-    __syncthreads();
-    double o = 0.0;
-#pragma unroll 8
-    for (int m = 0; m < TS; ++m) o = fma(a[ty][m], b[m][tx], o);
-    linv[((int64_t)i * TS + ty) * npad + (int64_t)j * TS + tx] = -o;
-    __threadfence();
-    __syncthreads();
+  }
+  for (int e = tid; e < PTILES * TS * TS; e += 256) {
+    const int tl = e >> 10, r = (e >> 5) & 31, c = e & 31;
+    const int ti = (tl >= 6) ? 3 : (tl >= 3) ? 2 : (tl >= 1) ? 1 : 0, tj = tl - ti * (ti + 1) / 2;
+    blk[(int64_t)(ti * TS + r) * npad + tj * TS + c] = Lt[tl * TS * PL + r * PL + c];
+    xblk[(int64_t)(ti * TS + r) * npad + tj * TS + c] = Xt[tl * TS * PL + r * PL + c];
   }
 }
 
@@ -341,34 +370,38 @@ static int coarse_factor(vcycle_t vc, cudaStream_t st) {
   const int nb = (int)(np / TS), npan = (int)(np / PANEL);
   CUDA_TRY(cudaMemsetAsync(vc->dense, 0, (size_t)np * np * 8, st));
   CUDA_TRY(cudaMemsetAsync(vc->linv, 0, (size_t)np * np * 8, st));
+  CUDA_TRY(cudaMemsetAsync(vc->linvT, 0, (size_t)np * np * 8, st));   // holds L's panels during the factorisation
   if (np > vc->nc) LAUNCH(dense_pad_kernel, (unsigned)((np - vc->nc + 63) / 64), 64, 0, st, vc->nc, np, vc->dense);
   const int64_t nvals = A->nnzb * A->bs_r * A->bs_c;
   if (nvals)
     LAUNCH(dense_fill_kernel, (unsigned)((nvals + 255) / 256), 256, 0, st, nvals, (int)A->bs_r, vc->coarse_rowidx,
            A->d_colidx, A->d_vals, np, vc->dense);
   const dim3 tb(TS, TS);
-  // ---- A = L L^T, right-looking over 128-wide panels
+  // ---- A = L L^T, right-looking over 128-wide panels: the diagonal block (factor + inverse, one CTA), the panel below
+  // it L21 = A21 X11^T and the trailing update, both GEMMs.  L21 is written OUT of place, into linvT (the GEMM's tiles
+  // would otherwise overwrite what their neighbours still read): from here to the final transpose linvT holds the
+  // off-diagonal panels of L and the strictly lower part of `dense` is free -- the workspace of the inverse below.
   // A banded operator (the lexicographic 27-point coarse grid: half-bandwidth 666 of 6000) keeps its band in L: below
   // the band every tile is zero and is skipped -- rows of a panel, of the trailing update and k-ranges of the inverse
   const int64_t band = std::min(vc->band, np);
-  const int btiles = (int)(band / TS) + PT;   // tile rows below a tile column that can hold nonzeros
+  static bool optin = false;
+  if (!optin) {
+    CUDA_TRY(cudaFuncSetAttribute(potrf_panel_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, PANEL_SMEM));
+    optin = true;
+  }
   for (int J = 0; J < npan; ++J) {
-    for (int s = 0; s < PT; ++s) {        // the panel itself, 32x32 tiles: factor, solve below, update the panel's own columns
-      const int c = J * PT + s, rest = std::min(nb - c - 1, btiles), pc = PT - 1 - s;
-      LAUNCH(potrf_tile_kernel, 1, TS, 0, st, np, c, vc->dense, vc->diaginv, vc->d_status);
-      if (rest > 0) LAUNCH(trsm_tile_kernel, (unsigned)rest, tb, 0, st, np, c, vc->dense, vc->diaginv);
-      if (rest > 0 && pc > 0) LAUNCH(syrk_tile_kernel, dim3(pc, rest), tb, 0, st, np, c, vc->dense);
-    }
-    const int64_t r0 = (int64_t)(J + 1) * PANEL;
+    LAUNCH(potrf_panel_kernel, 1, 256, PANEL_SMEM, st, np, J, vc->dense, vc->linv, vc->d_status);
+    const int64_t r0 = (int64_t)(J + 1) * PANEL, c0 = (int64_t)J * PANEL;
     const int m = (int)std::min(np - r0, band);
-    if (m > 0) {                          // trailing update: one GEMM over the lower tiles, k = the panel
-      const double* Lp = vc->dense + r0 * np + (int64_t)J * PANEL;
+    if (m > 0) {
+      double* Lp = vc->linvT + r0 * np + c0;
+      BSR_TRY(dgemm128(true, m, PANEL, PANEL, 1.0, vc->dense + r0 * np + c0, np, vc->linv + c0 * np + c0, np, 0.0, Lp, np, 1, 0,
+                       0, 0, 0, 0, st));
       BSR_TRY(dgemm128(true, m, m, PANEL, -1.0, Lp, np, Lp, np, 1.0, vc->dense + r0 * np + r0, np, 1, 0, 0, 0, 1, 0, st));
     }
   }
-  // ---- X = L^-1: the diagonal 128-blocks by the tile recurrence, then doubling: for the pair (X11, X22) of two
-  // consecutive inverted blocks of size b, X21 = -X22 (L21 X11); linvT is the workspace for L21 X11
-  LAUNCH(trinv_block_kernel, dim3(PT, npan), tb, 0, st, np, vc->dense, vc->diaginv, vc->linv);
+  // ---- X = L^-1: the diagonal 128-blocks are done; doubling: for the pair (X11, X22) of two consecutive inverted blocks
+  // of size b, X21 = -X22 (L21 X11), with T = L21 X11 in the lower part of `dense`
   for (int64_t b = PANEL; b < np; b *= 2) {
     const int64_t step = 2 * b;
     const int nfull = (int)(np / step);                       // pairs with a full second block
@@ -378,9 +411,9 @@ static int coarse_factor(vcycle_t vc, cudaStream_t st) {
       // L21 is banded: its row i is zero left of column b + i - band and entirely zero for i >= band, so T = L21 X11
       // has `mt` nonzero rows and the second product stops at k = mt
       const int64_t mt = std::min(b2, band);
-      BSR_TRY(dgemm128(false, (int)mt, (int)b, (int)b, 1.0, vc->dense + o21, np, vc->linv + o11, np, 0.0, vc->linvT + o21, np,
+      BSR_TRY(dgemm128(false, (int)mt, (int)b, (int)b, 1.0, vc->linvT + o21, np, vc->linv + o11, np, 0.0, vc->dense + o21, np,
                        batch, sp, sp, sp, 0, 1, st, (int)(b - band), 0));
-      return dgemm128(false, (int)b2, (int)b, (int)b2, -1.0, vc->linv + o22, np, vc->linvT + o21, np, 0.0, vc->linv + o21, np,
+      return dgemm128(false, (int)b2, (int)b, (int)b2, -1.0, vc->linv + o22, np, vc->dense + o21, np, 0.0, vc->linv + o21, np,
                       batch, sp, sp, sp, 0, 2, st, -(1 << 30), (int)mt);
     };
     if (nfull > 0) BSR_TRY(pair(0, b, nfull));
@@ -475,7 +508,7 @@ static int dot(vcycle_t vc, int64_t n, const double* a, const double* b, double*
 static void vc_release(vcycle_t vc) {
   if (!vc) return;
   for (auto& lv : vc->L) { dev_free(lv.Dinv); dev_free(lv.r); dev_free(lv.d); dev_free(lv.b); dev_free(lv.x); }
-  dev_free(vc->dense); dev_free(vc->diaginv); dev_free(vc->linv); dev_free(vc->linvT); dev_free(vc->ytmp);
+  dev_free(vc->dense); dev_free(vc->linv); dev_free(vc->linvT); dev_free(vc->ytmp);
   dev_free(vc->coarse_rowidx); dev_free(vc->d_status); dev_free(vc->pr); dev_free(vc->pz); dev_free(vc->pp); dev_free(vc->pq);
   dev_free(vc->partial); dev_free(vc->scal);
   vc->magic = 0;
@@ -562,7 +595,6 @@ int vcycle_create(vcycle_t* out, int32_t nlevels, const bsr_t* A, const bsr_t* P
   if (rc == BSR_OK) rc = dev_alloc_t(&vc->dense, np2);
   if (rc == BSR_OK) rc = dev_alloc_t(&vc->linv, np2);
   if (rc == BSR_OK) rc = dev_alloc_t(&vc->linvT, np2);
-  if (rc == BSR_OK) rc = dev_alloc_t(&vc->diaginv, (size_t)vc->npad * TS);
   if (rc == BSR_OK) rc = dev_alloc_t(&vc->ytmp, (size_t)vc->npad);
   if (rc == BSR_OK) rc = dev_alloc_t(&vc->d_status, 1);
   const int64_t n0 = vc->L[0].n;
