@@ -173,6 +173,16 @@ static int smooth(vcycle_t vc, int l, const double* b, double* x, bool x_zero, c
 
 // ------------------------------------------------------------------ coarsest level: dense Cholesky + L^-1
 // dense is npad x npad row-major, npad a multiple of TS; rows/cols >= nc carry the identity.
+// zero row i of an npad x npad matrix from `reach` columns left of its diagonal 128-block to the end of that block: the
+// part of the matrix the banded factorisation reads and writes
+__global__ void __launch_bounds__(256)
+band_zero_kernel(int64_t npad, int64_t reach, double* __restrict__ mat) {
+  const int64_t i = blockIdx.x, blk0 = (i / 128) * 128;
+  const int64_t c0 = blk0 > reach ? blk0 - reach : 0, c1 = blk0 + 128;
+  double2* row = reinterpret_cast<double2*>(mat + i * npad);
+  for (int64_t c = c0 / 2 + threadIdx.x; c < c1 / 2; c += blockDim.x) row[c] = make_double2(0.0, 0.0);
+}
+
 __global__ void dense_pad_kernel(int64_t nc, int64_t npad, double* __restrict__ dense) {
   const int64_t i = nc + (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (i < npad) dense[i * npad + i] = 1.0;
@@ -368,9 +378,13 @@ static int coarse_factor(vcycle_t vc, cudaStream_t st) {
   bsr_t A = vc->L[vc->nlevels - 1].A;
   const int64_t np = vc->npad;            // a multiple of PANEL
   const int nb = (int)(np / TS), npan = (int)(np / PANEL);
-  CUDA_TRY(cudaMemsetAsync(vc->dense, 0, (size_t)np * np * 8, st));
-  CUDA_TRY(cudaMemsetAsync(vc->linv, 0, (size_t)np * np * 8, st));
-  CUDA_TRY(cudaMemsetAsync(vc->linvT, 0, (size_t)np * np * 8, st));   // holds L's panels during the factorisation
+  // what the banded factorisation touches is cleared, nothing else: in `dense` the band below and the 128-block on the
+  // diagonal (fill-in and the inverse's workspace of the last refresh); in linvT, which holds L's panels until the final
+  // transpose, the band plus the two tile rows by which the k-ranges of the inverse overshoot it.  linv is written in
+  // its lower part only and was cleared once, at creation.
+  const int64_t band0 = std::min(vc->band, np);
+  LAUNCH(band_zero_kernel, (unsigned)np, 256, 0, st, np, band0, vc->dense);
+  LAUNCH(band_zero_kernel, (unsigned)np, 256, 0, st, np, band0 + 256, vc->linvT);
   if (np > vc->nc) LAUNCH(dense_pad_kernel, (unsigned)((np - vc->nc + 63) / 64), 64, 0, st, vc->nc, np, vc->dense);
   const int64_t nvals = A->nnzb * A->bs_r * A->bs_c;
   if (nvals)
@@ -595,6 +609,8 @@ int vcycle_create(vcycle_t* out, int32_t nlevels, const bsr_t* A, const bsr_t* P
   if (rc == BSR_OK) rc = dev_alloc_t(&vc->dense, np2);
   if (rc == BSR_OK) rc = dev_alloc_t(&vc->linv, np2);
   if (rc == BSR_OK) rc = dev_alloc_t(&vc->linvT, np2);
+  if (rc == BSR_OK && cudaMemsetAsync(vc->linv, 0, np2 * 8, st) != cudaSuccess) rc = fail(BSR_ERR_CUDA, "memset failed");
+  if (rc == BSR_OK && cudaMemsetAsync(vc->dense, 0, np2 * 8, st) != cudaSuccess) rc = fail(BSR_ERR_CUDA, "memset failed");
   if (rc == BSR_OK) rc = dev_alloc_t(&vc->ytmp, (size_t)vc->npad);
   if (rc == BSR_OK) rc = dev_alloc_t(&vc->d_status, 1);
   const int64_t n0 = vc->L[0].n;
