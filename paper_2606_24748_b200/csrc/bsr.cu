@@ -130,6 +130,15 @@ spmv_kernel(int32_t nbrows, const int32_t* __restrict__ rowptr, const int32_t* _
   const int64_t row = row_first + ri;
   const bool live = glive && (row < nbrows);
   const int32_t k0 = __shfl_sync(0xffffffffu, rp_lane, ri), k1 = __shfl_sync(0xffffffffu, rp_lane, ri + 1);
+  // the lane that will write y[row * BR + r].  What its epilogue reads (b or the old y) is requested from DRAM BEFORE
+  // the row's blocks, as an L2 prefetch, and loaded after them, ahead of the reduction's shuffles.  Measured on the 96^3
+  // operator (plain y = A x: 0.340 ms): load after the reduction 0.398 / 0.403 (RESID / SUB); this 0.376 / 0.377; the
+  // operand held in a register across the loop 0.379 / 0.425 (two of the 40 registers the batched loads live on);
+  // that with 5 resident CTAs instead of 6 0.401 / 0.420.
+  const int r = (S::PAIR && !S::ROWPAIR) ? q : q / S::LPR;
+  const bool writer = live && member == 0 && ((S::PAIR && !S::ROWPAIR) ? (q < BR) : (q % S::LPR) == 0);
+  if (EPI != EPI_ASSIGN && writer)
+    asm volatile("prefetch.global.L2 [%0];" ::"l"((EPI == EPI_RESID ? b : y) + row * BR + r));
   double accA = 0.0, accB = 0.0;
   if (live) {
     for (int32_t k = k0 + member; k < k1; k += TEAM * U) {
@@ -179,6 +188,9 @@ spmv_kernel(int32_t nbrows, const int32_t* __restrict__ rowptr, const int32_t* _
       }
     }
   }
+  // the epilogue's operand: an L2 hit by now, issued ahead of the reduction's shuffles
+  double prev = 0.0;
+  if (EPI != EPI_ASSIGN && writer) prev = (EPI == EPI_RESID) ? __ldg(b + row * BR + r) : y[row * BR + r];
   // 1) the TEAM groups of a row (lanes LB apart), fixed order
 #pragma unroll
   for (int s = 1; s < TEAM; s <<= 1) {
@@ -188,8 +200,6 @@ spmv_kernel(int32_t nbrows, const int32_t* __restrict__ rowptr, const int32_t* _
   }
   // 2) the lanes of one block row
   double out;
-  bool writer;
-  int r;
   if (S::PAIR && !S::ROWPAIR) {
     // lane t < BR of the group gathers elements t*BC .. t*BC+BC-1: element e sits in lane e/2, slot e%2
     out = 0.0;
@@ -201,8 +211,6 @@ spmv_kernel(int32_t nbrows, const int32_t* __restrict__ rowptr, const int32_t* _
       const double bb = __shfl_sync(0xffffffffu, accB, (base + e / 2) & 31);
       out += (e & 1) ? bb : a;
     }
-    r = q;
-    writer = q < BR;
   } else {
     out = accA;
     if (S::LPR == 3) {
@@ -212,15 +220,12 @@ spmv_kernel(int32_t nbrows, const int32_t* __restrict__ rowptr, const int32_t* _
     } else if (S::LPR == 2) {
       out += __shfl_down_sync(0xffffffffu, out, 1);
     }
-    r = q / S::LPR;
-    writer = (q % S::LPR) == 0;
   }
-  if (live && writer && member == 0) {
+  if (writer) {
     const int64_t o = row * BR + r;
     if (EPI == EPI_ASSIGN) y[o] = out;
-    else if (EPI == EPI_RESID) y[o] = b[o] - out;
-    else if (EPI == EPI_SUB) y[o] = y[o] - out;
-    else y[o] = y[o] + out;
+    else if (EPI == EPI_ADD) y[o] = prev + out;
+    else y[o] = prev - out;
   }
   }  // batch of row groups
 }
@@ -284,6 +289,14 @@ spmv_flat_kernel(int32_t nbrows, const int32_t* __restrict__ rowptr, const int32
   if (tid <= r1 - r0) rp[tid] = __ldg(rowptr + r0 + tid);
   const int32_t k0 = __ldg(rowptr + r0), k1 = __ldg(rowptr + r1);
   const int32_t T = (k1 - k0) * LB;                                    // 16-byte pairs of the CTA's run
+  constexpr int NOUT = (FLAT_ROWS * BR + FLAT_THREADS - 1) / FLAT_THREADS;   // output entries per thread
+  if (EPI != EPI_ASSIGN) {                                             // what the epilogue reads: on its way to L2
+#pragma unroll
+    for (int w = 0; w < NOUT; ++w) {
+      const int o = tid + w * FLAT_THREADS;
+      if (o < (r1 - r0) * BR) asm volatile("prefetch.global.L2 [%0];" ::"l"((EPI == EPI_RESID ? b : y) + (int64_t)r0 * BR + o));
+    }
+  }
   const double2* v2 = reinterpret_cast<const double2*>(vals) + (int64_t)k0 * LB;
   for (int32_t c = tid; c < T; c += FLAT_THREADS * FLAT_U) {
     int32_t cu[FLAT_U], col[FLAT_U];
@@ -303,7 +316,10 @@ spmv_flat_kernel(int32_t nbrows, const int32_t* __restrict__ rowptr, const int32
       if (c + u * FLAT_THREADS < T) part[cu[u]] = fma(v[u].y, xv[u].y, v[u].x * xv[u].x);
   }
   __syncthreads();
-  for (int o = tid; o < (r1 - r0) * BR; o += FLAT_THREADS) {
+#pragma unroll
+  for (int w = 0; w < NOUT; ++w) {
+    const int o = tid + w * FLAT_THREADS;
+    if (o >= (r1 - r0) * BR) break;
     const int rl = o / BR, r = o - rl * BR;
     const int32_t ks = rp[rl] - k0, ke = rp[rl + 1] - k0;
     double sum = 0.0;
@@ -311,9 +327,9 @@ spmv_flat_kernel(int32_t nbrows, const int32_t* __restrict__ rowptr, const int32
 #pragma unroll
       for (int cv = 0; cv < LPR; ++cv) sum += part[kk * LB + r * LPR + cv];
     }
-    const int64_t oi = (int64_t)(r0 + rl) * BR + r;
+    const int64_t oi = (int64_t)r0 * BR + o;
     if (EPI == EPI_ASSIGN) y[oi] = sum;
-    else if (EPI == EPI_RESID) y[oi] = b[oi] - sum;
+    else if (EPI == EPI_RESID) y[oi] = __ldg(b + oi) - sum;
     else if (EPI == EPI_SUB) y[oi] = y[oi] - sum;
     else y[oi] = y[oi] + sum;
   }
