@@ -472,7 +472,7 @@ def run_ours(args) -> dict | None:
                 "frac": ach / peak, "traffic": traffic, "algorithmic_bytes_per_launch": kb[dom],
                 "ms_per_launch": per[dom], "share_of_step": per[dom] / sum(per.values()),
                 "alu": dict(alu.get(dom, {}), unit="TFLOP/s", peak_source="bsr_measure_fp64_peak (this run)",
-                            all_kernels=alu),
+                            mma_peak=bsr.fp64_peak_tflops(mma=True), all_kernels=alu),
                 "all_kernels": {n: {"ms": per[n], "ms_min": per_min[n], "GB/s": kb[n] / (per[n] * 1e-3) / 1e9,
                                     "frac": kb[n] / (per[n] * 1e-3) / 1e9 / peak, "traffic": traffic_all.get(n)}
                                 for n in names}}

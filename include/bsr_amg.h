@@ -274,6 +274,9 @@ int bsr_counters(int64_t* n_kernel_launches, int64_t* n_allocs);
 /* Measured fp64 FMA peak of the current device in TFLOP/s (register-resident FMA chains, CUDA events, best of 5):
  * the ALU roof reported beside the HBM roof of the PtAP kernels.  COLD: allocates, synchronises. */
 int bsr_measure_fp64_peak(double* tflops, void* stream);
+/* The same for the fp64 tensor-core path (chains of mma.sync.aligned.m8n8k4.f64, 512 flops each): the roof of the dense
+ * GEMM inside vcycle_refresh.  COLD: allocates, synchronises. */
+int bsr_measure_fp64_mma_peak(double* tflops, void* stream);
 
 /* ------------------------------------------------------------------ workspace allocator (ownership)
  * Library-private workspace (the cached transpose, AP, plans, D^-1, work vectors, the dense factor) is obtained in COLD

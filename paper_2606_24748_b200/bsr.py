@@ -58,6 +58,7 @@ SYMBOLS = {
     "bsr_set_allocator": (C.c_int, [_V, _V, _V]),
     "bsr_counters": (C.c_int, [_PI64, _PI64]),
     "bsr_measure_fp64_peak": (C.c_int, [C.POINTER(_D), _V]),
+    "bsr_measure_fp64_mma_peak": (C.c_int, [C.POINTER(_D), _V]),
     "prolongator_smooth_symbolic": (C.c_int, [_PV, _V, _V, _PI64, _V]),
     "prolongator_smooth_structure": (C.c_int, [_V, _V, _V, _V]),
     "prolongator_smooth_numeric": (C.c_int, [_V, _V, _V, _D, _V, _V]),
@@ -181,10 +182,12 @@ def counters():
     return a.value, b.value
 
 
-def fp64_peak_tflops() -> float:
-    """Measured fp64 FMA peak of the current device (bsr_measure_fp64_peak)."""
+def fp64_peak_tflops(mma: bool = False) -> float:
+    """Measured fp64 peak of the current device: FMA chains (bsr_measure_fp64_peak) or, mma=True, chains of
+    mma.sync m8n8k4 on the fp64 tensor-core path (bsr_measure_fp64_mma_peak)."""
     t = C.c_double()
-    _check(lib().bsr_measure_fp64_peak(C.byref(t), _stream()))
+    fn = lib().bsr_measure_fp64_mma_peak if mma else lib().bsr_measure_fp64_peak
+    _check(fn(C.byref(t), _stream()))
     return t.value
 
 

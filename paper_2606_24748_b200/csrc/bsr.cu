@@ -245,13 +245,8 @@ static int spmv_dispatch_epi(bsr_t A, const double* x, double* y, const double* 
              A->d_vals, x, y, b);
       break;
     case EPI_RESID:
-      LAUNCH((spmv_kernel<BR, BC, TEAM, U, EPI_RESID, MINB, RB>), grid, block, 0, st, A->nbrows, A->d_rowptr, A->d_colidx,
-             A->d_vals, x, y, b);
-      break;
     case EPI_SUB:
-      LAUNCH((spmv_kernel<BR, BC, TEAM, U, EPI_SUB, MINB, RB>), grid, block, 0, st, A->nbrows, A->d_rowptr, A->d_colidx,
-             A->d_vals, x, y, b);
-      break;
+      return fail(BSR_ERR_SHAPE, "spmv: the subtracting epilogues were retired (vcycle.cu forms r = b - t itself)");
     default:
       LAUNCH((spmv_kernel<BR, BC, TEAM, U, EPI_ADD, MINB, RB>), grid, block, 0, st, A->nbrows, A->d_rowptr, A->d_colidx,
              A->d_vals, x, y, b);
@@ -358,13 +353,14 @@ static int spmv_flat_launch(bsr_t A, const double* x, double* y, const double* b
     }                                                                                                         \
   }
   if (prepare) {
-    FLAT_CASE(EPI_ASSIGN) FLAT_CASE(EPI_RESID) FLAT_CASE(EPI_SUB) FLAT_CASE(EPI_ADD)
+    FLAT_CASE(EPI_ASSIGN) FLAT_CASE(EPI_ADD)
     return BSR_OK;
   }
   switch (epi) {
     case EPI_ASSIGN: FLAT_CASE(EPI_ASSIGN) break;
-    case EPI_RESID: FLAT_CASE(EPI_RESID) break;
-    case EPI_SUB: FLAT_CASE(EPI_SUB) break;
+    case EPI_RESID:
+    case EPI_SUB:
+      return fail(BSR_ERR_SHAPE, "spmv: the subtracting epilogues were retired (vcycle.cu forms r = b - t itself)");
     default: FLAT_CASE(EPI_ADD) break;
   }
 #undef FLAT_CASE

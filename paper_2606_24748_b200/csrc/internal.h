@@ -66,11 +66,12 @@ inline bool shape_supported(int br, int bc) {
          (br == 3 && bc == 6) || (br == 6 && bc == 3) || (br == 6 && bc == 6);
 }
 
-// epilogues of the SpMV kernels (the V-cycle glue fused into the product)
-enum Epilogue { EPI_ASSIGN = 0, /* y = A x */ EPI_RESID = 1, /* y = b - A x */ EPI_SUB = 2, /* y -= A x */
-                EPI_ADD = 3 /* y += A x */ };
+// epilogues of the SpMV kernels (the V-cycle glue fused into the product).  EPI_RESID / EPI_SUB
+// (y = b - A x, y -= A x) are still understood by the kernels but no longer launched: at 10 % over the plain product
+// they lost to subtracting inside the Chebyshev update (vcycle.cu); spmv_launch refuses them.
+enum Epilogue { EPI_ASSIGN = 0, /* y = A x */ EPI_RESID = 1, EPI_SUB = 2, EPI_ADD = 3 /* y += A x */ };
 
-// internal SpMV with epilogue; b only for EPI_RESID
+// internal SpMV with epilogue (b: unused by the launched epilogues)
 int spmv_launch(bsr_t A, const double* d_x, double* d_y, const double* d_b, Epilogue epi, cudaStream_t st);
 // dinv[i] = inverse of A's bs x bs diagonal block of row i (point-block Jacobi data); *status |= 1 on a
 // missing or singular block

@@ -349,3 +349,12 @@ def test_ptap_host_buffer_path_is_chunked_and_exact(bsr, probs):
             assert torch.equal(vals_c, ref), (name, k)
             assert np.array_equal(hc.numpy(), ref.cpu().numpy()), (name, k)
             assert np.array_equal(GA.vals.cpu().numpy(), ha.numpy())        # the device copy of A holds the new values
+
+
+def test_fp64_peak_probes(bsr):
+    """The two ALU roofs bench.py reports: FMA chains and mma.sync m8n8k4 chains.  On B200 both land near 37 TFLOP/s;
+    the test only pins that they are positive, of the same order, and below what 148 SMs x 128 FMA/clk x 2.5 GHz allow."""
+    fma = bsr.fp64_peak_tflops()
+    mma = bsr.fp64_peak_tflops(mma=True)
+    assert 1.0 < fma < 100.0 and 1.0 < mma < 100.0
+    assert 0.5 < mma / fma < 2.0

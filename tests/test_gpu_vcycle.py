@@ -146,3 +146,67 @@ def test_vcycle_errors(bsr):
     b = pr.uniform(0, pr.PURPOSE_RHS, A.nbrows * 3)
     x = one.apply(dev(b)).cpu().numpy()
     assert relerr(orc.spmv(A, x), b) < 1e-9
+
+
+@pytest.mark.parametrize("degree", [1, 3, 4])
+def test_chebyshev_degrees(bsr, degree):
+    """Degrees other than the default 2: degree 1 never forms a second residual, degrees >= 3 store r for the next
+    step (from the zero guess only from step 1 on) and update it in place from step 2 on."""
+    g = pr.make_generator(0)
+    g.build_prolongator(0)
+    A, P = g.A(0), g.P(0)
+    Ac = as_host(orc.ptap(A, P))
+    lam = g.level_info(0)["lam"]
+    H = orc.Hierarchy([A, Ac], [P], [lam], cheb_degree=degree)
+    vc = bsr.VCycle([bsr.Bsr.from_host(A), bsr.Bsr.from_host(Ac)], [bsr.Bsr.from_host(P)], [lam], cheb_degree=degree)
+    n = A.nbrows * 3
+    b = pr.uniform(0, pr.PURPOSE_RHS, n)
+    x0 = pr.uniform(0, pr.PURPOSE_FINE, n)
+    assert relerr(vc.smooth(0, dev(b), dev(x0)).cpu().numpy(), H.smooth(0, b, x0)) < 1e-12
+    assert relerr(vc.smooth(0, dev(b), dev(np.zeros(n))).cpu().numpy(), H.smooth(0, b, np.zeros(n))) < 1e-12
+    assert relerr(vc.apply(dev(b)).cpu().numpy(), H.vcycle(b)) < 1e-10
+
+
+def _dense(M):
+    D = np.zeros((M.nbrows * M.bs_r, M.nbcols * M.bs_c))
+    for i in range(M.nbrows):
+        for k in range(M.rowptr[i], M.rowptr[i + 1]):
+            j = M.colidx[k]
+            D[i * M.bs_r:(i + 1) * M.bs_r, j * M.bs_c:(j + 1) * M.bs_c] = M.vals[k].reshape(M.bs_r, M.bs_c)
+    return D
+
+
+@pytest.mark.parametrize("case", ["tiny", "one_panel_and_a_bit", "banded", "not_banded"])
+def test_coarsest_direct_solve(bsr, case):
+    """The dense coarsest solve alone (a single level): x = L^-T (L^-1 b) against numpy's solve of the assembled matrix.
+    Sizes below one 128-panel, just above one, several panels with a band, and the same operator under a random
+    symmetric permutation of its block rows (no band: nothing is skipped)."""
+    import scipy.sparse as sp
+    if case == "tiny":
+        g = pr.Generator(3, 2, seed=7)            # 27 nodes, 81 unknowns: one padded panel
+        M = g.A(0)
+    elif case == "one_panel_and_a_bit":
+        g = pr.make_generator(0)
+        g.build_prolongator(0)
+        M = as_host(orc.ptap(g.A(0), g.P(0)))     # 27 aggregates x 6 = 162 unknowns, 6x6 blocks
+    else:
+        g = pr.Generator(3, 6, seed=7)            # 343 nodes, 1029 unknowns: 9 panels, half-bandwidth 57 nodes
+        M = g.A(0)
+        if case == "not_banded":
+            S = sp.bsr_matrix((M.vals.reshape(-1, 3, 3), M.colidx, M.rowptr), shape=(M.nbrows * 3, M.nbrows * 3)).tocsr()
+            perm = np.random.default_rng(3).permutation(M.nbrows)
+            idx = (perm[:, None] * 3 + np.arange(3)[None, :]).ravel()
+            S = S[idx][:, idx].tobsr(blocksize=(3, 3))
+            S.sort_indices()
+            M = pr.HostBSR(M.nbrows, M.nbrows, 3, 3, S.indptr.astype(np.int32), S.indices.astype(np.int32),
+                           np.ascontiguousarray(S.data))
+    D = _dense(M)
+    assert np.allclose(D, D.T, rtol=1e-12, atol=1e-12 * np.abs(D).max())
+    n = D.shape[0]
+    b = pr.uniform(1, pr.PURPOSE_RHS, n)
+    one = bsr.VCycle([bsr.Bsr.from_host(M)], [], [])
+    x = one.apply(dev(b)).cpu().numpy()
+    assert relerr(D @ x, b) < 1e-9
+    assert relerr(x, np.linalg.solve(D, b)) < 1e-7
+    one.refresh()                                  # a second factorisation into the same buffers
+    assert np.array_equal(one.apply(dev(b)).cpu().numpy(), x)
