@@ -24,6 +24,8 @@ struct bcoo_plan_s {
   int64_t n = 0, nnzb = 0;
   int32_t nbrows = 0, nbcols = 0, bs_r = 0, bs_c = 0;
   int32_t *rowptr = nullptr, *colidx = nullptr, *segptr = nullptr, *perm = nullptr;
+  int32_t* ctas = nullptr;   // staged kernel: per run {first block, blocks, first contribution, contributions}
+  int64_t nctas = 0;         // runs; 0: a block with more contributions than a buffer holds -> the per-value kernel
 };
 static const uint64_t BCOO_MAGIC = 0x42434f4f504c414eull;
 
@@ -53,6 +55,60 @@ bcoo_sum_kernel(int64_t nvals, const int32_t* __restrict__ segptr, const int32_t
     for (int u = 0; u < 4; ++u) s += (p + u < p1) ? v[u] : 0.0;
   }
   vals[t] = s;
+}
+
+// The same sums, a CTA at a time.  The per-value kernel above walks segment pointer -> stream position -> value once
+// per thread, and of the three dependent latencies only the last moves bytes.  Here the plan cuts the destination
+// blocks into runs whose contributions fill a CTA's shared memory (BCOO_ITEMS doubles, at most BCOO_NBMAX blocks); the
+// CTA fetches the run's segment pointers and stream positions with two coalesced loads, every thread then has up to 16
+// independent value loads to issue (two rounds of 8), parked in shared memory in contribution order, and one thread
+// per destination value adds its segment in declaration order (the order of the kernel above and of the oracle:
+// bit-identical) and stores coalesced.  4.47 -> 4.04 ms at config 3 (0.55 of the HBM peak).  A persistent variant
+// (two 32 KB buffers per CTA, values by LDGSTS, the next run's indices fetched in their shadow) measured 4.33 ms and
+// was not kept: the index latencies are not what binds this gather -- its reads are 72-byte pieces of the element
+// stream, every 4.6 KB element record visited at four different times.
+constexpr int BCOO_ITEMS = 8192;    // doubles of contributions a CTA parks (64 KB: three CTAs per SM)
+constexpr int BCOO_NBMAX = 512;     // destination blocks per run
+constexpr int BCOO_THREADS = 512;
+constexpr size_t BCOO_FLAT_SMEM = (size_t)BCOO_ITEMS * 8 + (size_t)(BCOO_NBMAX + 4) * 4 + (size_t)(BCOO_ITEMS / 4) * 4;
+
+template <int BB>
+__global__ void __launch_bounds__(BCOO_THREADS)
+bcoo_flat_kernel(const int4* __restrict__ runs, const int32_t* __restrict__ segptr, const int32_t* __restrict__ perm,
+                 const double* __restrict__ stream, double* __restrict__ vals) {
+  extern __shared__ __align__(16) unsigned char bcoo_smem[];
+  double* part = reinterpret_cast<double*>(bcoo_smem);
+  int32_t* seg = reinterpret_cast<int32_t*>(bcoo_smem + (size_t)BCOO_ITEMS * 8);
+  int32_t* pos = seg + BCOO_NBMAX + 4;
+  const int tid = threadIdx.x;
+  const int4 c = __ldg(runs + blockIdx.x);                   // {first block, blocks, first contribution, contributions}
+  const int b0 = c.x, nb = c.y, k0 = c.z, nk = c.w;
+  for (int i = tid; i <= nb; i += BCOO_THREADS) seg[i] = __ldg(segptr + b0 + i) - k0;
+  for (int i = tid; i < nk; i += BCOO_THREADS) pos[i] = __ldg(perm + k0 + i);
+  __syncthreads();
+  const int items = nk * BB;
+  for (int base = tid; base < items; base += BCOO_THREADS * 8) {
+    double v[8];
+#pragma unroll
+    for (int u = 0; u < 8; ++u) {
+      const int it = base + u * BCOO_THREADS;
+      const int k = it / BB, e = it - k * BB;
+      v[u] = 0.0;
+      if (it < items) v[u] = __ldg(stream + (int64_t)pos[k] * BB + e);
+    }
+#pragma unroll
+    for (int u = 0; u < 8; ++u) {
+      const int it = base + u * BCOO_THREADS;
+      if (it < items) part[it] = v[u];
+    }
+  }
+  __syncthreads();
+  for (int o = tid; o < nb * BB; o += BCOO_THREADS) {
+    const int bl = o / BB, e = o - bl * BB;
+    double s = 0.0;
+    for (int k = seg[bl]; k < seg[bl + 1]; ++k) s += part[k * BB + e];
+    vals[(int64_t)b0 * BB + o] = s;
+  }
 }
 
 // dst block t = src block idx[t] (bs doubles each): packs halo entries / prolongator rows for an exchange
@@ -150,7 +206,7 @@ q1_blocks_kernel(int ne, int64_t e0, int64_t ncontrib, const double* __restrict_
 
 static void bcoo_release(bcoo_plan_s* pl) {
   if (!pl) return;
-  dev_free(pl->rowptr); dev_free(pl->colidx); dev_free(pl->segptr); dev_free(pl->perm);
+  dev_free(pl->rowptr); dev_free(pl->colidx); dev_free(pl->segptr); dev_free(pl->perm); dev_free(pl->ctas);
   pl->magic = 0;
   delete pl;
 }
@@ -222,13 +278,30 @@ int bcoo_plan_create(bcoo_plan_t* out, int64_t n, const int32_t* d_brow, const i
         ++s;
       }
   }
+  // runs of destination blocks for the staged kernel: as many as fill one of its shared-memory buffers
+  std::vector<int32_t> ctas;
+  {
+    const int32_t cap = BCOO_ITEMS / (bs_r * bs_c);
+    bool fits = true;
+    for (int64_t b0 = 0; b0 < nnzb && fits;) {
+      int64_t b1 = b0;
+      while (b1 < nnzb && b1 - b0 < BCOO_NBMAX && segptr[(size_t)b1 + 1] - segptr[(size_t)b0] <= cap) ++b1;
+      if (b1 == b0) { fits = false; break; }   // one block with more contributions than a buffer parks
+      ctas.push_back((int32_t)b0); ctas.push_back((int32_t)(b1 - b0));
+      ctas.push_back(segptr[(size_t)b0]); ctas.push_back(segptr[(size_t)b1] - segptr[(size_t)b0]);
+      b0 = b1;
+    }
+    if (!fits) ctas.clear();
+  }
   bcoo_plan_s* pl = new (std::nothrow) bcoo_plan_s();
   if (!pl) return fail(BSR_ERR_ALLOC, "host allocation failed");
   pl->n = n; pl->nnzb = nnzb; pl->nbrows = nbrows; pl->nbcols = nbcols; pl->bs_r = bs_r; pl->bs_c = bs_c;
+  pl->nctas = (int64_t)ctas.size() / 4;
   int rc = upload(&pl->rowptr, rowptr, st);
   if (rc == BSR_OK) rc = upload(&pl->colidx, colidx, st);
   if (rc == BSR_OK) rc = upload(&pl->segptr, segptr, st);
   if (rc == BSR_OK) rc = upload(&pl->perm, byrow, st);
+  if (rc == BSR_OK && pl->nctas) rc = upload(&pl->ctas, ctas, st);
   if (rc == BSR_OK && cudaStreamSynchronize(st) != cudaSuccess) rc = fail(BSR_ERR_CUDA, "plan upload failed");
   if (rc != BSR_OK) { bcoo_release(pl); return rc; }
   pl->magic = BCOO_MAGIC;
@@ -254,6 +327,24 @@ int bcoo_set_values(bcoo_plan_t pl, const double* d_stream, double* d_vals, void
   NvtxRange nv("bcoo_set_values");
   const int bb = pl->bs_r * pl->bs_c;
   const int64_t nvals = pl->nnzb * bb;
+  if (pl->nctas) {
+    const int4* runs = reinterpret_cast<const int4*>(pl->ctas);
+#define BCOO_FLAT(BB)                                                                                                 \
+  case BB: {                                                                                                          \
+    static bool optin = false;                                                                                        \
+    if (!optin) {                                                                                                     \
+      CUDA_TRY(cudaFuncSetAttribute(bcoo_flat_kernel<BB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)BCOO_FLAT_SMEM)); \
+      optin = true;                                                                                                   \
+    }                                                                                                                 \
+    LAUNCH(bcoo_flat_kernel<BB>, (unsigned)pl->nctas, BCOO_THREADS, BCOO_FLAT_SMEM, st, runs, pl->segptr, pl->perm, d_stream, d_vals); \
+    return BSR_OK;                                                                                                    \
+  }
+    switch (bb) {
+      BCOO_FLAT(4) BCOO_FLAT(6) BCOO_FLAT(9) BCOO_FLAT(18) BCOO_FLAT(36)
+      default: return fail(BSR_ERR_BLOCK, "unsupported block shape");
+    }
+#undef BCOO_FLAT
+  }
   const unsigned grid = (unsigned)((nvals + 255) / 256);
   switch (bb) {
     case 4: LAUNCH(bcoo_sum_kernel<4>, grid, 256, 0, st, nvals, pl->segptr, pl->perm, d_stream, d_vals); break;

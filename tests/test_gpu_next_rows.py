@@ -253,6 +253,24 @@ def test_bcoo_edge_cases(bsr):
     assert np.array_equal(one.set_values(dev(s.reshape(-1))).cpu().numpy().reshape(2, 3), s.sum(axis=0))
 
 
+def test_bcoo_block_larger_than_a_cta(bsr):
+    """One destination block with more contributions than a CTA of the staged kernel parks (8192 doubles): the plan falls
+    back to the per-value kernel for the whole matrix; same sums in the same order."""
+    rng = np.random.default_rng(5)
+    n_big = 3000
+    brow = np.concatenate([np.full(n_big, 4), rng.integers(0, 9, 400)]).astype(np.int32)
+    bcol = np.concatenate([np.full(n_big, 2), rng.integers(0, 9, 400)]).astype(np.int32)
+    order = rng.permutation(brow.shape[0])
+    brow, bcol = brow[order], bcol[order]
+    stream = rng.uniform(-1, 1, (brow.shape[0], 3, 3))
+    ref = orc.bcoo_assemble(brow, bcol, stream, 9, 9)
+    plan = bsr.BcooPlan(dev(brow), dev(bcol), 9, 9, 3, 3)
+    assert np.array_equal(plan.rowptr.cpu().numpy(), ref.rowptr) and np.array_equal(plan.colidx.cpu().numpy(), ref.colidx)
+    vals = plan.set_values(dev(stream.reshape(-1))).cpu().numpy().reshape(ref.vals.shape)
+    mag = orc.bcoo_assemble(brow, bcol, np.abs(stream), 9, 9, structure=(ref.rowptr, ref.colidx)).vals
+    assert blockwise_rel_err(vals, ref.vals, mag) < TOL
+
+
 def fem_device_assembly(bsr, g, chunk=None):
     """Config's operator assembled on the device: coordinates and E_e * Ke blocks emitted by the library's Q1 driver,
     summed through the blocked COO plan."""
