@@ -19,7 +19,8 @@ from collections import OrderedDict
 BENCH_NAMES = [
     ("spmv_flat_kernel<3, 6", "spmv_P"), ("spmv_kernel<3, 3", "spmv_A"), ("spmv_kernel<6, 3", "spmv_Pt"),
     ("stream_product_kernel<3, 3, 6, 256, 0, 0", "ptap_stage1_AP"), ("stream_product_kernel<6, 3, 6", "ptap_stage2_RAP"),
-    ("stream_product_kernel<3, 3, 6, 256, 0, 1", "prolongator_smooth"), ("bcoo_sum_kernel<9", "bcoo_set_values"),
+    ("stream_product_kernel<3, 3, 6, 256, 0, 1", "prolongator_smooth"), ("bcoo_flat_kernel<9", "bcoo_set_values"),
+    ("bcoo_sum_kernel<9", "bcoo_set_values_per_value"),
     ("spmv_kernel<6, 6", "spmv_6x6"), ("cheb_update_kernel", "cheb_update"), ("trigemv_kernel", "trigemv"),
 ]
 METRICS = OrderedDict([
