@@ -293,6 +293,18 @@ int bcoo_plan_create(bcoo_plan_t* out, int64_t n, const int32_t* d_brow, const i
     }
     if (!fits) ctas.clear();
   }
+  if (!ctas.empty()) {   // cold: the staged kernel's shared memory, on the device the plan lives on
+    cudaError_t e = cudaSuccess;
+    switch (bs_r * bs_c) {
+      case 4: e = cudaFuncSetAttribute(bcoo_flat_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)BCOO_FLAT_SMEM); break;
+      case 6: e = cudaFuncSetAttribute(bcoo_flat_kernel<6>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)BCOO_FLAT_SMEM); break;
+      case 9: e = cudaFuncSetAttribute(bcoo_flat_kernel<9>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)BCOO_FLAT_SMEM); break;
+      case 18: e = cudaFuncSetAttribute(bcoo_flat_kernel<18>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)BCOO_FLAT_SMEM); break;
+      case 36: e = cudaFuncSetAttribute(bcoo_flat_kernel<36>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)BCOO_FLAT_SMEM); break;
+      default: break;
+    }
+    if (e != cudaSuccess) return fail(BSR_ERR_CUDA, "bcoo_flat_kernel: cannot opt in to shared memory: %s", cudaGetErrorString(e));
+  }
   bcoo_plan_s* pl = new (std::nothrow) bcoo_plan_s();
   if (!pl) return fail(BSR_ERR_ALLOC, "host allocation failed");
   pl->n = n; pl->nnzb = nnzb; pl->nbrows = nbrows; pl->nbcols = nbcols; pl->bs_r = bs_r; pl->bs_c = bs_c;
@@ -331,11 +343,6 @@ int bcoo_set_values(bcoo_plan_t pl, const double* d_stream, double* d_vals, void
     const int4* runs = reinterpret_cast<const int4*>(pl->ctas);
 #define BCOO_FLAT(BB)                                                                                                 \
   case BB: {                                                                                                          \
-    static bool optin = false;                                                                                        \
-    if (!optin) {                                                                                                     \
-      CUDA_TRY(cudaFuncSetAttribute(bcoo_flat_kernel<BB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)BCOO_FLAT_SMEM)); \
-      optin = true;                                                                                                   \
-    }                                                                                                                 \
     LAUNCH(bcoo_flat_kernel<BB>, (unsigned)pl->nctas, BCOO_THREADS, BCOO_FLAT_SMEM, st, runs, pl->segptr, pl->perm, d_stream, d_vals); \
     return BSR_OK;                                                                                                    \
   }

@@ -426,11 +426,6 @@ static int coarse_factor(vcycle_t vc, cudaStream_t st) {
   // A banded operator (the lexicographic 27-point coarse grid: half-bandwidth 666 of 6000) keeps its band in L: below
   // the band every tile is zero and is skipped -- rows of a panel, of the trailing update and k-ranges of the inverse
   const int64_t band = std::min(vc->band, np);
-  static bool optin = false;
-  if (!optin) {
-    CUDA_TRY(cudaFuncSetAttribute(potrf_panel_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, PANEL_SMEM));
-    optin = true;
-  }
   for (int J = 0; J < npan; ++J) {
     LAUNCH(potrf_panel_kernel, 1, 256, PANEL_SMEM, st, np, J, vc->dense, vc->linv, vc->d_status);
     const int64_t r0 = (int64_t)(J + 1) * PANEL, c0 = (int64_t)J * PANEL;
@@ -641,6 +636,9 @@ int vcycle_create(vcycle_t* out, int32_t nlevels, const bsr_t* A, const bsr_t* P
   if (rc == BSR_OK) rc = dev_alloc_t(&vc->dense, np2);
   if (rc == BSR_OK) rc = dev_alloc_t(&vc->linv, np2);
   if (rc == BSR_OK) rc = dev_alloc_t(&vc->linvT, np2);
+  // the panel kernel's 180 KB of dynamic shared memory: opted in here, cold, on the device the hierarchy lives on
+  if (rc == BSR_OK && cudaFuncSetAttribute(potrf_panel_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, PANEL_SMEM) != cudaSuccess)
+    rc = fail(BSR_ERR_CUDA, "potrf_panel_kernel: cannot opt in to %d bytes of shared memory", PANEL_SMEM);
   if (rc == BSR_OK && cudaMemsetAsync(vc->linv, 0, np2 * 8, st) != cudaSuccess) rc = fail(BSR_ERR_CUDA, "memset failed");
   if (rc == BSR_OK && cudaMemsetAsync(vc->dense, 0, np2 * 8, st) != cudaSuccess) rc = fail(BSR_ERR_CUDA, "memset failed");
   if (rc == BSR_OK) rc = dev_alloc_t(&vc->ytmp, (size_t)vc->npad);
