@@ -387,19 +387,55 @@ transpose_tile_kernel(int64_t npad, const double* __restrict__ src, double* __re
   dst[((int64_t)blockIdx.x * TS + ty) * npad + (int64_t)blockIdx.y * TS + tx] = t[tx][ty];
 }
 
-// y[i] = sum_{j in [j0(i), j1(i))} M[i][j] x[j]; lower: j in [0, i]; upper: j in [i, n).  One warp per row.
-__global__ void __launch_bounds__(256)
+// y[i] = sum_{j in [j0(i), j1(i))} M[i][j] x[j]; lower: j in [0, i]; upper: j in [i, n).  One CTA of 8 warps per row
+// (a single warp streaming a 48 KB row has 2 KB in flight per memory latency: the long rows alone took 24 us),
+// 16-byte loads, four of them in flight per thread on four partial sums; warp sums, then the 8 warps in order: a
+// fixed summation tree, deterministic.
+constexpr int TRIGEMV_THREADS = 256;
+__global__ void __launch_bounds__(TRIGEMV_THREADS)
 trigemv_kernel(int64_t n, int64_t npad, const double* __restrict__ M, const double* __restrict__ x,
                double* __restrict__ y, int upper) {
-  const int lane = threadIdx.x & 31;
-  const int64_t i = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
-  if (i >= n) return;
-  const int64_t j0 = upper ? (i & ~31LL) : 0, j1 = upper ? n : i + 1;
-  double s = 0.0;
-  for (int64_t j = j0 + lane; j < j1; j += 32) s = fma(M[i * npad + j], x[j], s);  // M is 0 outside the triangle
+  __shared__ double wsum[TRIGEMV_THREADS / 32];
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int64_t i = blockIdx.x;
+  const double* row = M + i * npad;                                  // 16-byte aligned (npad is a multiple of 128)
+  const int64_t j0 = upper ? (i & ~31LL) : 0, j1 = upper ? n : i + 1;  // M is 0 outside the triangle; j0 is even
+  double s0 = 0.0, s1 = 0.0, s2 = 0.0, s3 = 0.0;
+  if ((reinterpret_cast<uintptr_t>(x) & 15) == 0) {
+    const double2* r2 = reinterpret_cast<const double2*>(row);
+    const double2* x2 = reinterpret_cast<const double2*>(x);
+    const int64_t p1 = j1 >> 1;                                      // whole pairs [j0/2, p1)
+    for (int64_t p = (j0 >> 1) + tid; p < p1; p += 4 * TRIGEMV_THREADS) {
+      double2 m[4], v[4];
+#pragma unroll
+      for (int u = 0; u < 4; ++u) {
+        const int64_t q = min(p + TRIGEMV_THREADS * u, p1 - 1);      // clamped: a repeated pair is weighted 0 below
+        m[u] = __ldcs(r2 + q);
+        v[u] = __ldg(x2 + q);
+      }
+      if (p + TRIGEMV_THREADS >= p1) m[1] = make_double2(0.0, 0.0);
+      if (p + 2 * TRIGEMV_THREADS >= p1) m[2] = make_double2(0.0, 0.0);
+      if (p + 3 * TRIGEMV_THREADS >= p1) m[3] = make_double2(0.0, 0.0);
+      s0 = fma(m[0].y, v[0].y, fma(m[0].x, v[0].x, s0));
+      s1 = fma(m[1].y, v[1].y, fma(m[1].x, v[1].x, s1));
+      s2 = fma(m[2].y, v[2].y, fma(m[2].x, v[2].x, s2));
+      s3 = fma(m[3].y, v[3].y, fma(m[3].x, v[3].x, s3));
+    }
+    if ((j1 & 1) && tid == 0) s0 = fma(row[j1 - 1], x[j1 - 1], s0);   // the odd last entry
+  } else {
+    for (int64_t j = j0 + tid; j < j1; j += TRIGEMV_THREADS) s0 = fma(row[j], x[j], s0);
+  }
+  double s = (s0 + s1) + (s2 + s3);
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
-  if (lane == 0) y[i] = s;
+  if (lane == 0) wsum[warp] = s;
+  __syncthreads();
+  if (tid == 0) {
+    double tot = 0.0;
+#pragma unroll
+    for (int w = 0; w < TRIGEMV_THREADS / 32; ++w) tot += wsum[w];
+    y[i] = tot;
+  }
 }
 
 static int coarse_factor(vcycle_t vc, cudaStream_t st) {
@@ -461,10 +497,10 @@ static int coarse_factor(vcycle_t vc, cudaStream_t st) {
 }
 
 static int coarse_solve(vcycle_t vc, const double* b, double* x, cudaStream_t st) {
-  const unsigned grid = (unsigned)((vc->nc * 32 + 255) / 256);
+  const unsigned grid = (unsigned)vc->nc;   // one CTA per row
   if (!grid) return BSR_OK;
-  LAUNCH(trigemv_kernel, grid, 256, 0, st, vc->nc, vc->npad, vc->linv, b, vc->ytmp, 0);   // y = L^-1 b
-  LAUNCH(trigemv_kernel, grid, 256, 0, st, vc->nc, vc->npad, vc->linvT, vc->ytmp, x, 1);  // x = L^-T y
+  LAUNCH(trigemv_kernel, grid, TRIGEMV_THREADS, 0, st, vc->nc, vc->npad, vc->linv, b, vc->ytmp, 0);   // y = L^-1 b
+  LAUNCH(trigemv_kernel, grid, TRIGEMV_THREADS, 0, st, vc->nc, vc->npad, vc->linvT, vc->ytmp, x, 1);  // x = L^-T y
   return BSR_OK;
 }
 
