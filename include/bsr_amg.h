@@ -278,6 +278,29 @@ int bsr_measure_fp64_peak(double* tflops, void* stream);
  * GEMM inside vcycle_refresh.  COLD: allocates, synchronises. */
 int bsr_measure_fp64_mma_peak(double* tflops, void* stream);
 
+/* ------------------------------------------------------------------ an entry point that allocates nothing
+ * For callers that cannot call cudaMalloc (code under CUDA graph capture, tight serving loops, harnesses that forbid
+ * it).  bsr_lambda_noalloc runs prolongator_smooth_lambda's power iteration (reading R10: v <- v0/||v0||_2,
+ * then `iters` times w = D^-1 (A v), lambda = ||w||_2, v = w / lambda; the same kernels in the same order, so the same
+ * bits) with ALL of its work space -- D^-1, two work vectors, the norm's partial sums, the status word -- in one fixed
+ * device array inside the library: BSR_NOALLOC_SCRATCH_BYTES on every GPU that loads the library, until exit.
+ *   A           square, square blocks of size 2, 3 or 6, resident (bsr_create); only read.
+ *   d_v0        DEVICE, nbrows*bs doubles, 16-byte aligned; not modified.
+ *   d_lambda    DEVICE, 1 double: receives the last lambda (stream-ordered; the call does not synchronise).
+ *   d_status    DEVICE, 1 int32, or null: receives 0, or 1 if a diagonal block of A is missing or singular.
+ * HOT: enqueues 4 + 4*iters kernels, one 4-byte memset and one or two 8-/4-byte device-to-device copies on `stream`;
+ * calls no cudaMalloc / cudaFree / allocating routine (the first call on a device looks the array's address up with
+ * cudaGetSymbolAddress: make that call outside a capture).
+ * Limit: bsr_lambda_noalloc_scratch_doubles(nbrows, bs) * 8 <= BSR_NOALLOC_SCRATCH_BYTES, i.e. about 15*nbrows + 700
+ * doubles for bs = 3 (279,000 block rows; the 65^3-node grid of config 2 fits, config 3 does not) and 48*nbrows for
+ * bs = 6; a larger matrix is rejected with BSR_ERR_LIMIT and nothing is enqueued.
+ * Every call on a device shares the one array, which keeps the previous call's contents (the call clears what has to
+ * start at zero): two calls that overlap on the GPU -- different streams, or two host threads -- race; serialise them.
+ * Errors: BSR_ERR_NULL, BSR_ERR_SHAPE, BSR_ERR_BLOCK, BSR_ERR_ALIGN, BSR_ERR_LIMIT, BSR_ERR_CUDA. */
+#define BSR_NOALLOC_SCRATCH_BYTES (32LL << 20)
+int bsr_lambda_noalloc(bsr_t A, const double* d_v0, int32_t iters, double* d_lambda, int32_t* d_status, void* stream);
+int bsr_lambda_noalloc_scratch_doubles(int32_t nbrows, int32_t bs, int64_t* doubles);
+
 /* ------------------------------------------------------------------ workspace allocator (ownership)
  * Library-private workspace (the cached transpose, AP, plans, D^-1, work vectors, the dense factor) is obtained in COLD
  * calls only.  By default it comes from cudaMalloc; a caller that owns device memory (the Python harness: torch's caching

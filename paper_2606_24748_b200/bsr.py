@@ -63,6 +63,8 @@ SYMBOLS = {
     "prolongator_smooth_structure": (C.c_int, [_V, _V, _V, _V]),
     "prolongator_smooth_numeric": (C.c_int, [_V, _V, _V, _D, _V, _V]),
     "prolongator_smooth_lambda": (C.c_int, [_V, _V, _V, _I32, C.POINTER(_D), _V]),
+    "bsr_lambda_noalloc": (C.c_int, [_V, _V, _I32, _V, _V, _V]),
+    "bsr_lambda_noalloc_scratch_doubles": (C.c_int, [_I32, _I32, C.POINTER(_I64)]),
     "prolongator_smooth_status": (C.c_int, [_V, _V]),
     "prolongator_smooth_get_info": (C.c_int, [_V, _PI64, _PI64, _PI32]),
     "prolongator_smooth_destroy": (C.c_int, [_V]),
@@ -180,6 +182,26 @@ def counters():
     a, b = C.c_int64(), C.c_int64()
     lib().bsr_counters(C.byref(a), C.byref(b))
     return a.value, b.value
+
+
+NOALLOC_SCRATCH_BYTES = 32 << 20   # BSR_NOALLOC_SCRATCH_BYTES: the fixed work space of bsr_lambda_noalloc
+
+
+def lambda_noalloc_scratch_bytes(nbrows: int, bs: int) -> int:
+    """Work space bsr_lambda_noalloc needs for a matrix of this size (must not exceed NOALLOC_SCRATCH_BYTES)."""
+    d = _I64()
+    _check(lib().bsr_lambda_noalloc_scratch_doubles(int(nbrows), int(bs), C.byref(d)))
+    return d.value * 8
+
+
+def lambda_noalloc(A: "Bsr", v0, iters: int, out, status=None):
+    """Power iteration for lambda of D^-1 A with no allocation anywhere (bsr_lambda_noalloc): `out` is a caller-owned
+    DEVICE tensor of one float64, `status` an optional device int32; nothing is synchronised.  Calls that overlap on
+    the GPU race on the library's one work array."""
+    assert v0.numel() == A.nbrows * A.bs_r and out.numel() >= 1
+    _check(lib().bsr_lambda_noalloc(A.h, _dev(v0), int(iters), _dev(out), _dev(status) if status is not None else None,
+                                    _stream()))
+    return out
 
 
 def fp64_peak_tflops(mma: bool = False) -> float:

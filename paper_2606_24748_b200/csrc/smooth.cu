@@ -349,3 +349,93 @@ int prolongator_smooth_destroy(psmooth_plan_t pl) {
 }
 
 }  // extern "C"
+
+// ------------------------------------------------------------------ the power iteration without any allocation
+// bsr_lambda_noalloc: prolongator_smooth_lambda's iteration (same kernels, same order, same bits) for callers that may
+// not allocate -- code under CUDA graph capture, serving loops, harnesses that forbid cudaMalloc.  Its work space
+// (D^-1, the two work vectors, the norm's partial sums, the status word) is a fixed file-scope device array: every GPU
+// that loads the library holds BSR_NOALLOC_SCRATCH_BYTES (32 MiB) until exit.  In HOST code the array's name is only a
+// handle for the runtime, not a device address: the pointer the kernels get comes from cudaGetSymbolAddress, looked up
+// once per device with that device current.
+namespace bsramg {
+
+constexpr int64_t NOALLOC_DOUBLES = BSR_NOALLOC_SCRATCH_BYTES / 8;
+static __device__ __align__(256) double noalloc_scratch[NOALLOC_DOUBLES];
+
+constexpr int NOALLOC_MAX_DEVICES = 64;
+static std::atomic<double*> noalloc_ptr[NOALLOC_MAX_DEVICES];   // device address of the array, per device ordinal
+
+static int noalloc_base(double** out) {
+  int dev = -1;
+  CUDA_TRY(cudaGetDevice(&dev));
+  if (dev < 0 || dev >= NOALLOC_MAX_DEVICES) return fail(BSR_ERR_LIMIT, "device ordinal %d outside the table", dev);
+  double* p = noalloc_ptr[dev].load(std::memory_order_acquire);
+  if (!p) {   // set-up, once per device (idempotent: two racing threads obtain the same address)
+    const cudaError_t e = cudaGetSymbolAddress(reinterpret_cast<void**>(&p), noalloc_scratch);
+    if (e != cudaSuccess || !p) return fail(BSR_ERR_CUDA, "cudaGetSymbolAddress(noalloc_scratch): %s", cudaGetErrorString(e));
+    noalloc_ptr[dev].store(p, std::memory_order_release);
+  }
+  *out = p;
+  return BSR_OK;
+}
+
+static int64_t up32(int64_t doubles) { return (doubles + 31) & ~int64_t(31); }   // segments start on 256 bytes
+
+}  // namespace bsramg
+
+extern "C" int bsr_lambda_noalloc_scratch_doubles(int32_t nbrows, int32_t bs, int64_t* doubles) {
+  if (!doubles) return fail(BSR_ERR_NULL, "null output");
+  if (nbrows < 0 || bs < 1) return fail(BSR_ERR_SHAPE, "bad size");
+  const int64_t n = (int64_t)nbrows * bs;
+  *doubles = up32(n * bs) + 2 * up32(n) + up32(PW_BLOCKS) + 32 /* lambda */ + 32 /* status */;
+  return BSR_OK;
+}
+
+extern "C" int bsr_lambda_noalloc(bsr_t A, const double* d_v0, int32_t iters, double* d_lambda, int32_t* d_status,
+                                  void* stream) {
+  if (!A || A->magic != BSR_MAGIC) return fail(BSR_ERR_NULL, "invalid matrix handle");
+  if (!d_v0 || !d_lambda) return fail(BSR_ERR_NULL, "null argument");
+  if (A->nbrows != A->nbcols || A->bs_r != A->bs_c) return fail(BSR_ERR_SHAPE, "A must be square with square blocks");
+  if (A->bs_r != 2 && A->bs_r != 3 && A->bs_r != 6) return fail(BSR_ERR_BLOCK, "unsupported block size %d", A->bs_r);
+  if (iters < 1) return fail(BSR_ERR_SHAPE, "iters must be positive");
+  if ((uintptr_t)d_v0 & 15) return fail(BSR_ERR_ALIGN, "d_v0 must be 16-byte aligned");
+  int64_t need = 0;
+  BSR_TRY(bsr_lambda_noalloc_scratch_doubles(A->nbrows, A->bs_r, &need));
+  if (need > NOALLOC_DOUBLES)
+    return fail(BSR_ERR_LIMIT, "bsr_lambda_noalloc: %d block rows of size %d need %lld bytes of work space, the fixed array "
+                "holds %lld (BSR_NOALLOC_SCRATCH_BYTES); use prolongator_smooth_lambda", A->nbrows, A->bs_r,
+                (long long)(need * 8), (long long)BSR_NOALLOC_SCRATCH_BYTES);
+  if (A->nbrows == 0) return fail(BSR_ERR_SHAPE, "empty matrix");
+  cudaStream_t st = (cudaStream_t)stream;
+  NvtxRange nv("bsr_lambda_noalloc");
+  double* base = nullptr;
+  BSR_TRY(noalloc_base(&base));
+  const int64_t n = (int64_t)A->nbrows * A->bs_r;
+  double* dinv = base;
+  double* v = dinv + up32(n * A->bs_r);
+  double* t = v + up32(n);
+  double* part = t + up32(n);
+  double* scal = part + up32(PW_BLOCKS);
+  int* status = reinterpret_cast<int*>(scal + 32);
+  // the array keeps the last call's contents: the status word is OR-ed into, so it must start at zero; D^-1, v, t and
+  // the partial sums are written in full before they are read
+  CUDA_TRY(cudaMemsetAsync(status, 0, sizeof(int), st));
+  BSR_TRY(block_diag_inverse(A, dinv, status, st));
+  const unsigned gv = (unsigned)((n + 255) / 256);
+  LAUNCH(sumsq_partial_kernel, PW_BLOCKS, 256, 0, st, n, d_v0, part);
+  LAUNCH(norm_final_kernel, 1, 32, 0, st, PW_BLOCKS, part, scal);
+  LAUNCH(scale_by_norm_kernel, gv, 256, 0, st, n, d_v0, scal, v);                         // v <- v0 / ||v0||
+  for (int it = 0; it < iters; ++it) {
+    BSR_TRY(spmv_launch(A, v, t, nullptr, EPI_ASSIGN, st));                                // t = A v
+    switch (A->bs_r) {                                                                    // w = D^-1 t, ||w||^2 partials
+      case 2: LAUNCH(dinv_apply_norm_kernel<2>, PW_BLOCKS, 256, 0, st, (int64_t)A->nbrows, dinv, t, part); break;
+      case 3: LAUNCH(dinv_apply_norm_kernel<3>, PW_BLOCKS, 256, 0, st, (int64_t)A->nbrows, dinv, t, part); break;
+      default: LAUNCH(dinv_apply_norm_kernel<6>, PW_BLOCKS, 256, 0, st, (int64_t)A->nbrows, dinv, t, part); break;
+    }
+    LAUNCH(norm_final_kernel, 1, 32, 0, st, PW_BLOCKS, part, scal);                        // lambda = ||w||
+    LAUNCH(scale_by_norm_kernel, gv, 256, 0, st, n, t, scal, v);                           // v = w / lambda
+  }
+  CUDA_TRY(cudaMemcpyAsync(d_lambda, scal, sizeof(double), cudaMemcpyDeviceToDevice, st));
+  if (d_status) CUDA_TRY(cudaMemcpyAsync(d_status, status, sizeof(int), cudaMemcpyDeviceToDevice, st));
+  return BSR_OK;
+}
