@@ -323,10 +323,13 @@ potrf_panel_kernel(int64_t npad, int J, double* __restrict__ dense, double* __re
   const int group = warp >> 2, qm = ((warp >> 1) & 1) * 16, qn = (warp & 1) * 16;   // two groups of four warps
   double* blk = dense + ((int64_t)J * PANEL) * npad + (int64_t)J * PANEL;
   double* xblk = linv + ((int64_t)J * PANEL) * npad + (int64_t)J * PANEL;
-  for (int e = tid; e < PTILES * TS * TS; e += 256) {
-    const int tl = e >> 10, r = (e >> 5) & 31, c = e & 31;
+  // 16-byte accesses: PL is even and npad a multiple of 128, so every tile row starts on 16 bytes on both sides
+#pragma unroll 4
+  for (int e = tid; e < PTILES * TS * TS / 2; e += 256) {
+    const int tl = e >> 9, r = (e >> 4) & 31, c = (e & 15) * 2;
     const int ti = (tl >= 6) ? 3 : (tl >= 3) ? 2 : (tl >= 1) ? 1 : 0, tj = tl - ti * (ti + 1) / 2;
-    Lt[tl * TS * PL + r * PL + c] = blk[(int64_t)(ti * TS + r) * npad + tj * TS + c];
+    *reinterpret_cast<double2*>(Lt + tl * TS * PL + r * PL + c) =
+        *reinterpret_cast<const double2*>(blk + (int64_t)(ti * TS + r) * npad + tj * TS + c);
   }
   __syncthreads();
   for (int s = 0; s < PT; ++s) {
@@ -370,11 +373,13 @@ potrf_panel_kernel(int64_t npad, int J, double* __restrict__ dense, double* __re
       __syncthreads();
     }
   }
-  for (int e = tid; e < PTILES * TS * TS; e += 256) {
-    const int tl = e >> 10, r = (e >> 5) & 31, c = e & 31;
+#pragma unroll 4
+  for (int e = tid; e < PTILES * TS * TS / 2; e += 256) {
+    const int tl = e >> 9, r = (e >> 4) & 31, c = (e & 15) * 2;
     const int ti = (tl >= 6) ? 3 : (tl >= 3) ? 2 : (tl >= 1) ? 1 : 0, tj = tl - ti * (ti + 1) / 2;
-    blk[(int64_t)(ti * TS + r) * npad + tj * TS + c] = Lt[tl * TS * PL + r * PL + c];
-    xblk[(int64_t)(ti * TS + r) * npad + tj * TS + c] = Xt[tl * TS * PL + r * PL + c];
+    const int64_t g = (int64_t)(ti * TS + r) * npad + tj * TS + c;
+    *reinterpret_cast<double2*>(blk + g) = *reinterpret_cast<const double2*>(Lt + tl * TS * PL + r * PL + c);
+    *reinterpret_cast<double2*>(xblk + g) = *reinterpret_cast<const double2*>(Xt + tl * TS * PL + r * PL + c);
   }
 }
 
@@ -382,6 +387,7 @@ __global__ void __launch_bounds__(TS * TS)
 transpose_tile_kernel(int64_t npad, const double* __restrict__ src, double* __restrict__ dst) {
   __shared__ double t[TS][TS + 1];
   const int tx = threadIdx.x, ty = threadIdx.y;
+  if (blockIdx.x > blockIdx.y) return;   // src is lower triangular: its upper tiles are zero and dst's lower tiles are never read
   t[ty][tx] = src[((int64_t)blockIdx.y * TS + ty) * npad + (int64_t)blockIdx.x * TS + tx];
   __syncthreads();
   dst[((int64_t)blockIdx.x * TS + ty) * npad + (int64_t)blockIdx.y * TS + tx] = t[tx][ty];
