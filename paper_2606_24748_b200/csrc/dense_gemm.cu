@@ -16,7 +16,7 @@ namespace bsramg {
 
 constexpr int GK = 16;   // k-chunk
 
-// GT: the CTA's tile (128, or 64 for launches that would leave most SMs without a 128-tile); 2 GT threads
+// GT: the CTA's tile (128; 64 or 32 for launches that would leave most SMs without a larger tile); 2 GT threads
 template <int GT, bool TRANSB>
 __global__ void __launch_bounds__(2 * GT)
 dgemm128_kernel(int k, double alpha, const double* __restrict__ A, int64_t lda, const double* __restrict__ B,
@@ -119,15 +119,16 @@ int dgemm128(bool transB, int m, int n, int k, double alpha, const double* A, in
     return fail(BSR_ERR_SHAPE, "dgemm128: sizes must be multiples of the tile (m %d n %d k %d)", m, n, k);
   if (kcap <= 0 || kcap > k) kcap = k;
   if (koff < -(1 << 29)) koff = -(1 << 29);
-  // fewer 128-tiles than SMs: quarter tiles, four times the CTAs (a 128-tile is ~17 us of one SM's fp64 rate per 128 k)
-  const int64_t t128 = (int64_t)(m / 128) * (tri ? (n / 128 + 1) / 2 : n / 128) * batch;
-  const bool small = t128 < 148;
-  const int gt = small ? 64 : 128;
+  // a tile runs on ONE SM (64 fp64 FMAs per clock: a 64x64x128 tile is 4 us of arithmetic alone): take the largest tile
+  // that still gives every SM one
+  auto tiles = [&](int gt) { return (int64_t)(m / gt) * (tri ? (n / gt + 1) / 2 : n / gt) * batch; };
+  const int gt = tiles(128) >= 148 ? 128 : tiles(64) >= 148 ? 64 : 32;
   const dim3 grid((unsigned)(n / gt), (unsigned)(m / gt), (unsigned)batch);
 #define DGEMM_LAUNCH(GT, TB) \
   LAUNCH((dgemm128_kernel<GT, TB>), grid, 2 * GT, 0, st, k, alpha, A, lda, B, ldb, beta, C, ldc, sA, sB, sC, tri, klim, koff, kcap)
-  if (small) { if (transB) DGEMM_LAUNCH(64, true); else DGEMM_LAUNCH(64, false); }
-  else       { if (transB) DGEMM_LAUNCH(128, true); else DGEMM_LAUNCH(128, false); }
+  if (gt == 32)      { if (transB) DGEMM_LAUNCH(32, true); else DGEMM_LAUNCH(32, false); }
+  else if (gt == 64) { if (transB) DGEMM_LAUNCH(64, true); else DGEMM_LAUNCH(64, false); }
+  else               { if (transB) DGEMM_LAUNCH(128, true); else DGEMM_LAUNCH(128, false); }
 #undef DGEMM_LAUNCH
   return BSR_OK;
 }
